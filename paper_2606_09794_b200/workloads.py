@@ -1,0 +1,129 @@
+"""Seeded synthetic workloads (the five BASELINE.json configs).
+
+This module holds NO arithmetic of the method: it only draws the random inputs that both the
+CUDA path and the independent fp64 oracle consume (SURVEY.md section
+8(d)). Every array is drawn from its own PCG64 sub-stream ``default_rng([seed, tag])`` and cast to
+fp32 (uint8 for the mask) before either implementation sees it.
+
+Shapes follow the boundary in ``include/nasg.h``:
+  means [N,3] · quat [K,N,4] (w,x,y,z) · shape [K,N,4] = (log Lambda, log lambda, k, phi)
+  amp [K,3,N] · dc [3,N] · campos [C,3] · vis [C,N] uint8 or None · g_colors [C,N,3]
+  SH: coeffs [16,3,N]
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+
+# sub-stream tags (one independent stream per array)
+TAG_MEANS, TAG_CAMPOS, TAG_VIS, TAG_QUAT, TAG_BW, TAG_FREQ, TAG_PHASE = 0, 1, 2, 3, 4, 5, 6
+TAG_AMP, TAG_DC, TAG_GCOL, TAG_SH = 7, 8, 9, 10
+
+
+@dataclass(frozen=True)
+class Config:
+    """One BASELINE.json config. ``kind`` is "nasg" or "sh"."""
+    index: int
+    kind: str
+    seed: int
+    N: int
+    K: int            # lobes (0 for SH)
+    C: int            # cameras
+    fixed_campos: bool
+    vis_p: Optional[float]      # Bernoulli probability, None = all visible (vis pointer NULL)
+    bw_range: tuple             # log-bandwidth range
+    k_range: tuple              # Gabor frequency range
+    name: str
+
+
+CONFIGS = (
+    Config(0, "nasg", 0, 10_000, 2, 1, True, None, (0.0, 5.0), (0.0, 8.0), "cfg0 N=1e4 K=2 C=1"),
+    Config(1, "nasg", 1, 1_000_000, 4, 1, False, None, (0.0, 5.0), (0.0, 8.0), "cfg1 N=1e6 K=4 C=1"),
+    Config(2, "nasg", 2, 3_000_000, 4, 4, False, 0.6, (0.0, 5.0), (0.0, 8.0),
+           "cfg2 N=3e6 K=4 C=4 vis~Bern(0.6)"),
+    Config(3, "sh", 2, 3_000_000, 0, 4, False, 0.6, (0.0, 5.0), (0.0, 8.0),
+           "cfg3 SH-3 N=3e6 C=4 vis~Bern(0.6)"),
+    Config(4, "nasg", 4, 6_000_000, 8, 1, False, None, (3.0, 8.0), (4.0, 16.0),
+           "cfg4 N=6e6 K=8 C=1 high-frequency"),
+)
+
+
+def _rng(seed: int, tag: int) -> np.random.Generator:
+    return np.random.Generator(np.random.PCG64([seed, tag]))
+
+
+def make_geometry(cfg: Config, N: Optional[int] = None) -> dict:
+    """means, campos, vis, g_colors: the arrays config 3 shares with config 2 (same seed/tags)."""
+    N = cfg.N if N is None else int(N)
+    C = cfg.C
+    means = _rng(cfg.seed, TAG_MEANS).uniform(-1.0, 1.0, size=(N, 3)).astype(np.float32)
+    if cfg.fixed_campos:
+        campos = np.array([[0.0, 0.0, 4.0]], dtype=np.float32)
+    else:
+        g = _rng(cfg.seed, TAG_CAMPOS).standard_normal(size=(C, 3))
+        campos = (4.0 * g / np.linalg.norm(g, axis=1, keepdims=True)).astype(np.float32)
+    if cfg.vis_p is None:
+        vis = None
+    else:
+        vis = (_rng(cfg.seed, TAG_VIS).random(size=(C, N)) < cfg.vis_p).astype(np.uint8)
+    g_colors = _rng(cfg.seed, TAG_GCOL).standard_normal(size=(C, N, 3)).astype(np.float32)
+    return dict(N=N, C=C, means=means, campos=campos, vis=vis, g_colors=g_colors)
+
+
+def make_nasg(cfg: Config, N: Optional[int] = None) -> dict:
+    """Inputs of nasg_eval_fwd/bwd for a NASGabor config."""
+    assert cfg.kind == "nasg"
+    out = make_geometry(cfg, N)
+    N, K = out["N"], cfg.K
+    q = _rng(cfg.seed, TAG_QUAT).standard_normal(size=(K, N, 4))
+    q /= np.linalg.norm(q, axis=2, keepdims=True)
+    b = _rng(cfg.seed, TAG_BW).uniform(cfg.bw_range[0], cfg.bw_range[1], size=(K, N, 2))
+    shape = np.empty((K, N, 4), dtype=np.float64)
+    shape[..., 0] = b.max(axis=2)      # log Lambda: first bandwidth (>= second)
+    shape[..., 1] = b.min(axis=2)      # log lambda
+    shape[..., 2] = _rng(cfg.seed, TAG_FREQ).uniform(cfg.k_range[0], cfg.k_range[1], size=(K, N))
+    shape[..., 3] = _rng(cfg.seed, TAG_PHASE).uniform(0.0, 2.0 * np.pi, size=(K, N))
+    amp = _rng(cfg.seed, TAG_AMP).normal(0.0, 0.3, size=(K, 3, N))
+    dc = _rng(cfg.seed, TAG_DC).normal(0.0, 0.3, size=(3, N))
+    out.update(K=K, quat=q.astype(np.float32), shape=shape.astype(np.float32),
+               amp=amp.astype(np.float32), dc=dc.astype(np.float32))
+    return out
+
+
+def make_sh(cfg: Config, N: Optional[int] = None) -> dict:
+    """Inputs of sh_eval_fwd/bwd (config 3): geometry of config 2 plus degree-3 coefficients."""
+    assert cfg.kind == "sh"
+    out = make_geometry(cfg, N)
+    N = out["N"]
+    coeffs = _rng(cfg.seed, TAG_SH).normal(0.0, 0.2, size=(16, 3, N))
+    coeffs[0] += 0.5                   # DC band ~ N(0.5, 0.2)
+    out.update(coeffs=coeffs.astype(np.float32))
+    return out
+
+
+def make(cfg_index: int, N: Optional[int] = None) -> dict:
+    cfg = CONFIGS[cfg_index]
+    return make_nasg(cfg, N) if cfg.kind == "nasg" else make_sh(cfg, N)
+
+
+def take(inp: dict, idx: np.ndarray) -> dict:
+    """Gather a subset of Gaussians (per-Gaussian independent path): used to check sampled
+    outputs of a full-size run against the oracle."""
+    idx = np.asarray(idx, dtype=np.int64)
+    out = dict(inp)
+    out["N"] = int(idx.size)
+    out["means"] = np.ascontiguousarray(inp["means"][idx])
+    out["g_colors"] = np.ascontiguousarray(inp["g_colors"][:, idx])
+    if inp.get("vis") is not None:
+        out["vis"] = np.ascontiguousarray(inp["vis"][:, idx])
+    for key in ("quat", "shape"):
+        if key in inp:
+            out[key] = np.ascontiguousarray(inp[key][:, idx])
+    for key in ("amp", "coeffs"):
+        if key in inp:
+            out[key] = np.ascontiguousarray(inp[key][:, :, idx])
+    if "dc" in inp:
+        out["dc"] = np.ascontiguousarray(inp["dc"][:, idx])
+    return out

@@ -1,0 +1,427 @@
+"""Pins of the fp64 oracle against what the paper and the mathematics fix (CPU only).
+
+Nothing here compares the oracle with itself or with the CUDA path. Each test names the passage
+of /root/reference/PAPER.md it pins (file:line + equation) and the plausible mistake it catches.
+"""
+import mpmath as mp
+import numpy as np
+import pytest
+import scipy.special
+import scipy.stats
+
+from quadrature import sphere_integral_of_G
+
+TWO_PI = 2.0 * np.pi
+
+
+# ------------------------------------------------------------------------------------------
+# P1-P3: eq.(9) integrated over the sphere versus the closed forms
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("lam,a", [(0.5, 4.0), (1.0, 0.0), (3.0, 1.0), (7.4, 19.0), (20.0, 0.3),
+                                   (55.0, 1.7), (148.0, 0.01)])
+def test_P1_envelope_integral_is_nasg_normaliser(oracle, lam, a):
+    """k = 0, phi = 0: quadrature of eq.(9) == 2 pi (1-e^{-2 lambda})/(lambda sqrt(1+a))  (Table 6,
+    PAPER.md:423), in BOTH norm modes (eq.(10) 'becoming exact at k = 0').
+    Catches: wrong kappa/tau, wrong exponent sign, missing sqrt(1+a), Psi(k=0) != 1."""
+    for mode in (0, 1):
+        assert abs(sphere_integral_of_G(oracle, lam, a, 0.0, 0.0, mode) - 1.0) < 1e-9
+    closed = TWO_PI * (1.0 - np.exp(-2.0 * lam)) / (lam * np.sqrt(1.0 + a))
+    assert abs(oracle.integral(lam, a, 0.0, 0) / closed - 1.0) < 1e-14
+    assert abs(oracle.integral(lam, a, 0.0, 1) / closed - 1.0) < 1e-14
+
+
+@pytest.mark.parametrize("lam,k", [(1.0, 3.0), (3.0, 2.0), (3.0, 3.0 - 1e-7), (5.0, 7.5), (20.0, 8.0),
+                                   (2.0, 16.0), (60.0, 16.0)])
+def test_P2_eq10_exact_at_zero_anisotropy(oracle, lam, k):
+    """a = 0, phi = 0, any k on both sides of k = Lambda: eq.(10) == quadrature of eq.(9).
+    Catches: sinh instead of sinhc (reading R3), wrong continuation for k > Lambda (R4), a wrong
+    factor 2 or e^{-Lambda} in Psi."""
+    assert abs(sphere_integral_of_G(oracle, lam, 0.0, k, 0.0, 1) - 1.0) < 2e-9
+
+
+@pytest.mark.parametrize("phi", [0.7, 2.0, 3.1, 5.5])
+def test_P2_phase_enters_only_the_carrier(oracle, phi):
+    """Reading R5: H = (1+cos(k u + phi))/2, normaliser eq.(10) without phi. At a = 0 the exact
+    integral with a phase is base (1 + cos(phi) Psi) (the sin part is odd in u), so the oracle's
+    normalised lobe must integrate to (1 + cos(phi) Psi)/(1 + Psi). Pins the sign and place of phi."""
+    lam, k = 2.5, 3.0
+    Psi = oracle.psi(lam, k)[0]
+    want = (1.0 + np.cos(phi) * Psi) / (1.0 + Psi)
+    assert abs(sphere_integral_of_G(oracle, lam, 0.0, k, phi, 1) - want) < 2e-9
+
+
+def test_P3_eq10_is_only_approximate_for_anisotropic_lobes(oracle):
+    """DESIGN.md R2: eq.(10) as printed is NOT the integral of eq.(9) when a > 0 and k > 0. The
+    oracle implements it as printed; this test documents the size of the gap (eq10/quadrature - 1)
+    and that it closes as k -> 0."""
+    expect = {(3.0, 1.0, 2.0): -2.85e-3, (3.0, 2.0, 5.0): -1.69e-2, (1.0, 0.5, 4.0): -6.8e-2,
+              (0.5, 4.0, 6.0): -1.18e-1, (7.4, 19.0, 8.0): 9.1e-4, (55.0, 1.7, 8.0): 7.46e-5}
+    for (lam, a, k), dev in expect.items():
+        got = 1.0 / sphere_integral_of_G(oracle, lam, a, k, 0.0, 1) - 1.0
+        assert abs(got - dev) < 0.05 * abs(dev), (lam, a, k, got)
+    devs = [abs(1.0 / sphere_integral_of_G(oracle, 3.0, 1.0, k, 0.0, 1) - 1.0) for k in (2.0, 0.5, 0.1)]
+    assert devs[0] > devs[1] > devs[2] and devs[2] < 1e-5
+
+
+# ------------------------------------------------------------------------------------------
+# Psi of eq.(10) against the literal formula in 50-digit arithmetic
+# ------------------------------------------------------------------------------------------
+mp.mp.dps = 50
+
+
+def _psi_literal(Lam, k):
+    Lam, k = mp.mpf(Lam), mp.mpf(k)
+    s = Lam * Lam - k * k
+    r = mp.sqrt(s)                      # complex for k > Lambda; sinh(r)/r stays real
+    sinhc = mp.mpf(1) if s == 0 else mp.re(mp.sinh(r) / r)
+    return 2 * Lam * mp.exp(-Lam) * sinhc / (1 - mp.exp(-2 * Lam))
+
+
+@pytest.mark.parametrize("Lam,k", [(1.0, 0.0), (1.0, 0.5), (1.0, 1.0), (1.0, 1.0 + 1e-6), (1.0, 8.0),
+                                   (4.0, 3.999), (4.0, 4.001), (12.0, 16.0), (20.1, 4.0), (148.0, 8.0),
+                                   (700.0, 16.0), (2980.9, 16.0), (2980.9, 4.0), (0.3, 40.0),
+                                   (39.0, 40.0), (800.0, 900.0)])
+def test_psi_matches_literal_eq10(oracle, Lam, k):
+    """The overflow-safe rearrangement in psi_terms() equals the printed formula; derivatives equal
+    50-digit numerical differentiation. Catches a wrong branch, series or sign anywhere in Psi."""
+    P, PL, Pk = oracle.psi(Lam, k)
+    want = _psi_literal(Lam, k)
+    scale = max(abs(float(want)), 1e-300)
+    assert abs(P - float(want)) <= 2e-12 * scale + 1e-300
+    dL = mp.diff(lambda x: _psi_literal(x, k), mp.mpf(Lam))
+    dk = mp.diff(lambda x: _psi_literal(Lam, x), mp.mpf(k)) if k > 0 else mp.mpf(0)
+    # 1e-10: the oracle's fp64 Lam^2-k^2 near k = Lambda limits it, not the formula
+    assert abs(PL - float(dL)) <= 1e-9 * max(abs(float(dL)), scale) + 1e-300
+    assert abs(Pk - float(dk)) <= 1e-9 * max(abs(float(dk)), scale) + 1e-300
+
+
+def test_psi_is_one_at_zero_frequency(oracle):
+    """'becoming exact at k = 0' forces Psi(k=0) = 1, i.e. sinhc not sinh (R3)."""
+    for Lam in (0.2, 1.0, 7.0, 148.0, 2980.0):
+        assert abs(oracle.psi(Lam, 0.0)[0] - 1.0) < 1e-13
+
+
+# ------------------------------------------------------------------------------------------
+# P4: special cases that reduce to textbook / library functions
+# ------------------------------------------------------------------------------------------
+def _random_unit(rng, n):
+    x = rng.standard_normal((n, 3))
+    return x / np.linalg.norm(x, axis=1, keepdims=True)
+
+
+def test_P4_reduces_to_von_mises_fisher(oracle):
+    """k = 0, a = 0: G is the Spherical Gaussian lambda/(2 pi (1-e^{-2 lambda})) exp(lambda(z.d - 1))
+    (Table 6 first row) == scipy.stats.vonmises_fisher.pdf (library routine)."""
+    rng = np.random.default_rng(11)
+    N = 64
+    d = _random_unit(rng, N)
+    q = rng.standard_normal(4)
+    _, Z = oracle.frame(q)
+    for lam in (0.7, 4.0, 60.0):
+        inp = dict(N=N, K=1, C=1, means=3.0 * d + np.array([0.3, -0.2, 0.1]),
+                   campos=np.array([[0.3, -0.2, 0.1]]), quat=np.tile(q, (1, N, 1)),
+                   shape=np.tile([np.log(lam), np.log(lam), 0.0, 0.0], (1, N, 1)),
+                   amp=np.ones((1, 3, N)), dc=np.zeros((3, N)), vis=None)
+        want = scipy.stats.vonmises_fisher(Z / np.linalg.norm(Z), lam).pdf(d)
+        for mode in (0, 1):
+            got = oracle.nasg_fwd(inp, mode)[0, :, 1]
+            assert np.max(np.abs(got - want)) < 1e-12 * np.max(want)
+
+
+def test_P4_zero_frequency_is_nasg(oracle):
+    """k = 0, phi = 0: NASGabor == NASG of Table 6, written here in 40-digit mpmath
+    from the table row. Catches: kappa/tau mix-ups, wrong use of x vs y axis, a wrong normaliser."""
+    rng = np.random.default_rng(5)
+    for _ in range(12):
+        lam, a = float(np.exp(rng.uniform(-1, 4))), float(np.exp(rng.uniform(-3, 3)))
+        q = rng.standard_normal(4)
+        X, Z = oracle.frame(q)
+        d = _random_unit(rng, 1)[0]
+        u, v = mp.mpf(float(d @ X)), mp.mpf(float(d @ Z))
+        kappa = (v + 1) / 2
+        tau = mp.mpf(a) * u * u / (1 - v * v)
+        c = 2 * mp.pi * (1 - mp.exp(-2 * mp.mpf(lam))) / (mp.mpf(lam) * mp.sqrt(1 + mp.mpf(a)))
+        want = mp.exp(2 * lam * kappa ** (1 + tau) - 2 * lam) * kappa ** tau / c
+        inp = dict(N=1, K=1, C=1, means=d[None] * 2.5, campos=np.zeros((1, 3)), quat=q[None, None],
+                   shape=np.array([[[np.log(lam * (1 + a)), np.log(lam), 0.0, 0.0]]]),
+                   amp=np.ones((1, 3, 1)), dc=np.zeros((3, 1)), vis=None)
+        for mode in (0, 1):
+            got = oracle.nasg_fwd(inp, mode)[0, 0, 0]
+            assert abs(got - float(want)) <= 1e-11 * abs(float(want)) + 1e-300
+
+
+def test_frame_is_the_standard_rotation_matrix(oracle):
+    """R12: X, Z are columns 0 and 2 of the Hamilton rotation matrix of q/|q| == scipy Rotation."""
+    from scipy.spatial.transform import Rotation
+    rng = np.random.default_rng(2)
+    for _ in range(8):
+        q = rng.standard_normal(4) * rng.uniform(0.2, 3.0)
+        X, Z = oracle.frame(q)
+        R = Rotation.from_quat([q[1], q[2], q[3], q[0]]).as_matrix()   # scipy order is (x,y,z,w)
+        assert np.allclose(X, R[:, 0], atol=1e-14) and np.allclose(Z, R[:, 2], atol=1e-14)
+
+
+def test_appearance_model_eq6_and_layout(oracle):
+    """eq.(6): colour = c0 + sum_l w_l G_l, per channel; checks the [K,3,N]/[3,N]/[C,N,3]
+    indexing by building the sum from single-lobe, single-channel calls."""
+    from paper_2606_09794_b200 import workloads as W
+    inp = W.make(2, N=40)
+    full = oracle.nasg_fwd(inp)
+    acc = np.zeros_like(full)
+    for ch in range(3):
+        acc[:, :, ch] += inp["dc"][ch].astype(np.float64)[None, :]
+    for l in range(inp["K"]):
+        one = dict(inp, K=1, quat=inp["quat"][l:l + 1], shape=inp["shape"][l:l + 1],
+                   amp=np.ones((1, 3, 40)), dc=np.zeros((3, 40)))
+        G = oracle.nasg_fwd(one)[:, :, 0]
+        for ch in range(3):
+            acc[:, :, ch] += inp["amp"][l, ch].astype(np.float64)[None, :] * G
+    acc *= (inp["vis"] != 0)[:, :, None]
+    assert np.max(np.abs(acc - full)) < 1e-13 * np.max(np.abs(full))
+    assert np.all(full[inp["vis"] == 0] == 0.0)
+
+
+# ------------------------------------------------------------------------------------------
+# P5, P8: invariances and symmetries
+# ------------------------------------------------------------------------------------------
+def _quat_mul(r, q):
+    w1, x1, y1, z1 = r
+    w2, x2, y2, z2 = q[..., 0], q[..., 1], q[..., 2], q[..., 3]
+    return np.stack([w1 * w2 - x1 * x2 - y1 * y2 - z1 * z2, w1 * x2 + x1 * w2 + y1 * z2 - z1 * y2,
+                     w1 * y2 - x1 * z2 + y1 * w2 + z1 * x2, w1 * z2 + x1 * y2 - y1 * x2 + z1 * w2], -1)
+
+
+def test_P5_joint_rotation_invariance(oracle):
+    """G depends on d only through d.x and d.z: rotating the frame (q -> r*q),
+    the means and the cameras together leaves the colours unchanged and rotates g_means."""
+    from scipy.spatial.transform import Rotation
+    from paper_2606_09794_b200 import workloads as W
+    inp = {k: (v.astype(np.float64) if isinstance(v, np.ndarray) and v.dtype == np.float32 else v)
+           for k, v in W.make(2, N=200).items()}
+    r = np.array([0.3, -0.5, 0.7, 0.2]); r /= np.linalg.norm(r)
+    R = Rotation.from_quat([r[1], r[2], r[3], r[0]]).as_matrix()
+    rot = dict(inp, means=inp["means"] @ R.T, campos=inp["campos"] @ R.T, quat=_quat_mul(r, inp["quat"]))
+    c0, c1 = oracle.nasg_fwd(inp), oracle.nasg_fwd(rot)
+    assert np.max(np.abs(c0 - c1)) < 1e-11 * np.max(np.abs(c0))
+    g0, g1 = oracle.nasg_bwd(inp), oracle.nasg_bwd(rot)
+    assert np.max(np.abs(g0["g_means"] @ R.T - g1["g_means"])) < 1e-10 * np.max(np.abs(g0["g_means"]))
+    for key in ("g_shape", "g_amp", "g_dc"):
+        assert np.max(np.abs(g0[key] - g1[key])) < 1e-10 * np.max(np.abs(g0[key]))
+
+
+def test_P8_symmetries(oracle):
+    from paper_2606_09794_b200 import workloads as W
+    inp = {k: (v.astype(np.float64) if isinstance(v, np.ndarray) and v.dtype == np.float32 else v)
+           for k, v in W.make(2, N=300).items()}
+    base = oracle.nasg_fwd(inp)
+    tol = 1e-12 * np.max(np.abs(base))
+    # q -> -q is the same rotation
+    assert np.max(np.abs(oracle.nasg_fwd(dict(inp, quat=-inp["quat"])) - base)) < tol
+    # an unnormalised quaternion gives the same frame (library normalises)
+    assert np.max(np.abs(oracle.nasg_fwd(dict(inp, quat=2.5 * inp["quat"])) - base)) < tol
+    # phi -> phi + 2 pi
+    sh = inp["shape"].copy(); sh[..., 3] += TWO_PI
+    assert np.max(np.abs(oracle.nasg_fwd(dict(inp, shape=sh)) - base)) < 1e-11 * np.max(np.abs(base))
+    # turn the frame by pi about Z (X -> -X) and flip the phase: q -> q * (0,0,0,1), phi -> -phi
+    q = inp["quat"]
+    qz = np.stack([-q[..., 3], q[..., 2], -q[..., 1], q[..., 0]], -1)     # q (x) (0,0,0,1)
+    X0, Z0 = oracle.frame(q[0, 0]); X1, Z1 = oracle.frame(qz[0, 0])
+    assert np.allclose(X1, -X0) and np.allclose(Z1, Z0)
+    sh = inp["shape"].copy(); sh[..., 3] *= -1.0
+    assert np.max(np.abs(oracle.nasg_fwd(dict(inp, quat=qz, shape=sh)) - base)) < tol
+    # linearity over cameras: a C-camera backward equals the sum of C single-camera backwards
+    g = oracle.nasg_bwd(inp)
+    acc = None
+    for c in range(inp["C"]):
+        one = dict(inp, C=1, campos=inp["campos"][c:c + 1], vis=inp["vis"][c:c + 1],
+                   g_colors=inp["g_colors"][c:c + 1])
+        gc = oracle.nasg_bwd(one)
+        assert np.max(np.abs(gc["g_campos"][0] - g["g_campos"][c])) < 1e-10 * np.max(np.abs(g["g_campos"]))
+        gc.pop("g_campos")
+        acc = gc if acc is None else {k: acc[k] + gc[k] for k in acc}
+    for key, val in acc.items():
+        assert np.max(np.abs(val - g[key])) < 1e-12 * np.max(np.abs(g[key])), key
+    # a Gaussian culled in every camera has exactly zero gradients
+    dead = np.all(inp["vis"] == 0, axis=0)
+    assert dead.any()
+    assert np.all(g["g_means"][dead] == 0) and np.all(g["g_quat"][:, dead] == 0)
+    assert np.all(g["g_amp"][:, :, dead] == 0) and np.all(g["g_dc"][:, dead] == 0)
+
+
+# ------------------------------------------------------------------------------------------
+# P6: finite differences of sum(g_colors * colors), every input array, both normaliser modes
+# ------------------------------------------------------------------------------------------
+def _tiny(seed, cfg=2, N=5):
+    from paper_2606_09794_b200 import workloads as W
+    import dataclasses
+    cfg = dataclasses.replace(W.CONFIGS[cfg], seed=seed, K=3, C=2)
+    inp = W.make_nasg(cfg, N=N)
+    inp = {k: (v.astype(np.float64) if isinstance(v, np.ndarray) and v.dtype == np.float32 else v)
+           for k, v in inp.items()}
+    inp["quat"] = inp["quat"] * np.random.default_rng(seed).uniform(0.5, 2.0, size=inp["quat"].shape[:2] + (1,))
+    return inp
+
+
+@pytest.mark.parametrize("mode", [1, 0])
+@pytest.mark.parametrize("seed,cfg", [(100, 2), (101, 2), (102, 4)])
+def test_P6_finite_differences(oracle, mode, seed, cfg):
+    """Central differences (fp64, Richardson-extrapolated) of L = sum g_colors*colors w.r.t. every
+    element of means, quat (unnormalised), shape (log Lambda, log lambda, k, phi), amp, dc, campos.
+    Catches any dropped term, sign, index or transposed operand in the analytic backward, including
+    the eq.(10) normaliser terms the paper does not give."""
+    inp = _tiny(seed, cfg)
+    g = oracle.nasg_bwd(inp, mode)
+
+    def loss(x):
+        return float(np.sum(oracle.nasg_fwd(x, mode) * x["g_colors"]))
+
+    for key, gkey in (("means", "g_means"), ("quat", "g_quat"), ("shape", "g_shape"), ("amp", "g_amp"),
+                      ("dc", "g_dc"), ("campos", "g_campos")):
+        ana = g[gkey]
+        num = np.zeros_like(ana)
+        base = inp[key]
+        it = np.nditer(base, flags=["multi_index"])
+        for _ in it:
+            idx = it.multi_index
+            def fd(h):
+                p = base.copy(); p[idx] += h
+                m = base.copy(); m[idx] -= h
+                return (loss(dict(inp, **{key: p})) - loss(dict(inp, **{key: m}))) / (2 * h)
+            h = 2e-4
+            num[idx] = (4.0 * fd(h / 2) - fd(h)) / 3.0
+        scale = np.max(np.abs(ana)) + 1e-30
+        assert np.max(np.abs(num - ana)) < 2e-7 * scale, (key, np.max(np.abs(num - ana)) / scale)
+
+
+# ------------------------------------------------------------------------------------------
+# P7: the paper's own derivative formulas, Supplementary F eqs.(50)-(65)
+# ------------------------------------------------------------------------------------------
+def test_P7_paper_partials_eqs_50_to_65(oracle):
+    """With the NASG normaliser C^{-1} (eq.48; norm_mode 0) and phi = 0 the oracle's scalar partials
+    must equal the paper's printed chain-rule expressions, typed here from the supplement with the
+    two corrections DESIGN.md R6 lists (eq.55: minus sign; eq.60: braces)."""
+    rng = np.random.default_rng(77)
+    for _ in range(40):
+        lam, a, k = float(np.exp(rng.uniform(0, 4))), float(np.exp(rng.uniform(-2, 3))), float(rng.uniform(0, 10))
+        d = _random_unit(rng, 1)[0]
+        X, Z = oracle.frame(rng.standard_normal(4))
+        u, v = float(d @ X), float(d @ Z)
+        kappa = (v + 1) / 2; omv2 = 1 - v * v
+        tau = a * u * u / omv2; E = kappa ** tau                                   # eq.(47)
+        p = np.exp(2 * lam * (E * kappa - 1))                                       # eq.(48)
+        Ci = lam * np.sqrt(1 + a) / (TWO_PI * (1 - np.exp(-2 * lam)))               # eq.(48)
+        H = (1 + np.cos(k * u)) / 2
+        dtau_da = u * u / omv2                                                      # eq.(50)
+        dp_da = p * (2 * lam * E * kappa) * np.log(kappa) * dtau_da                 # eq.(51)
+        dE_da = E * np.log(kappa) * dtau_da                                         # eq.(52)
+        dC_da = lam / (2 * np.sqrt(1 + a)) / (TWO_PI * (1 - np.exp(-2 * lam)))      # eq.(53), eps = 0
+        G_a = (dp_da * E * Ci + p * dE_da * Ci + p * E * dC_da) * H
+        dp_dl = 2 * p * (E * kappa - 1)                                             # eq.(54)
+        e2 = np.exp(-2 * lam)
+        dC_dl = (np.sqrt(1 + a) * (1 - e2) - 2 * lam * np.sqrt(1 + a) * e2) / (TWO_PI * (1 - e2) ** 2)  # eq.(55), sign fixed
+        G_l = (E * Ci * dp_dl + E * p * dC_dl) * H                                  # eq.(56)
+        dtau_dx = 2 * a * u / omv2                                                  # eq.(57) (x d)
+        dE_dx = E * np.log(kappa) * dtau_dx; dp_dx = 2 * lam * p * kappa * dE_dx    # eq.(58)
+        dH_dx = -k / 2 * np.sin(k * u)                                              # eq.(59)
+        G_x = (dp_dx * E * Ci + p * dE_dx * Ci) * H + p * E * Ci * dH_dx            # eq.(60)
+        dk_dz = 0.5; dtau_dz = a * u * u * 2 * v / omv2 ** 2                        # eq.(61)
+        dE_dz = E * (tau / kappa * dk_dz + np.log(kappa) * dtau_dz)                 # eq.(62)
+        dp_dz = p * 2 * lam * (kappa * dE_dz + E * dk_dz)                           # eq.(63)
+        G_z = (dp_dz * E * Ci + p * dE_dz * Ci) * H                                 # eq.(64)
+        G_k = p * E * Ci * (-u / 2 * np.sin(k * u))                                 # eq.(65)
+        o = oracle.partials(u, v, lam, a, k, 0.0, 0)
+        want = np.array([p * E * Ci * H, G_x, G_z, G_l, G_a, G_k])
+        assert np.max(np.abs(o[:6] - want) / (np.abs(want) + 1e-300)) < 1e-9, (o[:6], want)
+
+
+# ------------------------------------------------------------------------------------------
+# P9: spherical harmonics of degree 3 (eq.(5))
+# ------------------------------------------------------------------------------------------
+def _scipy_real_sh(d):
+    """Real orthonormal SH with the (-1)^|m| sign kept (reading R15) from scipy's complex Y_l^m."""
+    theta = np.arccos(np.clip(d[:, 2], -1, 1)); phi = np.arctan2(d[:, 1], d[:, 0])
+    out = np.zeros((d.shape[0], 16))
+    for l in range(4):
+        for m in range(-l, l + 1):
+            Y = scipy.special.sph_harm_y(l, abs(m), theta, phi)       # includes Condon-Shortley
+            if m == 0:
+                val = Y.real
+            elif m > 0:
+                val = np.sqrt(2.0) * Y.real
+            else:
+                val = np.sqrt(2.0) * Y.imag
+            out[:, l * l + l + m] = val
+    return out
+
+
+def test_P9_sh_basis_matches_scipy(oracle):
+    rng = np.random.default_rng(3)
+    d = _random_unit(rng, 50)
+    got = np.stack([oracle.sh_basis(x)[0] for x in d])
+    assert np.max(np.abs(got - _scipy_real_sh(d))) < 1e-13
+
+
+def test_P9_sh_orthonormal_and_addition_theorem(oracle):
+    x, w = np.polynomial.legendre.leggauss(16)
+    az = (np.arange(32) + 0.5) * (TWO_PI / 32)
+    s = np.sqrt(1 - x * x)
+    d = np.stack([np.outer(s, np.cos(az)), np.outer(s, np.sin(az)), np.repeat(x[:, None], 32, 1)], -1).reshape(-1, 3)
+    wt = np.repeat(w[:, None], 32, 1).reshape(-1) * (TWO_PI / 32)
+    Y = np.stack([oracle.sh_basis(v)[0] for v in d])
+    gram = (Y * wt[:, None]).T @ Y
+    assert np.max(np.abs(gram - np.eye(16))) < 1e-12
+    for l in range(4):
+        band = (Y[:, l * l:(l + 1) * (l + 1)] ** 2).sum(axis=1)
+        assert np.max(np.abs(band - (2 * l + 1) / (4 * np.pi))) < 1e-13
+
+
+def test_P9_sh_forward_is_the_expansion_and_fd_gradients(oracle):
+    from paper_2606_09794_b200 import workloads as W
+    inp = {k: (v.astype(np.float64) if isinstance(v, np.ndarray) and v.dtype == np.float32 else v)
+           for k, v in W.make(3, N=6).items()}
+    col = oracle.sh_fwd(inp)
+    # eq.(5) with scipy's basis
+    for c in range(inp["C"]):
+        dvec = inp["means"] - inp["campos"][c]
+        dvec /= np.linalg.norm(dvec, axis=1, keepdims=True)
+        Y = _scipy_real_sh(dvec)                                  # [N,16]
+        want = np.einsum("nj,jkn->nk", Y, inp["coeffs"]) * (inp["vis"][c] != 0)[:, None]
+        assert np.max(np.abs(want - col[c])) < 1e-12
+    g = oracle.sh_bwd(inp)
+
+    def loss(x):
+        return float(np.sum(oracle.sh_fwd(x) * x["g_colors"]))
+
+    for key, gkey in (("means", "g_means"), ("coeffs", "g_coeffs"), ("campos", "g_campos")):
+        ana = g[gkey]; num = np.zeros_like(ana); base = inp[key]
+        it = np.nditer(base, flags=["multi_index"])
+        for _ in it:
+            idx = it.multi_index
+            def fd(h):
+                p = base.copy(); p[idx] += h
+                m = base.copy(); m[idx] -= h
+                return (loss(dict(inp, **{key: p})) - loss(dict(inp, **{key: m}))) / (2 * h)
+            num[idx] = (4.0 * fd(5e-4) - fd(1e-3)) / 3.0
+        assert np.max(np.abs(num - ana)) < 1e-8 * (np.max(np.abs(ana)) + 1e-30), key
+
+
+# ------------------------------------------------------------------------------------------
+# workloads: recipe checks (no method arithmetic)
+# ------------------------------------------------------------------------------------------
+def test_workload_recipe():
+    from paper_2606_09794_b200 import workloads as W
+    a = W.make(2, N=1000); b = W.make(3, N=1000)
+    for key in ("means", "campos", "vis", "g_colors"):
+        assert np.array_equal(a[key], b[key])           # config 3 shares config 2's geometry
+    assert a["quat"].shape == (4, 1000, 4) and a["shape"].shape == (4, 1000, 4)
+    assert a["amp"].shape == (4, 3, 1000) and a["dc"].shape == (3, 1000) and b["coeffs"].shape == (16, 3, 1000)
+    assert np.all(a["shape"][..., 0] >= a["shape"][..., 1])             # second bandwidth <= first
+    assert np.allclose(np.linalg.norm(a["campos"], axis=1), 4.0, atol=1e-5)
+    assert np.allclose(np.linalg.norm(a["quat"], axis=2), 1.0, atol=1e-5)
+    assert 0.5 < a["vis"].mean() < 0.7 and a["vis"].dtype == np.uint8
+    z = W.make(0)
+    assert z["vis"] is None and np.array_equal(z["campos"], np.array([[0, 0, 4]], np.float32))
+    s4 = W.make(4, N=1000)["shape"]
+    assert s4[..., 1].min() >= 3 and s4[..., 0].max() <= 8 and 4 <= s4[..., 2].min() and s4[..., 2].max() <= 16
+    sub = W.take(a, np.array([5, 17]))
+    assert np.array_equal(sub["amp"], a["amp"][:, :, [5, 17]]) and sub["N"] == 2
