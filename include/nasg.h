@@ -1,0 +1,137 @@
+/* nasg.h — C ABI of the B200-native (sm_100a) NASGabor / SH-3 per-Gaussian colour evaluation.
+ *
+ * What the library computes (arxiv/paper_2606_09794; citations are /root/reference/PAPER.md lines):
+ *
+ *   d_cn      = normalize(means[n] - campos[c])          central-ray direction, one evaluation per
+ *                                                        primitive per frame
+ *   colour    = c0 + sum_{l<K} w_l G_l(d)                appearance model, eq.(6)
+ *   G         = H p E / I                                NASGabor lobe, eq.(9)
+ *               kappa = (d.z+1)/2, tau = a (d.x)^2/(1-(d.z)^2), E = kappa^tau,
+ *               p = exp(2 lambda (E kappa - 1)), H = (1+cos(k d.x + phi))/2
+ *   I         = pi(1-e^{-2 lambda})/(lambda sqrt(1+a)) (1+Psi),                       eq.(10)
+ *               Psi = 2 Lambda e^{-Lambda} sinhc(sqrt(Lambda^2-k^2))/(1-e^{-2 Lambda}), Lambda = lambda(1+a)
+ *               (norm_mode 0: the NASG normaliser 2 pi(1-e^{-2 lambda})/(lambda sqrt(1+a)),
+ *                what the paper trained with)
+ *   SH path   = sum_{j<16} coeff_j Y_j(d), real SH of degree 3, eq.(5)
+ *   backward  = exact gradient of sum(g_colors * colors) w.r.t. every parameter and the mean
+ *               (through d); eqs.(50)-(65) PAPER.md:754-861 plus the terms derived in DESIGN.md §4.
+ *
+ * Parameterisation (DESIGN.md §3 readings R1, R5, R12): the frame [x y z] is R(q/|q|) of a per-lobe
+ * quaternion q = (w,x,y,z), x = column 0 (carrier axis), z = column 2 (lobe axis); the two
+ * log-bandwidths are l1 = log Lambda >= l2 = log lambda, a = Lambda/lambda - 1 >= 0; the phase phi
+ * enters the carrier only. No activation is applied to k, phi, w or c0 (Table 8 activations are the
+ * caller's); no clamp or +0.5 on the output.
+ *
+ * Conventions
+ *   - Every pointer of the device entry points is a DEVICE pointer, fp32 unless typed otherwise,
+ *     row-major with the shape written beside it. The caller owns every buffer; the library never
+ *     allocates, never synchronises, keeps no global state, and is CUDA-graph capturable. Work is
+ *     enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = legacy default stream).
+ *   - Outputs are overwritten, never accumulated. colors[c,n,:] of a culled pair (vis[c,n]==0) is 0;
+ *     every gradient of a Gaussian culled in all C cameras is 0.
+ *   - Return value: 0 (NASG_OK) or a negative NASG_ERR_* code. Nothing is thrown or printed.
+ *     Device-side faults (bad pointers) surface at the caller's next synchronisation.
+ *   - Inputs are not validated on the device: a zero quaternion or means[n]==campos[c] yields NaN.
+ *   - N == 0 is a successful no-op.
+ */
+#ifndef NASG_H_
+#define NASG_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NASG_OK                  0
+#define NASG_ERR_NULL           -1  /* a required pointer is NULL                                   */
+#define NASG_ERR_SHAPE          -2  /* N < 0, C < 1, C > NASG_MAX_CAMERAS                           */
+#define NASG_ERR_UNSUPPORTED_K  -3  /* K not in {1,2,3,4,5,8} (paper: 1..5; cfg4: 8)  */
+#define NASG_ERR_ALIGN          -4  /* quat/shape (or their gradients) not 16-byte aligned          */
+#define NASG_ERR_WORKSPACE      -5  /* g_campos requested but workspace NULL or too small           */
+#define NASG_ERR_CUDA           -6  /* launch / copy failed: cudaGetLastError()                     */
+#define NASG_ERR_NORM_MODE      -7  /* norm_mode not 0 or 1                                         */
+
+#define NASG_MAX_CAMERAS 64
+
+#define NASG_NORM_APPROX 0          /* NASG normaliser, carrier ignored              */
+#define NASG_NORM_EXACT  1          /* eq.(10) as printed                        */
+
+/* Inputs of one evaluation: N Gaussians, K lobes each, C cameras. */
+typedef struct {
+    int64_t N;
+    int32_t K;
+    int32_t C;
+    const float   *means;   /* [N,3]                                                                */
+    const float   *quat;    /* [K,N,4]  (w,x,y,z), any non-zero norm; 16-byte aligned               */
+    const float   *shape;   /* [K,N,4]  (log Lambda, log lambda, k, phi), log Lambda >= log lambda;  */
+                            /*          16-byte aligned                                             */
+    const float   *amp;     /* [K,3,N]  RGB amplitude w_l (planar)                                   */
+    const float   *dc;      /* [3,N]    c0 (planar)                                                  */
+    const float   *campos;  /* [C,3]                                                                */
+    const uint8_t *vis;     /* [C,N] non-zero = visible, or NULL = all visible                      */
+} nasg_inputs;
+
+/* Gradient outputs of nasg_eval_bwd; same shapes as the inputs. Any pointer may be NULL = skip. */
+typedef struct {
+    float *g_means;         /* [N,3]                                                                */
+    float *g_quat;          /* [K,N,4]  w.r.t. the raw (unnormalised) quaternion; 16-byte aligned   */
+    float *g_shape;         /* [K,N,4]  (d/dlogLambda, d/dloglambda, d/dk, d/dphi); 16-byte aligned */
+    float *g_amp;           /* [K,3,N]                                                              */
+    float *g_dc;            /* [3,N]                                                                */
+    float *g_campos;        /* [C,3]    optional per-camera term (needs workspace)                  */
+    void  *workspace;       /* device scratch, >= nasg_workspace_bytes(N,K,C); only for g_campos    */
+    size_t workspace_bytes;
+} nasg_grads;
+
+/* colors[C,N,3] = c0 + sum_l w_l G_l(d)   (eq.(6), eq.(9), eq.(10)). Asynchronous on cuda_stream. */
+int nasg_eval_fwd(const nasg_inputs *in, float *colors, int norm_mode, void *cuda_stream);
+
+/* Gradients of sum(g_colors[C,N,3] * colors) (Supplementary F + DESIGN.md §4). Nothing saved by the
+ * forward is needed: the lobe values are recomputed. Each gradient element is written exactly once
+ * by one thread (no atomics); g_campos is a warp-shuffle -> block -> second-stage reduction through
+ * `workspace`, deterministic for a given N. */
+int nasg_eval_bwd(const nasg_inputs *in, const float *g_colors, const nasg_grads *out, int norm_mode,
+                  void *cuda_stream);
+
+/* Comparison path: real SH degree 3, coeffs [16,3,N] (j = l^2+l+m, Condon-Shortley sign kept,
+ * DESIGN.md R15), colors[C,N,3] = sum_j coeffs[j,:,n] Y_j(d). */
+int sh_eval_fwd(int64_t N, int32_t C, const float *means, const float *coeffs, const float *campos,
+                const uint8_t *vis, float *colors, void *cuda_stream);
+int sh_eval_bwd(int64_t N, int32_t C, const float *means, const float *coeffs, const float *campos,
+                const uint8_t *vis, const float *g_colors, float *g_means, float *g_coeffs,
+                float *g_campos, void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* Bytes of device scratch nasg_eval_bwd / sh_eval_bwd need when g_campos != NULL (pass K = 0 for SH). */
+size_t nasg_workspace_bytes(int64_t N, int32_t K, int32_t C);
+
+/* ---- end-to-end entry points with HOST buffers -------------------------------------------------
+ * Same computation, forward then backward, but every array pointer in `in`, `colors`, `g_colors`
+ * and `out` is a HOST pointer (pinned memory makes the copies asynchronous and fast; pageable works).
+ * The call copies the inputs to `dev_scratch` (a DEVICE buffer of >= *_host_scratch_bytes), runs the
+ * two kernels, copies colours and gradients back, all on cuda_stream, and returns without
+ * synchronising. out->workspace is ignored (carved from dev_scratch). */
+size_t nasg_host_scratch_bytes(int64_t N, int32_t K, int32_t C);
+int nasg_eval_fwd_bwd_host(const nasg_inputs *in, const float *g_colors, float *colors,
+                           const nasg_grads *out, int norm_mode, void *dev_scratch,
+                           size_t dev_scratch_bytes, void *cuda_stream);
+size_t sh_host_scratch_bytes(int64_t N, int32_t C);
+int sh_eval_fwd_bwd_host(int64_t N, int32_t C, const float *means, const float *coeffs,
+                         const float *campos, const uint8_t *vis, const float *g_colors,
+                         float *colors, float *g_means, float *g_coeffs, float *g_campos,
+                         void *dev_scratch, size_t dev_scratch_bytes, void *cuda_stream);
+
+/* Human-readable text for a return code (static string; for NASG_ERR_CUDA the last CUDA error). */
+const char *nasg_strerror(int code);
+
+/* Library version, e.g. "0.1.0 sm_100a". */
+const char *nasg_version(void);
+
+/* Number of kernels the library has launched since load (all entry points; for bench accounting). */
+int64_t nasg_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NASG_H_ */

@@ -1,0 +1,247 @@
+"""Thin ctypes binding of ``include/nasg.h`` (argument marshalling only).
+
+Every step of the path runs in the CUDA kernels of ``libnasg_b200.so``; PyTorch is used for device
+memory and streams. There is NO CPU fallback: if the library cannot be loaded (or built) the import
+fails loudly, and every entry point raises :class:`NasgError` on a non-zero return code.
+
+Names mirror the C ABI: ``nasg_eval_fwd``, ``nasg_eval_bwd``, ``sh_eval_fwd``, ``sh_eval_bwd``,
+``nasg_workspace_bytes``, ``nasg_eval_fwd_bwd_host``, ``sh_eval_fwd_bwd_host``, ``nasg_strerror``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import torch
+
+from . import build as _build
+
+NORM_APPROX, NORM_EXACT = 0, 1
+MAX_CAMERAS = 64
+SYMBOLS = ("nasg_eval_fwd", "nasg_eval_bwd", "sh_eval_fwd", "sh_eval_bwd", "nasg_workspace_bytes",
+           "nasg_host_scratch_bytes", "nasg_eval_fwd_bwd_host", "sh_host_scratch_bytes",
+           "sh_eval_fwd_bwd_host", "nasg_strerror", "nasg_version", "nasg_launch_count")
+
+
+class NasgError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where} failed with code {code}: {nasg_strerror(code)}")
+
+
+class _Inputs(C.Structure):
+    _fields_ = [("N", C.c_int64), ("K", C.c_int32), ("C", C.c_int32), ("means", C.c_void_p),
+                ("quat", C.c_void_p), ("shape", C.c_void_p), ("amp", C.c_void_p), ("dc", C.c_void_p),
+                ("campos", C.c_void_p), ("vis", C.c_void_p)]
+
+
+class _Grads(C.Structure):
+    _fields_ = [("g_means", C.c_void_p), ("g_quat", C.c_void_p), ("g_shape", C.c_void_p),
+                ("g_amp", C.c_void_p), ("g_dc", C.c_void_p), ("g_campos", C.c_void_p),
+                ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
+
+
+def _load():
+    path = _build.LIB
+    if _build.is_stale():
+        try:
+            _build.build()
+        except Exception as exc:  # no nvcc on this machine and no prebuilt library: fail loudly
+            if not os.path.exists(path):
+                raise ImportError(
+                    f"libnasg_b200.so is missing and could not be built ({exc}); run "
+                    f"`python -m paper_2606_09794_b200.build`. There is no CPU fallback.") from exc
+    lib = C.CDLL(path)
+    vp, i64, i32, sz = C.c_void_p, C.c_int64, C.c_int32, C.c_size_t
+    lib.nasg_eval_fwd.argtypes = [C.POINTER(_Inputs), vp, C.c_int, vp]
+    lib.nasg_eval_bwd.argtypes = [C.POINTER(_Inputs), vp, C.POINTER(_Grads), C.c_int, vp]
+    lib.sh_eval_fwd.argtypes = [i64, i32, vp, vp, vp, vp, vp, vp]
+    lib.sh_eval_bwd.argtypes = [i64, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.nasg_workspace_bytes.argtypes = [i64, i32, i32]
+    lib.nasg_workspace_bytes.restype = sz
+    lib.nasg_host_scratch_bytes.argtypes = [i64, i32, i32]
+    lib.nasg_host_scratch_bytes.restype = sz
+    lib.sh_host_scratch_bytes.argtypes = [i64, i32]
+    lib.sh_host_scratch_bytes.restype = sz
+    lib.nasg_eval_fwd_bwd_host.argtypes = [C.POINTER(_Inputs), vp, vp, C.POINTER(_Grads), C.c_int, vp, sz, vp]
+    lib.sh_eval_fwd_bwd_host.argtypes = [i64, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.nasg_strerror.argtypes = [C.c_int]
+    lib.nasg_strerror.restype = C.c_char_p
+    lib.nasg_version.restype = C.c_char_p
+    lib.nasg_launch_count.restype = i64
+    for name in ("nasg_eval_fwd", "nasg_eval_bwd", "sh_eval_fwd", "sh_eval_bwd", "nasg_eval_fwd_bwd_host",
+                 "sh_eval_fwd_bwd_host"):
+        getattr(lib, name).restype = C.c_int
+    return lib
+
+
+_lib = _load()
+LIB_PATH = _build.LIB
+
+
+def nasg_strerror(code: int) -> str:
+    return _lib.nasg_strerror(int(code)).decode()
+
+
+def nasg_version() -> str:
+    return _lib.nasg_version().decode()
+
+
+def nasg_launch_count() -> int:
+    return int(_lib.nasg_launch_count())
+
+
+def nasg_workspace_bytes(N: int, K: int, Cn: int) -> int:
+    return int(_lib.nasg_workspace_bytes(N, K, Cn))
+
+
+def nasg_host_scratch_bytes(N: int, K: int, Cn: int) -> int:
+    return int(_lib.nasg_host_scratch_bytes(N, K, Cn))
+
+
+def sh_host_scratch_bytes(N: int, Cn: int) -> int:
+    return int(_lib.sh_host_scratch_bytes(N, Cn))
+
+
+def _ptr(t: Optional[torch.Tensor]):
+    return None if t is None else t.data_ptr()
+
+
+def _stream(stream) -> Optional[int]:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def _chk(t: Optional[torch.Tensor], name: str, shape, dtype, device_type: str):
+    if t is None:
+        return
+    if tuple(t.shape) != tuple(shape) or t.dtype != dtype or not t.is_contiguous() or t.device.type != device_type:
+        raise ValueError(f"{name}: expected contiguous {dtype} {tuple(shape)} on {device_type}, got "
+                         f"{t.dtype} {tuple(t.shape)} on {t.device} contiguous={t.is_contiguous()}")
+
+
+def _inputs(means, quat, shape, amp, dc, campos, vis, device_type="cuda") -> _Inputs:
+    K, N = int(quat.shape[0]), int(quat.shape[1])
+    Cn = int(campos.shape[0])
+    f32 = torch.float32
+    _chk(means, "means", (N, 3), f32, device_type); _chk(quat, "quat", (K, N, 4), f32, device_type)
+    _chk(shape, "shape", (K, N, 4), f32, device_type); _chk(amp, "amp", (K, 3, N), f32, device_type)
+    _chk(dc, "dc", (3, N), f32, device_type); _chk(campos, "campos", (Cn, 3), f32, device_type)
+    _chk(vis, "vis", (Cn, N), torch.uint8, device_type)
+    return _Inputs(N, K, Cn, _ptr(means), _ptr(quat), _ptr(shape), _ptr(amp), _ptr(dc), _ptr(campos), _ptr(vis))
+
+
+def nasg_eval_fwd(means, quat, shape, amp, dc, campos, vis=None, norm_mode: int = NORM_EXACT,
+                  out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    """colors [C,N,3] = c0 + sum_l w_l G_l(normalize(mean - campos))  (eq.(6), eq.(9), eq.(10))."""
+    inp = _inputs(means, quat, shape, amp, dc, campos, vis)
+    if out is None:
+        out = torch.empty((inp.C, inp.N, 3), dtype=torch.float32, device=means.device)
+    _chk(out, "colors", (inp.C, inp.N, 3), torch.float32, "cuda")
+    rc = _lib.nasg_eval_fwd(C.byref(inp), _ptr(out), int(norm_mode), _stream(stream))
+    if rc != 0:
+        raise NasgError(rc, "nasg_eval_fwd")
+    return out
+
+
+def nasg_alloc_grads(K: int, N: int, Cn: int, device, want_campos: bool = False) -> dict:
+    f32 = torch.float32
+    g = dict(g_means=torch.empty((N, 3), dtype=f32, device=device), g_quat=torch.empty((K, N, 4), dtype=f32, device=device),
+             g_shape=torch.empty((K, N, 4), dtype=f32, device=device), g_amp=torch.empty((K, 3, N), dtype=f32, device=device),
+             g_dc=torch.empty((3, N), dtype=f32, device=device))
+    if want_campos:
+        g["g_campos"] = torch.empty((Cn, 3), dtype=f32, device=device)
+        g["workspace"] = torch.empty(max(1, nasg_workspace_bytes(N, K, Cn)), dtype=torch.uint8, device=device)
+    return g
+
+
+def _grads_struct(g: dict) -> _Grads:
+    ws = g.get("workspace")
+    return _Grads(_ptr(g.get("g_means")), _ptr(g.get("g_quat")), _ptr(g.get("g_shape")), _ptr(g.get("g_amp")),
+                  _ptr(g.get("g_dc")), _ptr(g.get("g_campos")), _ptr(ws), 0 if ws is None else ws.numel())
+
+
+def nasg_eval_bwd(means, quat, shape, amp, dc, campos, g_colors, vis=None, norm_mode: int = NORM_EXACT,
+                  want_campos: bool = False, out: Optional[dict] = None, stream=None) -> dict:
+    """Gradients of sum(g_colors * colors): dict g_means, g_quat, g_shape, g_amp, g_dc[, g_campos]."""
+    inp = _inputs(means, quat, shape, amp, dc, campos, vis)
+    _chk(g_colors, "g_colors", (inp.C, inp.N, 3), torch.float32, "cuda")
+    if out is None:
+        out = nasg_alloc_grads(inp.K, inp.N, inp.C, means.device, want_campos)
+    gs = _grads_struct(out)
+    rc = _lib.nasg_eval_bwd(C.byref(inp), _ptr(g_colors), C.byref(gs), int(norm_mode), _stream(stream))
+    if rc != 0:
+        raise NasgError(rc, "nasg_eval_bwd")
+    return out
+
+
+def sh_eval_fwd(means, coeffs, campos, vis=None, out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    """colors [C,N,3] = sum_j coeffs[j,:,n] Y_j(d), real SH degree 3 (eq.(5))."""
+    N, Cn = int(means.shape[0]), int(campos.shape[0])
+    f32 = torch.float32
+    _chk(means, "means", (N, 3), f32, "cuda"); _chk(coeffs, "coeffs", (16, 3, N), f32, "cuda")
+    _chk(campos, "campos", (Cn, 3), f32, "cuda"); _chk(vis, "vis", (Cn, N), torch.uint8, "cuda")
+    if out is None:
+        out = torch.empty((Cn, N, 3), dtype=f32, device=means.device)
+    rc = _lib.sh_eval_fwd(N, Cn, _ptr(means), _ptr(coeffs), _ptr(campos), _ptr(vis), _ptr(out), _stream(stream))
+    if rc != 0:
+        raise NasgError(rc, "sh_eval_fwd")
+    return out
+
+
+def sh_alloc_grads(N: int, Cn: int, device, want_campos: bool = False) -> dict:
+    f32 = torch.float32
+    g = dict(g_means=torch.empty((N, 3), dtype=f32, device=device), g_coeffs=torch.empty((16, 3, N), dtype=f32, device=device))
+    if want_campos:
+        g["g_campos"] = torch.empty((Cn, 3), dtype=f32, device=device)
+        g["workspace"] = torch.empty(max(1, nasg_workspace_bytes(N, 0, Cn)), dtype=torch.uint8, device=device)
+    return g
+
+
+def sh_eval_bwd(means, coeffs, campos, g_colors, vis=None, want_campos: bool = False, out: Optional[dict] = None,
+                stream=None) -> dict:
+    N, Cn = int(means.shape[0]), int(campos.shape[0])
+    f32 = torch.float32
+    _chk(means, "means", (N, 3), f32, "cuda"); _chk(coeffs, "coeffs", (16, 3, N), f32, "cuda")
+    _chk(campos, "campos", (Cn, 3), f32, "cuda"); _chk(vis, "vis", (Cn, N), torch.uint8, "cuda")
+    _chk(g_colors, "g_colors", (Cn, N, 3), f32, "cuda")
+    if out is None:
+        out = sh_alloc_grads(N, Cn, means.device, want_campos)
+    ws = out.get("workspace")
+    rc = _lib.sh_eval_bwd(N, Cn, _ptr(means), _ptr(coeffs), _ptr(campos), _ptr(vis), _ptr(g_colors),
+                          _ptr(out.get("g_means")), _ptr(out.get("g_coeffs")), _ptr(out.get("g_campos")),
+                          _ptr(ws), 0 if ws is None else ws.numel(), _stream(stream))
+    if rc != 0:
+        raise NasgError(rc, "sh_eval_bwd")
+    return out
+
+
+def nasg_eval_fwd_bwd_host(host: dict, host_out: dict, dev_scratch: torch.Tensor, norm_mode: int = NORM_EXACT,
+                           stream=None) -> None:
+    """End-to-end call with HOST tensors (pinned recommended): H2D copies, forward, backward, D2H copies,
+    all enqueued on ``stream``; returns without synchronising. ``host`` holds means, quat, shape, amp, dc,
+    campos, vis (or None), g_colors; ``host_out`` holds colors and any of g_means, g_quat, g_shape, g_amp,
+    g_dc, g_campos."""
+    inp = _inputs(host["means"], host["quat"], host["shape"], host["amp"], host["dc"], host["campos"],
+                  host.get("vis"), device_type="cpu")
+    _chk(host["g_colors"], "g_colors", (inp.C, inp.N, 3), torch.float32, "cpu")
+    _chk(host_out["colors"], "colors", (inp.C, inp.N, 3), torch.float32, "cpu")
+    gs = _grads_struct({k: v for k, v in host_out.items() if k != "colors"})
+    rc = _lib.nasg_eval_fwd_bwd_host(C.byref(inp), _ptr(host["g_colors"]), _ptr(host_out["colors"]), C.byref(gs),
+                                     int(norm_mode), _ptr(dev_scratch), dev_scratch.numel() * dev_scratch.element_size(),
+                                     _stream(stream))
+    if rc != 0:
+        raise NasgError(rc, "nasg_eval_fwd_bwd_host")
+
+
+def sh_eval_fwd_bwd_host(host: dict, host_out: dict, dev_scratch: torch.Tensor, stream=None) -> None:
+    N, Cn = int(host["means"].shape[0]), int(host["campos"].shape[0])
+    rc = _lib.sh_eval_fwd_bwd_host(N, Cn, _ptr(host["means"]), _ptr(host["coeffs"]), _ptr(host["campos"]),
+                                   _ptr(host.get("vis")), _ptr(host["g_colors"]), _ptr(host_out["colors"]),
+                                   _ptr(host_out.get("g_means")), _ptr(host_out.get("g_coeffs")),
+                                   _ptr(host_out.get("g_campos")), _ptr(dev_scratch),
+                                   dev_scratch.numel() * dev_scratch.element_size(), _stream(stream))
+    if rc != 0:
+        raise NasgError(rc, "sh_eval_fwd_bwd_host")

@@ -1,0 +1,46 @@
+// nasg_internal.h — kernel parameter blocks and launcher declarations shared by the .cu files of the
+// library (not part of the public ABI; the oracle does not see this file).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace nasg {
+
+struct FwdParams {
+    int64_t N;
+    int C;
+    const float *means, *quat, *shape, *amp, *dc, *campos;
+    const uint8_t *vis;
+    float *colors;
+};
+
+struct BwdParams {
+    int64_t N;
+    int C;
+    const float *means, *quat, *shape, *amp, *campos;
+    const uint8_t *vis;
+    const float *g_colors;
+    float *g_means, *g_quat, *g_shape, *g_amp, *g_dc;
+    float *cam_partial;          // [blocks, C, 3] per-block partial sums of g_campos, or nullptr
+};
+
+struct ShParams {
+    int64_t N;
+    int C;
+    const float *means, *coeffs, *campos;
+    const uint8_t *vis;
+    const float *g_colors;       // backward only
+    float *colors;               // forward only
+    float *g_means, *g_coeffs;   // backward only
+    float *cam_partial;
+};
+
+int64_t grid_blocks(int64_t N);
+cudaError_t launch_nasg_fwd(const FwdParams &p, int K, bool exact, cudaStream_t st);
+cudaError_t launch_nasg_bwd(const BwdParams &p, int K, bool exact, cudaStream_t st);
+cudaError_t launch_campos_reduce(const float *partial, int64_t nblocks, int C, float *out, cudaStream_t st);
+cudaError_t launch_sh_fwd(const ShParams &p, cudaStream_t st);
+cudaError_t launch_sh_bwd(const ShParams &p, cudaStream_t st);
+
+} // namespace nasg
