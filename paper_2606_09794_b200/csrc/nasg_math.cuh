@@ -275,6 +275,7 @@ NASG_HD float lobe_eval(const Lobe &L, float dx, float dy, float dz, EvalTerms &
     float em1 = expm1_neg(x1);                               // kappa^(1+tau) - 1
     float arg = fmaf(L.lam2, em1, tau * Lk);                 // ln(p E)
     float Gbar = f_exp(arg) * L.invI;
+    Gbar = (s2 <= 1e-30f && !upper) ? 0.0f : Gbar;           // d = -z: G = 0 (eq.(9), third case)
     float theta = fmaf(L.k, u, L.phi);
     float H;
     if (FULL) {

@@ -1,0 +1,71 @@
+"""Helpers of the GPU parity tests: move a workload to the device, run the CUDA path through the
+C-ABI binding, compare with the fp64 oracle. Tolerances are BASELINE.json's: max|err| <= 1e-5 max|ref|
+for the forward colours, <= 1e-4 max|ref| for every gradient array."""
+import numpy as np
+import torch
+
+FWD_TOL = 1e-5
+BWD_TOL = 1e-4
+NASG_KEYS = ("means", "quat", "shape", "amp", "dc", "campos", "vis", "g_colors")
+SH_KEYS = ("means", "coeffs", "campos", "vis", "g_colors")
+
+
+def to_dev(inp: dict, keys) -> dict:
+    out = {}
+    for k in keys:
+        v = inp.get(k)
+        out[k] = None if v is None else torch.from_numpy(np.ascontiguousarray(v)).cuda()
+    return out
+
+
+def rel_err(got, ref) -> float:
+    got = got.detach().cpu().numpy().astype(np.float64) if isinstance(got, torch.Tensor) else np.asarray(got, np.float64)
+    assert np.all(np.isfinite(got)), "non-finite output"
+    return float(np.max(np.abs(got - ref)) / (np.max(np.abs(ref)) + 1e-300))
+
+
+def run_nasg(B, d: dict, norm_mode=1, want_campos=False):
+    col = B.nasg_eval_fwd(d["means"], d["quat"], d["shape"], d["amp"], d["dc"], d["campos"], d["vis"], norm_mode)
+    g = B.nasg_eval_bwd(d["means"], d["quat"], d["shape"], d["amp"], d["dc"], d["campos"], d["g_colors"],
+                        d["vis"], norm_mode, want_campos=want_campos)
+    torch.cuda.synchronize()
+    return col, g
+
+
+def run_sh(B, d: dict, want_campos=False):
+    col = B.sh_eval_fwd(d["means"], d["coeffs"], d["campos"], d["vis"])
+    g = B.sh_eval_bwd(d["means"], d["coeffs"], d["campos"], d["g_colors"], d["vis"], want_campos=want_campos)
+    torch.cuda.synchronize()
+    return col, g
+
+
+def check_nasg(B, oracle, inp: dict, norm_mode=1, want_campos=False, label=""):
+    d = to_dev(inp, NASG_KEYS)
+    col, g = run_nasg(B, d, norm_mode, want_campos)
+    rc = oracle.nasg_fwd(inp, norm_mode)
+    rg = oracle.nasg_bwd(inp, norm_mode)
+    errs = {"colors": rel_err(col, rc)}
+    for k in ("g_means", "g_quat", "g_shape", "g_amp", "g_dc") + (("g_campos",) if want_campos else ()):
+        errs[k] = rel_err(g[k], rg[k])
+    print(label, " ".join(f"{k}={v:.2e}" for k, v in errs.items()))
+    assert errs["colors"] <= FWD_TOL, (label, errs)
+    for k, v in errs.items():
+        if k != "colors":
+            assert v <= BWD_TOL, (label, k, errs)
+    return col, g, errs
+
+
+def check_sh(B, oracle, inp: dict, want_campos=False, label=""):
+    d = to_dev(inp, SH_KEYS)
+    col, g = run_sh(B, d, want_campos)
+    rc = oracle.sh_fwd(inp)
+    rg = oracle.sh_bwd(inp)
+    errs = {"colors": rel_err(col, rc)}
+    for k in ("g_means", "g_coeffs") + (("g_campos",) if want_campos else ()):
+        errs[k] = rel_err(g[k], rg[k])
+    print(label, " ".join(f"{k}={v:.2e}" for k, v in errs.items()))
+    assert errs["colors"] <= FWD_TOL, (label, errs)
+    for k, v in errs.items():
+        if k != "colors":
+            assert v <= BWD_TOL, (label, k, errs)
+    return col, g, errs

@@ -1,0 +1,107 @@
+"""CPU-only checks of the C-ABI library: it loads, exports every symbol include/nasg.h declares, and
+its argument validation returns the documented codes without touching a GPU (no compute calls)."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2606_09794_b200 import binding
+    return binding
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "nasg.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b((?:nasg|sh)_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol(B):
+    names = _declared_symbols()
+    assert {"nasg_eval_fwd", "nasg_eval_bwd", "sh_eval_fwd", "sh_eval_bwd", "nasg_workspace_bytes",
+            "nasg_strerror"} <= set(names)
+    lib = C.CDLL(B.LIB_PATH)
+    for name in names:
+        assert hasattr(lib, name), name
+    assert set(B.SYMBOLS) == set(names)
+    assert "sm_100a" in B.nasg_version()
+
+
+def test_library_is_sm100a_only():
+    import subprocess
+    from paper_2606_09794_b200 import build
+    out = subprocess.run(["cuobjdump", "-lelf", build.LIB], capture_output=True, text=True).stdout
+    assert "sm_100a" in out and not re.search(r"sm_(?!100a)\d+", out), out
+
+
+def test_error_codes_without_gpu(B):
+    lib = C.CDLL(B.LIB_PATH)
+    lib.nasg_eval_fwd.restype = C.c_int
+    lib.nasg_eval_bwd.restype = C.c_int
+    lib.sh_eval_fwd.restype = C.c_int
+    lib.sh_eval_fwd.argtypes = [C.c_int64, C.c_int32] + [C.c_void_p] * 6
+    buf = (C.c_float * 64)()
+    p = C.addressof(buf)
+
+    def inputs(N=4, K=2, Cn=1, **kw):
+        d = dict(means=p, quat=p, shape=p, amp=p, dc=p, campos=p, vis=None)
+        d.update(kw)
+        return B._Inputs(N, K, Cn, d["means"], d["quat"], d["shape"], d["amp"], d["dc"], d["campos"], d["vis"])
+
+    fwd = lambda inp, colors=p, mode=1: lib.nasg_eval_fwd(C.byref(inp), C.c_void_p(colors), mode, None)
+    assert lib.nasg_eval_fwd(None, C.c_void_p(p), 1, None) == -1                 # NASG_ERR_NULL
+    assert fwd(inputs(means=None)) == -1
+    assert fwd(inputs(), colors=None) == -1
+    assert fwd(inputs(N=-1)) == -2 and fwd(inputs(Cn=0)) == -2 and fwd(inputs(Cn=65)) == -2   # SHAPE
+    assert fwd(inputs(K=6)) == -3 and fwd(inputs(K=0)) == -3                     # UNSUPPORTED_K
+    assert fwd(inputs(quat=p + 4)) == -4                                        # ALIGN
+    assert fwd(inputs(), mode=2) == -7                                          # NORM_MODE
+    assert fwd(inputs(N=0, means=None)) == 0                                    # N == 0 is a no-op
+    g = B._Grads(p, p, p, p, p, p, None, 0)
+    assert lib.nasg_eval_bwd(C.byref(inputs()), C.c_void_p(p), C.byref(g), 1, None) == -5   # WORKSPACE
+    g = B._Grads(p, p + 8, p, p, p, None, None, 0)
+    assert lib.nasg_eval_bwd(C.byref(inputs()), C.c_void_p(p), C.byref(g), 1, None) == -4   # ALIGN (g_quat)
+    assert lib.nasg_eval_bwd(C.byref(inputs()), None, C.byref(g), 1, None) == -1
+    assert lib.sh_eval_fwd(4, 0, p, p, p, None, p, None) == -2
+    assert lib.sh_eval_fwd(4, 1, None, p, p, None, p, None) == -1
+    for code in (0, -1, -2, -3, -4, -5, -7):
+        assert B.nasg_strerror(code) and "unknown" not in B.nasg_strerror(code)
+    assert "unknown" in B.nasg_strerror(-99)
+
+
+def test_workspace_sizes(B):
+    assert B.nasg_workspace_bytes(0, 4, 4) == 0
+    assert B.nasg_workspace_bytes(3_000_000, 4, 4) == ((3_000_000 + 255) // 256) * 4 * 3 * 4
+    n, k, c = 1000, 4, 4
+    need = n * 12 * 2 + 2 * 2 * k * n * 16 + 2 * k * n * 12 + 2 * n * 12 + c * n + 2 * c * n * 12
+    assert B.nasg_host_scratch_bytes(n, k, c) >= need
+    assert B.sh_host_scratch_bytes(n, c) >= 2 * n * 12 + 2 * 48 * n * 4 + c * n + 2 * c * n * 12
+
+
+def test_binding_rejects_bad_tensors(B):
+    import torch
+    N, K = 8, 2
+    t = lambda *s: torch.zeros(*s)
+    with pytest.raises(ValueError):
+        B._inputs(t(N, 3), t(K, N, 4), t(K, N, 4), t(K, 3, N), t(3, N), t(1, 3), None, device_type="cuda")
+    with pytest.raises(ValueError):
+        B._inputs(t(N, 3), t(K, N, 4), t(K, N, 3), t(K, 3, N), t(3, N), t(1, 3), None, device_type="cpu")
+    B._inputs(t(N, 3), t(K, N, 4), t(K, N, 4), t(K, 3, N), t(3, N), t(1, 3), None, device_type="cpu")
+
+
+def test_product_never_imports_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2606_09794_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle", src, flags=re.M), f
+                assert "oracle/" not in src and "nasg_ref" not in src and "sh_ref" not in src, f
+    for f in ("nasg_ref.c", "sh_ref.c", "ref.py"):
+        src = open(os.path.join(ROOT, "oracle", f)).read()
+        assert "binding" not in src and "csrc" not in src and "nasg.h" not in src, f

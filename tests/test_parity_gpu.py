@@ -1,0 +1,224 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the fp64 oracle, element by element
+on the same seeded inputs. Run on the B200 box with ``pytest -m gpu``."""
+import dataclasses
+
+import numpy as np
+import pytest
+import torch
+
+from gpu_util import (BWD_TOL, FWD_TOL, NASG_KEYS, SH_KEYS, check_nasg, check_sh, rel_err, run_nasg, run_sh,
+                      to_dev)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    from paper_2606_09794_b200 import binding
+    return binding
+
+
+@pytest.fixture(scope="module")
+def W():
+    from paper_2606_09794_b200 import workloads
+    return workloads
+
+
+# ---- element-by-element at sizes the oracle finishes in seconds (several tiles + a ragged tail) ----
+@pytest.mark.parametrize("cfg,N", [(0, None), (1, 70_001), (2, 50_003), (4, 40_007)])
+@pytest.mark.parametrize("mode", [1, 0])
+def test_nasg_configs_small(B, W, oracle, cfg, N, mode):
+    inp = W.make(cfg, N)
+    check_nasg(B, oracle, inp, mode, want_campos=True, label=f"cfg{cfg} N={inp['N']} mode={mode}")
+
+
+def test_sh_config_small(B, W, oracle):
+    inp = W.make(3, 60_001)
+    check_sh(B, oracle, inp, want_campos=True, label="cfg3 N=60001")
+
+
+@pytest.mark.parametrize("K", [1, 2, 3, 4, 5, 8])
+@pytest.mark.parametrize("C", [1, 3, 4, 5, 9])
+def test_all_lobe_counts_and_camera_tiles(B, W, oracle, K, C):
+    """Every compiled K, and camera counts that exercise the C==1 path, a partial tile, a full tile and
+    the multi-tile read-modify-write path (C > 4)."""
+    cfg = dataclasses.replace(W.CONFIGS[2], seed=50 + K * 10 + C, K=K, C=C)
+    inp = W.make_nasg(cfg, N=2_000 + 37 * K + C)
+    check_nasg(B, oracle, inp, 1, want_campos=True, label=f"K={K} C={C}")
+
+
+@pytest.mark.parametrize("C", [1, 2, 6])
+def test_sh_camera_tiles(B, W, oracle, C):
+    cfg = dataclasses.replace(W.CONFIGS[3], seed=70 + C, C=C)
+    inp = W.make_sh(cfg, N=3_011)
+    check_sh(B, oracle, inp, want_campos=True, label=f"sh C={C}")
+
+
+# ---- full BASELINE sizes, launch configuration of bench.py: sampled outputs + size-independent properties ----
+def _sampled_check_nasg(B, W, oracle, cfg, n_sample=30_000):
+    inp = W.make(cfg)
+    d = to_dev(inp, NASG_KEYS)
+    col, g = run_nasg(B, d, 1)
+    N = inp["N"]
+    rng = np.random.default_rng(999 + cfg)
+    idx = np.unique(np.concatenate([rng.integers(0, N, n_sample), [0, 1, 255, 256, N - 257, N - 2, N - 1]]))
+    sub = W.take(inp, idx)
+    rc = oracle.nasg_fwd(sub, 1)
+    rg = oracle.nasg_bwd(sub, 1)
+    ti = torch.from_numpy(idx).cuda()
+    errs = {"colors": rel_err(col[:, ti], rc), "g_means": rel_err(g["g_means"][ti], rg["g_means"]),
+            "g_quat": rel_err(g["g_quat"][:, ti], rg["g_quat"]), "g_shape": rel_err(g["g_shape"][:, ti], rg["g_shape"]),
+            "g_amp": rel_err(g["g_amp"][:, :, ti], rg["g_amp"]), "g_dc": rel_err(g["g_dc"][:, ti], rg["g_dc"])}
+    print(f"cfg{cfg} full N={N} sampled {idx.size}:", " ".join(f"{k}={v:.2e}" for k, v in errs.items()))
+    assert errs.pop("colors") <= FWD_TOL
+    for k, v in errs.items():
+        assert v <= BWD_TOL, (k, v)
+    # properties that hold at any size
+    assert torch.isfinite(col).all() and all(torch.isfinite(v).all() for k, v in g.items())
+    if d["vis"] is not None:
+        v = d["vis"] != 0
+        assert (col[~v] == 0).all()                                        # culled pairs are exactly 0
+        want_dc = (d["g_colors"] * v[:, :, None]).sum(0).T.contiguous()    # g_c0 = sum_c vis g_col
+        assert (g["g_dc"] - want_dc).abs().max() <= 1e-5 * want_dc.abs().max()
+        dead = ~v.any(0)
+        assert (g["g_means"][dead] == 0).all() and (g["g_quat"][:, dead] == 0).all() and (g["g_amp"][:, :, dead] == 0).all()
+    else:
+        assert torch.equal(g["g_dc"], d["g_colors"][0].T.contiguous())
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 4])
+def test_nasg_full_size_sampled(B, W, oracle, cfg):
+    _sampled_check_nasg(B, W, oracle, cfg)
+    torch.cuda.empty_cache()
+
+
+def test_sh_full_size_sampled(B, W, oracle):
+    inp = W.make(3)
+    d = to_dev(inp, SH_KEYS)
+    col, g = run_sh(B, d)
+    N = inp["N"]
+    idx = np.unique(np.concatenate([np.random.default_rng(1002).integers(0, N, 30_000), [0, 255, 256, N - 1]]))
+    sub = W.take(inp, idx)
+    rc, rg = oracle.sh_fwd(sub), oracle.sh_bwd(sub)
+    ti = torch.from_numpy(idx).cuda()
+    assert rel_err(col[:, ti], rc) <= FWD_TOL
+    assert rel_err(g["g_means"][ti], rg["g_means"]) <= BWD_TOL
+    assert rel_err(g["g_coeffs"][:, :, ti], rg["g_coeffs"]) <= BWD_TOL
+    assert (col[d["vis"] == 0] == 0).all()
+    torch.cuda.empty_cache()
+
+
+# ---- edge cases -------------------------------------------------------------------------------
+@pytest.mark.parametrize("N", [1, 31, 255, 256, 257])
+def test_tiny_and_ragged_sizes(B, W, oracle, N):
+    check_nasg(B, oracle, W.make(2, N), 1, want_campos=True, label=f"N={N}")
+    check_sh(B, oracle, W.make(3, N), want_campos=True, label=f"sh N={N}")
+
+
+def test_empty_input_is_a_noop(B):
+    z = lambda *s, dt=torch.float32: torch.zeros(*s, dtype=dt, device="cuda")
+    col = B.nasg_eval_fwd(z(0, 3), z(2, 0, 4), z(2, 0, 4), z(2, 3, 0), z(3, 0), z(1, 3))
+    assert col.shape == (1, 0, 3)
+    g = B.nasg_eval_bwd(z(0, 3), z(2, 0, 4), z(2, 0, 4), z(2, 3, 0), z(3, 0), z(1, 3), z(1, 0, 3), want_campos=True)
+    torch.cuda.synchronize()
+    assert (g["g_campos"] == 0).all()
+    assert B.sh_eval_fwd(z(0, 3), z(16, 3, 0), z(2, 3)).shape == (2, 0, 3)
+
+
+def test_all_culled_and_all_visible_masks(B, W, oracle):
+    inp = W.make(2, 1_500)
+    dead = dict(inp, vis=np.zeros_like(inp["vis"]))
+    col, g, _ = check_nasg(B, oracle, dead, 1, want_campos=True, label="all culled")
+    assert (col == 0).all() and all((g[k] == 0).all() for k in ("g_means", "g_quat", "g_shape", "g_amp", "g_dc", "g_campos"))
+    full = dict(inp, vis=np.ones_like(inp["vis"]))
+    c1, g1, _ = check_nasg(B, oracle, full, 1, label="all visible (mask)")
+    c2, g2, _ = check_nasg(B, oracle, dict(inp, vis=None), 1, label="all visible (NULL)")
+    assert torch.equal(c1, c2) and all(torch.equal(g1[k], g2[k]) for k in g2)
+
+
+def test_optional_gradient_pointers_and_determinism(B, W):
+    inp = W.make(2, 20_011)
+    d = to_dev(inp, NASG_KEYS)
+    _, g_all = run_nasg(B, d, 1, want_campos=True)
+    _, g_again = run_nasg(B, d, 1, want_campos=True)
+    for k in ("g_means", "g_quat", "g_shape", "g_amp", "g_dc", "g_campos"):
+        assert torch.equal(g_all[k], g_again[k]), k                       # bit-identical reruns (no atomics)
+    only = {"g_shape": torch.full_like(g_all["g_shape"], 7.0)}
+    B.nasg_eval_bwd(d["means"], d["quat"], d["shape"], d["amp"], d["dc"], d["campos"], d["g_colors"], d["vis"], 1, out=only)
+    torch.cuda.synchronize()
+    assert torch.equal(only["g_shape"], g_all["g_shape"])
+
+
+def test_direction_on_the_lobe_axis_is_finite(B, oracle):
+    """d = +z and d = -z (reading R11: parity unpinned there; the kernel must stay finite)."""
+    N = 4
+    q = np.tile(np.array([1.0, 0, 0, 0], np.float32), (1, N, 1))
+    means = np.array([[0, 0, 3], [0, 0, -3], [0, 0, 3], [0, 0, -3]], np.float32)
+    inp = dict(N=N, K=1, C=1, means=means, campos=np.zeros((1, 3), np.float32), quat=q,
+               shape=np.tile(np.array([3.0, 1.0, 2.0, 0.3], np.float32), (1, N, 1)), amp=np.ones((1, 3, N), np.float32),
+               dc=np.zeros((3, N), np.float32), vis=None, g_colors=np.ones((1, N, 3), np.float32))
+    d = to_dev(inp, NASG_KEYS)
+    col, g = run_nasg(B, d, 1)
+    assert torch.isfinite(col).all() and all(torch.isfinite(v).all() for v in g.values())
+    ref = oracle.nasg_fwd(inp, 1)
+    assert abs(col[0, 0, 0].item() - ref[0, 0, 0]) <= 1e-5 * abs(ref[0, 0, 0])      # value at +z follows eq.(9)
+    assert abs(col[0, 1, 0].item()) <= 1e-6                                        # value at -z is 0
+
+
+def test_unnormalised_quaternions(B, W, oracle):
+    inp = W.make(1, 5_000)
+    scale = np.random.default_rng(3).uniform(0.1, 10.0, size=inp["quat"].shape[:2] + (1,)).astype(np.float32)
+    check_nasg(B, oracle, dict(inp, quat=inp["quat"] * scale), 1, label="unnormalised q")
+
+
+def test_host_entry_point_matches_device_path(B, W):
+    inp = W.make(2, 30_001)
+    d = to_dev(inp, NASG_KEYS)
+    col, g = run_nasg(B, d, 1, want_campos=True)
+    host = {k: (None if inp.get(k) is None else torch.from_numpy(np.ascontiguousarray(inp[k])).pin_memory()) for k in NASG_KEYS}
+    N, K, C = inp["N"], inp["K"], inp["C"]
+    out = dict(colors=torch.empty((C, N, 3)).pin_memory(), g_means=torch.empty((N, 3)).pin_memory(),
+               g_quat=torch.empty((K, N, 4)).pin_memory(), g_shape=torch.empty((K, N, 4)).pin_memory(),
+               g_amp=torch.empty((K, 3, N)).pin_memory(), g_dc=torch.empty((3, N)).pin_memory(),
+               g_campos=torch.empty((C, 3)).pin_memory())
+    scratch = torch.empty(B.nasg_host_scratch_bytes(N, K, C), dtype=torch.uint8, device="cuda")
+    B.nasg_eval_fwd_bwd_host(host, out, scratch, 1)
+    torch.cuda.synchronize()
+    assert torch.equal(out["colors"], col.cpu())
+    for k in ("g_means", "g_quat", "g_shape", "g_amp", "g_dc", "g_campos"):
+        assert torch.equal(out[k], g[k].cpu()), k
+    # SH twin
+    inp = W.make(3, 10_007)
+    d = to_dev(inp, SH_KEYS)
+    col, g = run_sh(B, d, want_campos=True)
+    host = {k: torch.from_numpy(np.ascontiguousarray(inp[k])).pin_memory() for k in SH_KEYS}
+    N, C = inp["N"], inp["C"]
+    out = dict(colors=torch.empty((C, N, 3)).pin_memory(), g_means=torch.empty((N, 3)).pin_memory(),
+               g_coeffs=torch.empty((16, 3, N)).pin_memory(), g_campos=torch.empty((C, 3)).pin_memory())
+    scratch = torch.empty(B.sh_host_scratch_bytes(N, C), dtype=torch.uint8, device="cuda")
+    B.sh_eval_fwd_bwd_host(host, out, scratch)
+    torch.cuda.synchronize()
+    assert torch.equal(out["colors"], col.cpu()) and torch.equal(out["g_coeffs"], g["g_coeffs"].cpu())
+    assert torch.equal(out["g_means"], g["g_means"].cpu()) and torch.equal(out["g_campos"], g["g_campos"].cpu())
+
+
+def test_runs_on_a_side_stream_and_in_a_cuda_graph(B, W):
+    inp = W.make(1, 40_000)
+    d = to_dev(inp, NASG_KEYS)
+    col, g = run_nasg(B, d, 1)
+    s = torch.cuda.Stream()
+    out = torch.empty_like(col)
+    grads = B.nasg_alloc_grads(inp["K"], inp["N"], inp["C"], "cuda")
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        B.nasg_eval_fwd(d["means"], d["quat"], d["shape"], d["amp"], d["dc"], d["campos"], None, 1, out=out, stream=s)  # warm
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=s):
+            B.nasg_eval_fwd(d["means"], d["quat"], d["shape"], d["amp"], d["dc"], d["campos"], None, 1, out=out, stream=s)
+            B.nasg_eval_bwd(d["means"], d["quat"], d["shape"], d["amp"], d["dc"], d["campos"], d["g_colors"], None, 1,
+                            out=grads, stream=s)
+    out.zero_()
+    graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(out, col) and torch.equal(grads["g_quat"], g["g_quat"])
