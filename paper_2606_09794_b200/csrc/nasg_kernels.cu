@@ -174,17 +174,15 @@ __global__ void __launch_bounds__(BLOCK, 2) nasg_bwd_kernel(BwdParams p)
                             gw[2] = fmaf(gc[t][2], G, gw[2]);
                             const float gGG = gG * G;
                             // ln(pE) = 2 lambda (kappa' - 1) + tau ln kappa, kappa' = kappa^(1+tau)
-                            const float A_tau = T.Lk * fmaf(L.lam2, T.kp, 1.0f);                    // d/d tau
-                            const float A_kap2 = fmaf(L.lam2 * (1.0f + T.tau), T.kp, T.tau)          // (d/d kappa)/2
-                                                 * T.inv_2kappa;
-                            const float tau_u = 2.0f * L.a * T.u * T.inv_s2;                         // eq.(57)
-                            const float tau_v = 2.0f * T.tau * T.v * T.inv_s2;                       // eq.(61)
-                            const float hs = 0.5f * gG * T.Gbar * T.sn;                              // carrier terms, eqs.(59),(65)
-                            const float gu = fmaf(gGG * A_tau, tau_u, -hs * L.k);                    // gG dG/du
-                            const float gv = gGG * fmaf(A_tau, tau_v, A_kap2);                       // gG dG/dv
+                            const float A_tau = T.Lk * fmaf(B.lam2, T.kp, 1.0f);                    // d/d tau
+                            const float A_kap2 = fmaf(B.lam2 * (1.0f + T.tau), T.kp, T.tau) * T.inv_2kappa; // (d/d kappa)/2
+                            const float B1 = 2.0f * gGG * A_tau * T.inv_s2;
+                            const float hs = gG * T.Gh * T.sn;                                       // carrier terms, eqs.(59),(65)
+                            const float gu = fmaf(B1 * L.a, T.u, -hs * B.k);                         // gG dG/du, tau_u = 2 a u / s^2 (eq.57)
+                            const float gv = fmaf(B1 * T.tau, T.v, gGG * A_kap2);                    // gG dG/dv, tau_v = 2 tau v / s^2 (eq.61)
                             S0 += gGG;
                             S1 = fmaf(gGG, T.em1, S1);
-                            S2 = fmaf(gGG * A_tau, T.c2, S2);
+                            S2 = fmaf(B1, T.uu, S2);                                                 // 2 gGG A_tau c2 (halved below)
                             Sk = fmaf(hs, T.u, Sk);
                             Sp += hs;
                             gX0 = fmaf(gu, dx[t], gX0); gX1 = fmaf(gu, dy[t], gX1); gX2 = fmaf(gu, dz[t], gX2);  // eq.(60)
@@ -195,8 +193,8 @@ __global__ void __launch_bounds__(BLOCK, 2) nasg_bwd_kernel(BwdParams p)
                         }
                     }
                     // shape: (lambda, a) = (e^{l2}, e^{l1-l2} - 1)
-                    gs[0] = fmaf(S2, B.one_pa, -S0 * B.nA);
-                    gs[1] = fmaf(L.lam2, S1, -S0 * B.nL) - gs[0];
+                    gs[0] = fmaf(0.5f * S2, B.one_pa, -S0 * B.nA);
+                    gs[1] = fmaf(B.lam2, S1, -S0 * B.nL) - gs[0];
                     gs[2] = -fmaf(S0, B.nk, Sk);
                     gs[3] = -Sp;
                     // frame: transpose Jacobian of columns X and Z of R(qhat), then qhat = q/|q|

@@ -6,10 +6,14 @@
 // DESIGN.md §5, because the literal transcription loses the 1e-5 parity bar exactly where sharp
 // lobes are bright:
 //   * s^2 = 1-(d.z)^2 is formed as (d.x)^2 + (d.y)^2, never by subtraction;
-//   * 1-kappa = s^2/(2(1+v)) for v > 0, ln kappa = log1p(-(1-kappa)) by polynomial when it is small;
-//   * 2 lambda (kappa^(1+tau) - 1) uses an expm1 polynomial when the argument is small;
-//   * MUFU approximations (ex2, lg2, sin, cos, rcp, rsqrt) only where their error is relative to the
-//     exponent or otherwise bounded well inside the tolerance (DESIGN.md §5 table).
+//   * q = (1-|v|)/2 = s^2/(2(1+|v|)) is 1-kappa on the lobe side and kappa on the far side, so neither
+//     1-v nor 1+v is formed by a cancelling subtraction; log2(kappa) = log2(1-q) by series for small q;
+//   * kappa^(1+tau) - 1 uses an exp2m1 series when the argument is small;
+//   * exponents are kept in base 2 (one ex2 for p*E/I including the normaliser), and MUFU
+//     approximations (ex2, lg2, sin, cos, rcp, rsqrt) are used only where their error is relative to
+//     the exponent or otherwise bounded well inside the tolerance (DESIGN.md §5 table).
+// The XU (MUFU) pipe issues 16 lanes/clk/SM on B200 (measured, profiles/), 1/8 of the FP32 rate, so
+// every reciprocal that can be shared is shared: 5 MUFU per forward lobe evaluation, 6 backward.
 #pragma once
 
 #include <cuda_runtime.h>
@@ -19,108 +23,63 @@
 
 namespace nasg {
 
-// ---------------------------------------------------------------------------------------------
-// MUFU wrappers (one SFU instruction each on the device)
-// ---------------------------------------------------------------------------------------------
-NASG_HD float f_rcp(float x)
-{
-#ifdef __CUDA_ARCH__
-    float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r;
-#else
-    return 1.0f / x;
-#endif
-}
-NASG_HD float f_rsqrt(float x)
-{
-#ifdef __CUDA_ARCH__
-    float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r;
-#else
-    return 1.0f / sqrtf(x);
-#endif
-}
-NASG_HD float f_sqrt(float x)
-{
-#ifdef __CUDA_ARCH__
-    float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r;
-#else
-    return sqrtf(x);
-#endif
-}
-NASG_HD float f_ex2(float x)
-{
-#ifdef __CUDA_ARCH__
-    float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r;
-#else
-    return exp2f(x);
-#endif
-}
-NASG_HD float f_lg2(float x)
-{
-#ifdef __CUDA_ARCH__
-    float r; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r;
-#else
-    return log2f(x);
-#endif
-}
-NASG_HD float f_exp(float x) { return f_ex2(x * 1.4426950408889634f); }
-
-// sin and cos of theta after a two-constant Cody-Waite reduction to [-pi, pi] (|theta| <~ 1e3)
-NASG_HD void f_sincos(float theta, float &sn, float &cs)
-{
-    float n = rintf(theta * 0.15915494309189535f);
-    float r = fmaf(n, -6.2831854820251465f, theta);     // 2pi hi (fp32)
-    r = fmaf(n, 1.7484555e-7f, r);                      // 2pi lo: 2pi = hi - 1.7484555e-7
-#ifdef __CUDA_ARCH__
-    asm("sin.approx.ftz.f32 %0, %1;" : "=f"(sn) : "f"(r));
-    asm("cos.approx.ftz.f32 %0, %1;" : "=f"(cs) : "f"(r));
-#else
-    sn = sinf(r); cs = cosf(r);
-#endif
-}
-NASG_HD float f_cos(float theta)
-{
-    float n = rintf(theta * 0.15915494309189535f);
-    float r = fmaf(n, -6.2831854820251465f, theta);
-    r = fmaf(n, 1.7484555e-7f, r);
-#ifdef __CUDA_ARCH__
-    float cs; asm("cos.approx.ftz.f32 %0, %1;" : "=f"(cs) : "f"(r)); return cs;
-#else
-    return cosf(r);
-#endif
-}
+constexpr float LOG2E = 1.4426950408889634f;
+constexpr float LN2 = 0.6931471805599453f;
+constexpr float TWO_PI = 6.283185307179586f;
+constexpr float INV_TWO_PI = 0.15915494309189535f;
+constexpr float TINY = 1e-30f;
 
 // ---------------------------------------------------------------------------------------------
-// accurate small-argument helpers
+// MUFU wrappers (one XU instruction each on the device)
 // ---------------------------------------------------------------------------------------------
-// ln(kappa) where kappa = 1-q if `upper` (v > 0: q = 1-kappa is small near the lobe axis) else kappa = q
-// (v <= 0: kappa itself is small near the antipode). Polynomial -q(1 + q/2 + ...) for q < 1/8 on the
-// upper side (relative error < 1e-7), lg2 otherwise (its absolute error 2^-22 is then < 2e-6 relative).
-NASG_HD float log_kappa(float q, bool upper)
+#ifdef __CUDA_ARCH__
+#define NASG_MUFU(name, ptx, hostexpr)                                                             \
+    NASG_HD float name(float x) { float r; asm(ptx " %0, %1;" : "=f"(r) : "f"(x)); return r; }
+#else
+#define NASG_MUFU(name, ptx, hostexpr) NASG_HD float name(float x) { return hostexpr; }
+#endif
+NASG_MUFU(f_rcp, "rcp.approx.ftz.f32", 1.0f / x)
+NASG_MUFU(f_rsqrt, "rsqrt.approx.ftz.f32", 1.0f / sqrtf(x))
+NASG_MUFU(f_ex2, "ex2.approx.ftz.f32", exp2f(x))
+NASG_MUFU(f_lg2, "lg2.approx.ftz.f32", log2f(x))
+NASG_MUFU(f_sin, "sin.approx.ftz.f32", sinf(x))
+NASG_MUFU(f_cos, "cos.approx.ftz.f32", cosf(x))
+#undef NASG_MUFU
+NASG_HD float f_exp(float x) { return f_ex2(x * LOG2E); }
+// angle given in TURNS (theta/2pi): exact reduction to [-1/2,1/2] turns, then radians in [-pi,pi]
+NASG_HD float reduce_turns(float t) { return TWO_PI * (t - rintf(t)); }
+
+// ---------------------------------------------------------------------------------------------
+// accurate small-argument helpers (base 2)
+// ---------------------------------------------------------------------------------------------
+// log2(kappa) where kappa = 1-q if `upper` (v > 0: q is small near the lobe axis) else kappa = q.
+// Series -log2e q (1 + q/2 + ... + q^5/6) for q < 1/16 on the upper side (truncation 8e-9 relative);
+// lg2.approx otherwise (absolute error 2^-22 on |log2| >= 0.093: < 3e-6 relative, and an error that is
+// relative to the exponent only perturbs G by |exponent| * 3e-6, which is largest, 1e-6 of the lobe
+// peak, at exponent -1).
+NASG_HD float log2_kappa(float q, bool upper)
 {
-    float p = fmaf(q, 0.11111111f, 0.125f);
-    p = fmaf(q, p, 0.14285714f);
-    p = fmaf(q, p, 0.16666667f);
-    p = fmaf(q, p, 0.2f);
-    p = fmaf(q, p, 0.25f);
-    p = fmaf(q, p, 0.33333333f);
-    p = fmaf(q, p, 0.5f);
-    p = fmaf(q, p, 1.0f);
-    float small = -q * p;
-    float big = 0.6931471805599453f * f_lg2(upper ? 1.0f - q : q);
-    return (upper && q < 0.125f) ? small : big;
+    float p = fmaf(q, -LOG2E / 6.0f, -LOG2E / 5.0f);
+    p = fmaf(q, p, -LOG2E / 4.0f);
+    p = fmaf(q, p, -LOG2E / 3.0f);
+    p = fmaf(q, p, -LOG2E / 2.0f);
+    p = fmaf(q, p, -LOG2E);
+    const float small = q * p;
+    const float big = f_lg2(upper ? 1.0f - q : q);
+    return (upper && q < 0.0625f) ? small : big;
 }
-// e^x - 1 for x <= 0. Polynomial for |x| < 1/8, ex2 otherwise.
-NASG_HD float expm1_neg(float x)
+// 2^x - 1 for x <= 0; also returns 2^x. Series for |x| < 1/8 (truncation 7e-9 relative), ex2 otherwise.
+NASG_HD float exp2m1_neg(float x, float &two_x)
 {
-    float p = fmaf(x, 1.9841270e-4f, 1.3888889e-3f);
-    p = fmaf(x, p, 8.3333333e-3f);
-    p = fmaf(x, p, 4.1666667e-2f);
-    p = fmaf(x, p, 0.16666667f);
-    p = fmaf(x, p, 0.5f);
-    p = fmaf(x, p, 1.0f);
-    float small = x * p;
-    float big = f_exp(x) - 1.0f;
-    return x > -0.125f ? small : big;
+    float p = fmaf(x, 1.3333558e-3f, 9.6181291e-3f);   // ln2^5/120, ln2^4/24
+    p = fmaf(x, p, 5.5504109e-2f);                       // ln2^3/6
+    p = fmaf(x, p, 0.24022651f);                         // ln2^2/2
+    p = fmaf(x, p, LN2);
+    const float small = x * p;
+    const float e = f_ex2(x);
+    const bool s = x > -0.125f;
+    two_x = s ? small + 1.0f : e;
+    return s ? small : e - 1.0f;
 }
 // g(x) = (x coth x - 1)/x^2, x > 0   (d ln sinhc(x)/dx = x g(x))
 NASG_HD float g_fun(float x)
@@ -142,83 +101,86 @@ NASG_HD float g_fun(float x)
 // ---------------------------------------------------------------------------------------------
 struct Lobe {
     float Xx, Xy, Xz, Yx, Yy, Yz, Zx, Zy, Zz; // columns of R(q/|q|)
-    float lam2;                                // 2 lambda
     float a;                                   // Lambda/lambda - 1
-    float k, phi;
-    float invI;                                // 1 / normalising integral
+    float lam2e;                               // 2 lambda log2(e)
+    float kt, pt;                              // k/2pi, phi/2pi (carrier angle in turns)
+    float lgI;                                 // log2(1/(2 I)): normaliser and the carrier's 1/2, folded into the exponent
 };
 struct LobeBwd {        // extra camera-independent terms of the backward pass
     float qw, qx, qy, qz, inv_qn;  // unit quaternion and 1/|q|
+    float lam2, k;                 // 2 lambda, k
     float one_pa;                  // 1 + a = Lambda/lambda
     float nA;                      // (1+a) d ln I / d a        = -1/2 + Lambda D
     float nL;                      // lambda d ln I / d lambda  = 2 lambda e^{-2 lambda}/(1-e^{-2 lambda}) - 1 + Lambda D
     float nk;                      // d ln I / d k
 };
 
-// Normaliser 1/I of eq.(10) (EXACT) or of NASG (approximate), and, if GRAD, the log-derivative terms.
+// lgI = log2(1/(2I)) for I of eq.(10) (EXACT) or of NASG (approximate); if GRAD also the
+// log-derivative terms of I. D = Psi_Lambda/(1+Psi).
 template <bool EXACT, bool GRAD>
-NASG_HD void normaliser(float l1, float l2, float Lam, float lam, float k, float &invI, float &nA,
+NASG_HD void normaliser(float l1, float l2, float Lam, float lam, float k, float &lgI, float &nA,
                         float &nL, float &nk)
 {
-    const float INV_PI = 0.3183098861837907f;
-    float em = f_exp(-2.0f * lam);
-    float one_m = lam > 0.5f ? 1.0f - em : -expm1f(-2.0f * lam);
-    float root = f_exp(0.5f * (l1 + l2));                   // lambda sqrt(1+a) = sqrt(lambda Lambda)
-    float inv_base = root * INV_PI * f_rcp(one_m);          // 1 / (pi (1-e^{-2 lambda})/(lambda sqrt(1+a)))
+    const float em = f_exp(-2.0f * lam);
+    const float one_m = lam > 0.5f ? 1.0f - em : -expm1f(-2.0f * lam);   // 1 - e^{-2 lambda}, epsilon = 0 (R8)
+    // 1/(2I) = lambda sqrt(1+a) / (2 pi (1-e^{-2 lambda}) (1+Psi));  lambda sqrt(1+a) = e^{(l1+l2)/2}
+    const float lg_root = 0.5f * LOG2E * (l1 + l2);
     float dl = 0.f;
-    if (GRAD) dl = 2.0f * lam * em * f_rcp(one_m) - 1.0f;   // lambda d ln(base)/d lambda
+    if (GRAD) dl = 2.0f * lam * em * f_rcp(one_m) - 1.0f;                 // lambda d ln(base)/d lambda
     if (!EXACT) {
-        invI = 0.5f * inv_base;
+        lgI = lg_root - f_lg2(2.0f * TWO_PI * one_m);                     // NASG: I = 2 pi (1-e^{-2 lambda})/(lambda sqrt(1+a))
         if (GRAD) { nA = -0.5f; nL = dl; nk = 0.f; }
         return;
     }
-    float s = (Lam - k) * (Lam + k);                        // Lambda^2 - k^2
-    float Psi, LD, dk;                                      // Psi, Lambda dPsi/dLambda, dPsi/dk
+    const float s = (Lam - k) * (Lam + k);                                // Lambda^2 - k^2
+    float Psi, LD = 0.f, dk = 0.f;                                        // Psi, Lambda dPsi/dLambda, dPsi/dk
     if (s > 0.05f) {
         // k < Lambda:  Psi = (Lambda/r) e^{r-Lambda} (1-e^{-2r})/(1-e^{-2 Lambda}),  r-Lambda = -k^2/(Lambda+r)
-        float r = f_sqrt(s);
-        float ir = f_rcp(r);
-        float del = k * k * f_rcp(Lam + r);                 // Lambda - r
-        float e2r = f_exp(-2.0f * r), e2L = f_exp(-2.0f * Lam);
-        Psi = Lam * ir * f_exp(-del) * (1.0f - e2r) * f_rcp(1.0f - e2L);
+        const float ir = f_rsqrt(s), r = s * ir;
+        const float del = k * k * f_rcp(Lam + r);                         // Lambda - r
+        const float e2r = f_exp(-2.0f * r), e2L = f_exp(-2.0f * Lam);
+        const float i1L = f_rcp(1.0f - e2L);
+        Psi = Lam * ir * f_exp(-del) * (1.0f - e2r) * i1L;
         if (GRAD) {
-            float gr = g_fun(r), dg;
+            const float gr = g_fun(r);
+            float dg;
             if (r >= 4.0f) {
                 // g(r) - g(Lambda) without cancellation
-                float iL = f_rcp(Lam);
-                float tail = 2.0f * (ir * e2r * f_rcp(1.0f - e2r) - iL * e2L * f_rcp(1.0f - e2L));
+                const float iL = f_rcp(Lam);
+                const float tail = 2.0f * (ir * e2r * f_rcp(1.0f - e2r) - iL * e2L * i1L);
                 dg = fmaf(del * ir * iL, 1.0f - (Lam + r) * ir * iL, tail);
             } else {
                 dg = gr - g_fun(Lam);
             }
-            LD = Psi * Lam * Lam * dg;                      // Lambda dPsi/dLambda = Psi Lambda^2 (g(r)-g(Lambda))
+            LD = Psi * Lam * Lam * dg;                                    // = Psi Lambda^2 (g(r) - g(Lambda))
             dk = -Psi * k * gr;
         }
     } else {
-        // k >= Lambda (or |s| tiny): S(s) = sinhc(sqrt(s)) continued to s < 0, S' = dS/ds
+        // k >= Lambda (or |s| tiny): S(s) = sinhc(sqrt(s)) continued to s < 0 (reading R4), S' = dS/ds
         float S, Sp;
         if (s > -0.05f) {
             S = fmaf(s, fmaf(s, fmaf(s, 1.9841270e-4f, 8.3333333e-3f), 0.16666667f), 1.0f);
             Sp = fmaf(s, fmaf(s, fmaf(s, 1.1022928e-5f, 5.9523810e-4f), 1.6666667e-2f), 0.16666667f);
         } else {
-            float rho = f_sqrt(-s), sn, cs;
-            f_sincos(rho, sn, cs);
-            S = sn * f_rcp(rho);
-            Sp = (cs - S) * f_rcp(2.0f * s);
+            const float irho = f_rsqrt(-s), rho = -s * irho;
+            const float ang = reduce_turns(rho * INV_TWO_PI);
+            S = f_sin(ang) * irho;
+            Sp = (f_cos(ang) - S) * f_rcp(2.0f * s);
         }
-        float eL = f_exp(-Lam);
-        float ish = 2.0f * eL * f_rcp(1.0f - eL * eL);      // 1/sinh(Lambda)
+        const float eL = f_exp(-Lam);
+        const float i1L = f_rcp(1.0f - eL * eL);
+        const float ish = 2.0f * eL * i1L;                                // 1/sinh(Lambda)
         Psi = Lam * S * ish;
         if (GRAD) {
-            float coth = (1.0f + eL * eL) * f_rcp(1.0f - eL * eL);
+            const float coth = (1.0f + eL * eL) * i1L;
             LD = Psi + 2.0f * Lam * Lam * Lam * Sp * ish - Psi * Lam * coth;
             dk = -2.0f * k * Lam * Sp * ish;
         }
     }
-    float i1p = f_rcp(1.0f + Psi);
-    invI = inv_base * i1p;
+    lgI = lg_root - f_lg2(TWO_PI * one_m * (1.0f + Psi));
     if (GRAD) {
-        float LamD = LD * i1p;
+        const float i1p = f_rcp(1.0f + Psi);
+        const float LamD = LD * i1p;
         nA = -0.5f + LamD;
         nL = dl + LamD;
         nk = dk * i1p;
@@ -228,22 +190,25 @@ NASG_HD void normaliser(float l1, float l2, float Lam, float lam, float k, float
 template <bool EXACT, bool GRAD>
 NASG_HD void lobe_setup(const float4 q, const float4 sp, Lobe &L, LobeBwd &B)
 {
-    float inv_qn = f_rsqrt(q.x * q.x + q.y * q.y + q.z * q.z + q.w * q.w);
-    // one Newton step: the frame error would otherwise be 2^-22 relative on every axis
-    inv_qn = inv_qn * fmaf(-0.5f * (q.x * q.x + q.y * q.y + q.z * q.z + q.w * q.w), inv_qn * inv_qn, 1.5f);
-    float w = q.x * inv_qn, x = q.y * inv_qn, y = q.z * inv_qn, z = q.w * inv_qn;
-    L.Xx = 1.0f - 2.0f * (y * y + z * z); L.Xy = 2.0f * (x * y + w * z); L.Xz = 2.0f * (x * z - w * y);
-    L.Yx = 2.0f * (x * y - w * z); L.Yy = 1.0f - 2.0f * (x * x + z * z); L.Yz = 2.0f * (y * z + w * x);
-    L.Zx = 2.0f * (x * z + w * y); L.Zy = 2.0f * (y * z - w * x); L.Zz = 1.0f - 2.0f * (x * x + y * y);
-    float Lam = expf(sp.x), lam = expf(sp.y);
-    float one_pa = f_exp(sp.x - sp.y);
-    L.lam2 = 2.0f * lam;
+    const float qq = q.x * q.x + q.y * q.y + q.z * q.z + q.w * q.w;
+    float inv_qn = f_rsqrt(qq);
+    inv_qn = inv_qn * fmaf(-0.5f * qq, inv_qn * inv_qn, 1.5f);            // one Newton step
+    const float w = q.x * inv_qn, x = q.y * inv_qn, y = q.z * inv_qn, z = q.w * inv_qn;
+    const float x2 = x + x, y2 = y + y, z2 = z + z;
+    L.Xx = 1.0f - fmaf(y2, y, z2 * z); L.Xy = fmaf(x2, y, z2 * w); L.Xz = fmaf(x2, z, -y2 * w);
+    L.Yx = fmaf(x2, y, -z2 * w); L.Yy = 1.0f - fmaf(x2, x, z2 * z); L.Yz = fmaf(y2, z, x2 * w);
+    L.Zx = fmaf(x2, z, y2 * w); L.Zy = fmaf(y2, z, -x2 * w); L.Zz = 1.0f - fmaf(x2, x, y2 * y);
+    // relative errors of Lambda, lambda only scale the exponent (benign), so ex2.approx is enough
+    const float Lam = f_exp(sp.x), lam = f_exp(sp.y);
+    const float one_pa = f_exp(sp.x - sp.y);
     L.a = fmaxf(one_pa - 1.0f, 0.0f);
-    L.k = sp.z; L.phi = sp.w;
+    L.lam2e = 2.0f * LOG2E * lam;
+    L.kt = sp.z * INV_TWO_PI; L.pt = sp.w * INV_TWO_PI;
     float nA = 0.f, nL = 0.f, nk = 0.f;
-    normaliser<EXACT, GRAD>(sp.x, sp.y, Lam, lam, sp.z, L.invI, nA, nL, nk);
+    normaliser<EXACT, GRAD>(sp.x, sp.y, Lam, lam, sp.z, L.lgI, nA, nL, nk);
     if (GRAD) {
         B.qw = w; B.qx = x; B.qy = y; B.qz = z; B.inv_qn = inv_qn;
+        B.lam2 = 2.0f * lam; B.k = sp.z;
         B.one_pa = one_pa; B.nA = nA; B.nL = nL; B.nk = nk;
     }
 }
@@ -252,43 +217,40 @@ NASG_HD void lobe_setup(const float4 q, const float4 sp, Lobe &L, LobeBwd &B)
 // per (lobe, camera) evaluation
 // ---------------------------------------------------------------------------------------------
 struct EvalTerms {      // what the backward needs from the recomputed forward
-    float u, v, c2, inv_s2, tau, Lk, kp, em1, inv_2kappa, Gbar, H, sn;
+    float u, v, uu, inv_s2, tau, Lk, kp, em1, inv_2kappa, Gh, sn;
 };
 
-// G = H p E / I at direction (dx,dy,dz). If T != nullptr-like (FULL), also fills the terms for backward.
+// G = H p E / I at direction (dx,dy,dz) (eq.(9) over eq.(10)). With FULL also fills the terms the
+// backward needs. MUFU count: rcp, lg2, ex2, ex2, cos (+ sin with FULL).
 template <bool FULL>
 NASG_HD float lobe_eval(const Lobe &L, float dx, float dy, float dz, EvalTerms &T)
 {
-    float u = fmaf(dx, L.Xx, fmaf(dy, L.Xy, dz * L.Xz));
-    float om = fmaf(dx, L.Yx, fmaf(dy, L.Yy, dz * L.Yz));
-    float v = fmaf(dx, L.Zx, fmaf(dy, L.Zy, dz * L.Zz));
-    float s2 = fmaxf(fmaf(u, u, om * om), 1e-30f);          // 1 - v^2 without cancellation
-    float inv_s2 = f_rcp(s2);
-    float c2 = u * u * inv_s2;                               // d tau / d a, eq.(50)
-    float tau = L.a * c2;
-    // q = (1 - |v|)/2 = s^2/(2(1+|v|)): 1-kappa on the lobe side (v > 0), kappa itself on the far side;
-    // neither 1 - v nor 1 + v is ever formed by a cancelling subtraction
+    const float u = fmaf(dx, L.Xx, fmaf(dy, L.Xy, dz * L.Xz));
+    const float om = fmaf(dx, L.Yx, fmaf(dy, L.Yy, dz * L.Yz));
+    const float v = fmaf(dx, L.Zx, fmaf(dy, L.Zy, dz * L.Zz));
+    const float uu = u * u;
+    const float s2 = fmaxf(fmaf(om, om, uu), TINY);          // 1 - v^2 without cancellation
+    const float w2 = fmaf(fabsf(v), 2.0f, 2.0f);             // 2 (1 + |v|)
+    const float rw = f_rcp(s2 * w2);                         // one reciprocal serves 1/s^2 and 1/(1+|v|)
+    const float inv_s2 = rw * w2;
+    const float q = s2 * (s2 * rw);                          // (1 - |v|)/2 = s^2 / (2 (1 + |v|))
+    const float tau = L.a * uu * inv_s2;                     // a (d.x)^2 / (1 - (d.z)^2)
     const bool upper = v > 0.0f;
-    float q = fmaxf(0.5f * s2 * f_rcp(1.0f + fabsf(v)), 1e-30f);
-    float Lk = log_kappa(q, upper);                          // ln kappa
-    float x1 = fmaf(tau, Lk, Lk);                            // (1+tau) ln kappa
-    float em1 = expm1_neg(x1);                               // kappa^(1+tau) - 1
-    float arg = fmaf(L.lam2, em1, tau * Lk);                 // ln(p E)
-    float Gbar = f_exp(arg) * L.invI;
-    Gbar = (s2 <= 1e-30f && !upper) ? 0.0f : Gbar;           // d = -z: G = 0 (eq.(9), third case)
-    float theta = fmaf(L.k, u, L.phi);
-    float H;
+    const float L2 = log2_kappa(q, upper);                   // log2 kappa
+    const float x1 = fmaf(tau, L2, L2);                      // (1+tau) log2 kappa
+    float kp;
+    const float em1 = exp2m1_neg(x1, kp);                    // kappa^(1+tau) - 1, kappa^(1+tau)
+    const float arg = fmaf(L.lam2e, em1, fmaf(tau, L2, L.lgI));   // log2( p E / (2 I) )
+    float Gh = f_ex2(arg);
+    Gh = (s2 <= TINY && !upper) ? 0.0f : Gh;                 // d = -z: G = 0 (eq.(9), third case)
+    const float ang = reduce_turns(fmaf(L.kt, u, L.pt));     // k d.x + phi  (mod 2 pi)
+    const float G = fmaf(Gh, f_cos(ang), Gh);                // (1 + cos)/2 * p E / I
     if (FULL) {
-        float sn, cs;
-        f_sincos(theta, sn, cs);
-        H = fmaf(0.5f, cs, 0.5f);
-        T.u = u; T.v = v; T.c2 = c2; T.inv_s2 = inv_s2; T.tau = tau; T.Lk = Lk; T.kp = em1 + 1.0f; T.em1 = em1;
-        T.inv_2kappa = f_rcp(2.0f * (upper ? 1.0f - q : q));
-        T.Gbar = Gbar; T.H = H; T.sn = sn;
-    } else {
-        H = fmaf(0.5f, f_cos(theta), 0.5f);
+        T.u = u; T.v = v; T.uu = uu; T.inv_s2 = inv_s2; T.tau = tau; T.Lk = LN2 * L2; T.kp = kp; T.em1 = em1;
+        T.inv_2kappa = upper ? 2.0f * s2 * rw : 0.5f * w2 * inv_s2;      // 1/(1+v)
+        T.Gh = Gh; T.sn = f_sin(ang);
     }
-    return Gbar * H;
+    return G;
 }
 
 } // namespace nasg
