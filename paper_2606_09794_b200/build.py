@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = [os.path.join(CSRC, f) for f in ("nasg_api.cu", "nasg_kernels.cu", "sh_kernels.cu")]
+SOURCES = [os.path.join(CSRC, f) for f in ("nasg_api.cu", "nasg_kernels.cu", "nasg_pipe_kernels.cu", "sh_kernels.cu")]
 HEADERS = [os.path.join(CSRC, f) for f in ("nasg_internal.h", "nasg_math.cuh")] + [
     os.path.join(ROOT, "include", "nasg.h")]
 LIB = os.path.join(HERE, "libnasg_b200.so")

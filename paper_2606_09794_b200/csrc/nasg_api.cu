@@ -5,6 +5,7 @@
 #include "nasg_internal.h"
 
 #include <atomic>
+#include <cstdlib>
 
 namespace {
 
@@ -14,6 +15,14 @@ thread_local cudaError_t t_last_cuda = cudaSuccess;
 inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 inline bool supported_K(int K) { return K == 1 || K == 2 || K == 3 || K == 4 || K == 5 || K == 8; }
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+// C <= 4 runs the persistent cp.async-pipelined kernels; NASG_FORCE_GENERIC=1 (debug/AB testing) or a
+// larger camera batch runs the generic ones.
+bool use_pipe(int C)
+{
+    static const bool force_generic = [] { const char *e = getenv("NASG_FORCE_GENERIC"); return e && e[0] == '1'; }();
+    return C <= 4 && !force_generic;
+}
 
 int cuda_fail(cudaError_t e) { t_last_cuda = e; return NASG_ERR_CUDA; }
 
@@ -56,7 +65,9 @@ int nasg_eval_fwd(const nasg_inputs *in, float *colors, int norm_mode, void *cud
     if (!colors) return NASG_ERR_NULL;
     if (!aligned16(in->quat) || !aligned16(in->shape)) return NASG_ERR_ALIGN;
     nasg::FwdParams p{in->N, in->C, in->means, in->quat, in->shape, in->amp, in->dc, in->campos, in->vis, colors};
-    cudaError_t e = nasg::launch_nasg_fwd(p, in->K, norm_mode == NASG_NORM_EXACT, (cudaStream_t)cuda_stream);
+    const bool exact = norm_mode == NASG_NORM_EXACT;
+    cudaError_t e = use_pipe(in->C) ? nasg::launch_nasg_fwd_pipe(p, in->K, exact, (cudaStream_t)cuda_stream)
+                                    : nasg::launch_nasg_fwd(p, in->K, exact, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return cuda_fail(e);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     return NASG_OK;
@@ -87,7 +98,9 @@ int nasg_eval_bwd(const nasg_inputs *in, const float *g_colors, const nasg_grads
     }
     nasg::BwdParams p{in->N, in->C, in->means, in->quat, in->shape, in->amp, in->campos, in->vis, g_colors,
                       out->g_means, out->g_quat, out->g_shape, out->g_amp, out->g_dc, partial};
-    cudaError_t e = nasg::launch_nasg_bwd(p, in->K, norm_mode == NASG_NORM_EXACT, st);
+    const bool exact = norm_mode == NASG_NORM_EXACT;
+    cudaError_t e = (use_pipe(in->C) && !partial) ? nasg::launch_nasg_bwd_pipe(p, in->K, exact, st)
+                                                  : nasg::launch_nasg_bwd(p, in->K, exact, st);
     if (e != cudaSuccess) return cuda_fail(e);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     if (partial) {
