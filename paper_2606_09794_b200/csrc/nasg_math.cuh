@@ -47,7 +47,13 @@ NASG_MUFU(f_cos, "cos.approx.ftz.f32", cosf(x))
 #undef NASG_MUFU
 NASG_HD float f_exp(float x) { return f_ex2(x * LOG2E); }
 // angle given in TURNS (theta/2pi): exact reduction to [-1/2,1/2] turns, then radians in [-pi,pi]
-NASG_HD float reduce_turns(float t) { return TWO_PI * (t - rintf(t)); }
+// (round-to-nearest via the 1.5*2^23 magic constant: two FADDs on the FMA pipe instead of an FRND on the
+// XU pipe; exact for |t| < 2^22)
+NASG_HD float reduce_turns(float t)
+{
+    const float n = (t + 12582912.0f) - 12582912.0f;
+    return TWO_PI * (t - n);
+}
 
 // ---------------------------------------------------------------------------------------------
 // accurate small-argument helpers (base 2)
@@ -138,9 +144,10 @@ NASG_HD void normaliser(float l1, float l2, float Lam, float lam, float k, float
         // k < Lambda:  Psi = (Lambda/r) e^{r-Lambda} (1-e^{-2r})/(1-e^{-2 Lambda}),  r-Lambda = -k^2/(Lambda+r)
         const float ir = f_rsqrt(s), r = s * ir;
         const float del = k * k * f_rcp(Lam + r);                         // Lambda - r
-        const float e2r = f_exp(-2.0f * r), e2L = f_exp(-2.0f * Lam);
+        const float ed = f_exp(-del);                                      // e^{r - Lambda}
+        const float e2r = f_exp(-2.0f * r), e2L = e2r * ed * ed;          // e^{-2 Lambda} = e^{-2r} e^{-2(Lambda-r)}
         const float i1L = f_rcp(1.0f - e2L);
-        Psi = Lam * ir * f_exp(-del) * (1.0f - e2r) * i1L;
+        Psi = Lam * ir * ed * (1.0f - e2r) * i1L;
         if (GRAD) {
             const float gr = g_fun(r);
             float dg;
@@ -199,8 +206,9 @@ NASG_HD void lobe_setup(const float4 q, const float4 sp, Lobe &L, LobeBwd &B)
     L.Yx = fmaf(x2, y, -z2 * w); L.Yy = 1.0f - fmaf(x2, x, z2 * z); L.Yz = fmaf(y2, z, x2 * w);
     L.Zx = fmaf(x2, z, y2 * w); L.Zy = fmaf(y2, z, -x2 * w); L.Zz = 1.0f - fmaf(x2, x, y2 * y);
     // relative errors of Lambda, lambda only scale the exponent (benign), so ex2.approx is enough
-    const float Lam = f_exp(sp.x), lam = f_exp(sp.y);
+    const float lam = f_exp(sp.y);
     const float one_pa = f_exp(sp.x - sp.y);
+    const float Lam = lam * one_pa;
     L.a = fmaxf(one_pa - 1.0f, 0.0f);
     L.lam2e = 2.0f * LOG2E * lam;
     L.kt = sp.z * INV_TWO_PI; L.pt = sp.w * INV_TWO_PI;

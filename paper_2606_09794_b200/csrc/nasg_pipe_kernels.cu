@@ -153,7 +153,7 @@ __global__ void __launch_bounds__(PBLOCK, 2) nasg_fwd_pipe_kernel(FwdParams p)
                 lobe_setup<EXACT, false>(q, sp, L, B);
 #pragma unroll
                 for (int t = 0; t < CT; ++t) {
-                    if (CT == 1 || (mask & (1u << t))) {
+                    {   // every camera slot is evaluated: culled slots carry g_colors = 0 / are zeroed at the store
                         EvalTerms T;
                         const float G = lobe_eval<false>(L, dx[t], dy[t], dz[t], T);
                         col[t][0] = fmaf(w0, G, col[t][0]);
@@ -259,7 +259,7 @@ __global__ void __launch_bounds__(PBLOCK, 2) nasg_bwd_pipe_kernel(BwdParams p)
                 float S0 = 0.f, S1 = 0.f, S2 = 0.f, Sk = 0.f, Sp = 0.f;
 #pragma unroll
                 for (int t = 0; t < CT; ++t) {
-                    if (CT == 1 || (mask & (1u << t))) {
+                    {   // every camera slot is evaluated: culled slots carry g_colors = 0 / are zeroed at the store
                         EvalTerms T;
                         const float G = lobe_eval<true>(L, dx[t], dy[t], dz[t], T);
                         const float gG = fmaf(gc[t][0], w0, fmaf(gc[t][1], w1, gc[t][2] * w2));   // dL/dG, eq.(6)
@@ -325,15 +325,23 @@ __global__ void __launch_bounds__(PBLOCK, 2) nasg_bwd_pipe_kernel(BwdParams p)
 // ---------------------------------------------------------------------------------------------
 // launchers: persistent grid, 2 blocks per SM
 // ---------------------------------------------------------------------------------------------
+// Resident-grid size of a persistent kernel; the occupancy query and the shared-memory opt-in are done
+// once per (kernel instantiation, device) and cached (benign, idempotent state).
 template <typename Kernel>
-static int pipe_grid(Kernel kernel, size_t smem, int64_t N)
+static int pipe_grid(Kernel kernel, size_t smem, int64_t N, int *cached /* [64], one per kernel instantiation */)
 {
-    int dev = 0, sms = 148, per_sm = 2;
+    int dev = 0;
     cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, PBLOCK, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
-    const int64_t need = (N + PBLOCK - 1) / PBLOCK, resident = (int64_t)per_sm * sms;
+    int resident = (dev >= 0 && dev < 64) ? cached[dev] : 0;
+    if (resident == 0) {
+        int sms = 148, per_sm = 1;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, PBLOCK, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
+        resident = per_sm * sms;
+        if (dev >= 0 && dev < 64) cached[dev] = resident;
+    }
+    const int64_t need = (N + PBLOCK - 1) / PBLOCK;
     return (int)(need < resident ? need : resident);
 }
 
@@ -342,8 +350,9 @@ static cudaError_t launch_fwd_pipe_kc(const FwdParams &p, bool exact, cudaStream
 {
     constexpr size_t smem = pipe_smem_bytes(PipeCfg<K>::HR, 6);
     const dim3 block(PBLOCK);
-    if (exact) nasg_fwd_pipe_kernel<K, CT, true><<<pipe_grid(nasg_fwd_pipe_kernel<K, CT, true>, smem, p.N), block, smem, st>>>(p);
-    else nasg_fwd_pipe_kernel<K, CT, false><<<pipe_grid(nasg_fwd_pipe_kernel<K, CT, false>, smem, p.N), block, smem, st>>>(p);
+    static int cache[2][64] = {{0}};        // per (K, CT, norm mode) instantiation and device
+    if (exact) nasg_fwd_pipe_kernel<K, CT, true><<<pipe_grid(nasg_fwd_pipe_kernel<K, CT, true>, smem, p.N, cache[1]), block, smem, st>>>(p);
+    else nasg_fwd_pipe_kernel<K, CT, false><<<pipe_grid(nasg_fwd_pipe_kernel<K, CT, false>, smem, p.N, cache[0]), block, smem, st>>>(p);
     return cudaGetLastError();
 }
 template <int K>
@@ -351,6 +360,7 @@ static cudaError_t launch_fwd_pipe_k(const FwdParams &p, bool exact, cudaStream_
 {
     if (p.C == 1) return launch_fwd_pipe_kc<K, 1>(p, exact, st);
     if (p.C == 2) return launch_fwd_pipe_kc<K, 2>(p, exact, st);
+    if (p.C == 3) return launch_fwd_pipe_kc<K, 3>(p, exact, st);
     return launch_fwd_pipe_kc<K, 4>(p, exact, st);
 }
 cudaError_t launch_nasg_fwd_pipe(const FwdParams &p, int K, bool exact, cudaStream_t st)
@@ -371,8 +381,9 @@ static cudaError_t launch_bwd_pipe_kc(const BwdParams &p, bool exact, cudaStream
 {
     constexpr size_t smem = pipe_smem_bytes(PipeCfg<K>::HR, 3 + 3 * CT);
     const dim3 block(PBLOCK);
-    if (exact) nasg_bwd_pipe_kernel<K, CT, true><<<pipe_grid(nasg_bwd_pipe_kernel<K, CT, true>, smem, p.N), block, smem, st>>>(p);
-    else nasg_bwd_pipe_kernel<K, CT, false><<<pipe_grid(nasg_bwd_pipe_kernel<K, CT, false>, smem, p.N), block, smem, st>>>(p);
+    static int cache[2][64] = {{0}};        // per (K, CT, norm mode) instantiation and device
+    if (exact) nasg_bwd_pipe_kernel<K, CT, true><<<pipe_grid(nasg_bwd_pipe_kernel<K, CT, true>, smem, p.N, cache[1]), block, smem, st>>>(p);
+    else nasg_bwd_pipe_kernel<K, CT, false><<<pipe_grid(nasg_bwd_pipe_kernel<K, CT, false>, smem, p.N, cache[0]), block, smem, st>>>(p);
     return cudaGetLastError();
 }
 template <int K>
@@ -380,6 +391,7 @@ static cudaError_t launch_bwd_pipe_k(const BwdParams &p, bool exact, cudaStream_
 {
     if (p.C == 1) return launch_bwd_pipe_kc<K, 1>(p, exact, st);
     if (p.C == 2) return launch_bwd_pipe_kc<K, 2>(p, exact, st);
+    if (p.C == 3) return launch_bwd_pipe_kc<K, 3>(p, exact, st);
     return launch_bwd_pipe_kc<K, 4>(p, exact, st);
 }
 cudaError_t launch_nasg_bwd_pipe(const BwdParams &p, int K, bool exact, cudaStream_t st)
