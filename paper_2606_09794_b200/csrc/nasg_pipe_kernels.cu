@@ -41,6 +41,7 @@ __device__ __forceinline__ void st_cs4(float *p, float4 v) { __stcs(reinterpret_
 
 template <int K> struct PipeCfg {
     static constexpr int HR = (K <= 2) ? 4 : 2;          // header slots: ceil(DIST/K)+1 rounded to a power of 2
+    static constexpr bool STATIC_SLOTS = (K % RING) == 0; // lobe l always lives in ring slot l % RING
 };
 
 // shared-memory carve-up for one block
@@ -94,7 +95,7 @@ __device__ __forceinline__ unsigned load_mask(const uint8_t *vis, int64_t N, int
 // forward
 // ---------------------------------------------------------------------------------------------
 template <int K, int CT, bool EXACT>
-__global__ void __launch_bounds__(PBLOCK, 2) nasg_fwd_pipe_kernel(FwdParams p)
+__global__ void __launch_bounds__(PBLOCK, CT >= 3 ? 3 : 4) nasg_fwd_pipe_kernel(FwdParams p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int HR = PipeCfg<K>::HR, HF = 6;
@@ -124,7 +125,7 @@ __global__ void __launch_bounds__(PBLOCK, 2) nasg_fwd_pipe_kernel(FwdParams p)
         float dx[CT], dy[CT], dz[CT], col[CT][3];
 #pragma unroll
         for (int l = 0; l < K; ++l) {
-            prefetch_item(n + ((l + DIST) / K) * stride, (l + DIST) % K, (sbase + l + DIST) % RING,
+            prefetch_item(n + ((l + DIST) / K) * stride, (l + DIST) % K, ((PipeCfg<K>::STATIC_SLOTS ? 0u : sbase) + (l + DIST) % RING) % RING,
                           (hs + (l + DIST) / K) % HR);
             cp_async_wait<DIST>();
             if (l == 0) {
@@ -144,7 +145,7 @@ __global__ void __launch_bounds__(PBLOCK, 2) nasg_fwd_pipe_kernel(FwdParams p)
                 }
             }
             if (mask != 0) {
-                const int slot = (sbase + l) % RING;
+                const int slot = ((PipeCfg<K>::STATIC_SLOTS ? 0u : sbase) + l) % RING;
                 const float4 q = r.q[slot * PBLOCK + tid];
                 const float4 sp = r.s[slot * PBLOCK + tid];
                 const float w0 = r.w[(slot * 3 + 0) * PBLOCK + tid], w1 = r.w[(slot * 3 + 1) * PBLOCK + tid],
@@ -219,7 +220,7 @@ __global__ void __launch_bounds__(PBLOCK, 2) nasg_bwd_pipe_kernel(BwdParams p)
         float dx[CT], dy[CT], dz[CT], idist[CT], gc[CT][3], gd[CT][3];
 #pragma unroll
         for (int l = 0; l < K; ++l) {
-            prefetch_item(n + ((l + DIST) / K) * stride, (l + DIST) % K, (sbase + l + DIST) % RING,
+            prefetch_item(n + ((l + DIST) / K) * stride, (l + DIST) % K, ((PipeCfg<K>::STATIC_SLOTS ? 0u : sbase) + (l + DIST) % RING) % RING,
                           (hs + (l + DIST) / K) % HR);
             cp_async_wait<DIST>();
             if (l == 0) {
@@ -248,7 +249,7 @@ __global__ void __launch_bounds__(PBLOCK, 2) nasg_bwd_pipe_kernel(BwdParams p)
             float4 gq = make_float4(0.f, 0.f, 0.f, 0.f), gs = make_float4(0.f, 0.f, 0.f, 0.f);
             float gw0 = 0.f, gw1 = 0.f, gw2 = 0.f;
             if (mask != 0) {
-                const int slot = (sbase + l) % RING;
+                const int slot = ((PipeCfg<K>::STATIC_SLOTS ? 0u : sbase) + l) % RING;
                 const float4 q = r.q[slot * PBLOCK + tid];
                 const float4 sp = r.s[slot * PBLOCK + tid];
                 const float w0 = r.w[(slot * 3 + 0) * PBLOCK + tid], w1 = r.w[(slot * 3 + 1) * PBLOCK + tid],
