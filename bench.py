@@ -216,13 +216,13 @@ def run_ours(args, W, cfg):
             ev[s][0].record(stream); fwd(); ev[s][1].record(stream); bwd(); ev[s][2].record(stream)
         barrier()
         timed_wall = time.perf_counter() - t_wall
+        launches = B.nasg_launch_count() - launches0          # kernels launched inside the timed region
         # the timed region is short (ms): keep the identical load running, untimed, until nvidia-smi
         # (50 ms period) has had ~1 s to sample clocks and throttle reasons under this load
         while time.perf_counter() - t_wall < 1.0:
             for _ in range(20):
                 fwd(); bwd()
             torch.cuda.synchronize()
-    launches = B.nasg_launch_count() - launches0
     total_ms = ev[0][0].elapsed_time(ev[-1][2])
     fwd_ms = sum(e[0].elapsed_time(e[1]) for e in ev) / args.steps
     bwd_ms = sum(e[1].elapsed_time(e[2]) for e in ev) / args.steps
@@ -264,7 +264,9 @@ def run_ours(args, W, cfg):
         fb, bb = algorithmic_bytes(cfg.kind, K, C, d["vis"] is not None)
         peak, peak_src = measured_peak()
         achieved = bb * N / (bwd_ms * 1e-3) / 1e9
-        kname = "sh_bwd_kernel" if cfg.kind == "sh" else "nasg_bwd_kernel"
+        pipe = C <= 4
+        kname = ("sh_bwd_pipe_kernel" if pipe else "sh_bwd_kernel") if cfg.kind == "sh" else \
+                ("nasg_bwd_pipe_kernel" if pipe else "nasg_bwd_kernel")
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,

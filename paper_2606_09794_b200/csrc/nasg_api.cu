@@ -118,7 +118,7 @@ int sh_eval_fwd(int64_t N, int32_t C, const float *means, const float *coeffs, c
     if (N == 0) return NASG_OK;
     if (!means || !coeffs || !campos || !colors) return NASG_ERR_NULL;
     nasg::ShParams p{N, C, means, coeffs, campos, vis, nullptr, colors, nullptr, nullptr, nullptr};
-    cudaError_t e = nasg::launch_sh_fwd(p, (cudaStream_t)cuda_stream);
+    cudaError_t e = use_pipe(C) ? nasg::launch_sh_fwd_pipe(p, (cudaStream_t)cuda_stream) : nasg::launch_sh_fwd(p, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return cuda_fail(e);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     return NASG_OK;
@@ -144,7 +144,7 @@ int sh_eval_bwd(int64_t N, int32_t C, const float *means, const float *coeffs, c
         partial = static_cast<float *>(workspace);
     }
     nasg::ShParams p{N, C, means, coeffs, campos, vis, g_colors, nullptr, g_means, g_coeffs, partial};
-    cudaError_t e = nasg::launch_sh_bwd(p, st);
+    cudaError_t e = (use_pipe(C) && !partial) ? nasg::launch_sh_bwd_pipe(p, st) : nasg::launch_sh_bwd(p, st);
     if (e != cudaSuccess) return cuda_fail(e);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     if (partial) {

@@ -15,29 +15,12 @@
 // per-Gaussian header (mean, dc or g_colors) travels with lobe 0 into header slot i % HR.
 #include "nasg_internal.h"
 #include "nasg_math.cuh"
+#include "pipe_common.cuh"
 
 namespace nasg {
 
-constexpr int PBLOCK = 256;
 constexpr int RING = 4;     // lobe slots per thread
 constexpr int DIST = 3;     // prefetch distance in lobes
-
-__device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
-{
-    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
-}
-__device__ __forceinline__ void cp_async4(void *smem, const void *gmem)
-{
-    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(s), "l"(gmem) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N_PENDING>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N_PENDING) : "memory"); }
-
-__device__ __forceinline__ void st_cs(float *p, float v) { __stcs(p, v); }
-__device__ __forceinline__ void st_cs4(float *p, float4 v) { __stcs(reinterpret_cast<float4 *>(p), v); }
 
 template <int K> struct PipeCfg {
     static constexpr int HR = (K <= 2) ? 4 : 2;          // header slots: ceil(DIST/K)+1 rounded to a power of 2
@@ -78,17 +61,6 @@ __device__ __forceinline__ void prefetch_lobe(const Ring &r, int slot, int tid, 
         cp_async4(&r.w[(slot * 3 + 1) * PBLOCK + tid], a + N);
         cp_async4(&r.w[(slot * 3 + 2) * PBLOCK + tid], a + 2 * N);
     }
-}
-
-__device__ __forceinline__ unsigned load_mask(const uint8_t *vis, int64_t N, int64_t n, int C)
-{
-    unsigned m = 0;
-    if (n < N) {
-        if (!vis) return (1u << C) - 1u;
-#pragma unroll 4
-        for (int c = 0; c < C; ++c) m |= (vis[(int64_t)c * N + n] != 0 ? 1u : 0u) << c;
-    }
-    return m;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -326,26 +298,6 @@ __global__ void __launch_bounds__(PBLOCK, 2) nasg_bwd_pipe_kernel(BwdParams p)
 // ---------------------------------------------------------------------------------------------
 // launchers: persistent grid, 2 blocks per SM
 // ---------------------------------------------------------------------------------------------
-// Resident-grid size of a persistent kernel; the occupancy query and the shared-memory opt-in are done
-// once per (kernel instantiation, device) and cached (benign, idempotent state).
-template <typename Kernel>
-static int pipe_grid(Kernel kernel, size_t smem, int64_t N, int *cached /* [64], one per kernel instantiation */)
-{
-    int dev = 0;
-    cudaGetDevice(&dev);
-    int resident = (dev >= 0 && dev < 64) ? cached[dev] : 0;
-    if (resident == 0) {
-        int sms = 148, per_sm = 1;
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, PBLOCK, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
-        resident = per_sm * sms;
-        if (dev >= 0 && dev < 64) cached[dev] = resident;
-    }
-    const int64_t need = (N + PBLOCK - 1) / PBLOCK;
-    return (int)(need < resident ? need : resident);
-}
-
 template <int K, int CT>
 static cudaError_t launch_fwd_pipe_kc(const FwdParams &p, bool exact, cudaStream_t st)
 {

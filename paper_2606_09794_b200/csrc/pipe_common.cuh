@@ -1,0 +1,60 @@
+// pipe_common.cuh — pieces shared by the persistent cp.async-pipelined kernels (NASGabor and SH):
+// LDGSTS wrappers, streaming stores, the visibility-mask load and the resident-grid launch helper.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace nasg {
+
+constexpr int PBLOCK = 256;
+
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async4(void *smem, const void *gmem)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N_PENDING>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N_PENDING) : "memory"); }
+
+__device__ __forceinline__ void st_cs(float *p, float v) { __stcs(p, v); }
+__device__ __forceinline__ void st_cs4(float *p, float4 v) { __stcs(reinterpret_cast<float4 *>(p), v); }
+
+__device__ __forceinline__ unsigned load_mask(const uint8_t *vis, int64_t N, int64_t n, int C)
+{
+    unsigned m = 0;
+    if (n < N) {
+        if (!vis) return (1u << C) - 1u;
+#pragma unroll 4
+        for (int c = 0; c < C; ++c) m |= (vis[(int64_t)c * N + n] != 0 ? 1u : 0u) << c;
+    }
+    return m;
+}
+
+// Resident-grid size of a persistent kernel; the occupancy query and the shared-memory opt-in are done
+// once per (kernel instantiation, device) and cached (benign, idempotent state).
+template <typename Kernel>
+static int pipe_grid(Kernel kernel, size_t smem, int64_t N, int *cached /* [64], one per kernel instantiation */)
+{
+    int dev = 0;
+    cudaGetDevice(&dev);
+    int resident = (dev >= 0 && dev < 64) ? cached[dev] : 0;
+    if (resident == 0) {
+        int sms = 148, per_sm = 1;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, PBLOCK, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
+        resident = per_sm * sms;
+        if (dev >= 0 && dev < 64) cached[dev] = resident;
+    }
+    const int64_t need = (N + PBLOCK - 1) / PBLOCK;
+    return (int)(need < resident ? need : resident);
+}
+
+} // namespace nasg

@@ -1,0 +1,280 @@
+// sh_pipe_kernels.cu — fast path of the SH degree-3 comparison kernels for C <= 4 cameras (sm_100a),
+// built the same way as the NASGabor fast path (nasg_pipe_kernels.cu): persistent threads, one thread per
+// Gaussian, parameters streamed through a private shared-memory ring filled by cp.async (LDGSTS)
+// SH_DIST items ahead of use, gradients written once with streaming stores, no atomics.
+//
+// Item stream of a thread: (Gaussian i, group g), g = 0..3; group g holds the 4 basis functions
+// j = 4g..4g+3, i.e. 12 planar coefficient rows = 48 B per Gaussian (a NASGabor lobe is 44 B), and always
+// lives in ring slot g. The per-Gaussian header (mean, and g_colors in the backward) travels with
+// group 0 into header slot i % 2. A thread only reads slots it filled itself: no block barrier.
+#include "nasg_internal.h"
+#include "pipe_common.cuh"
+#include "sh_math.cuh"
+
+namespace nasg {
+
+constexpr int SH_GROUPS = 4;    // groups of 4 basis functions
+constexpr int SH_DIST = 3;      // prefetch distance in groups
+constexpr int SH_HR = 2;        // header slots
+
+__host__ __device__ constexpr size_t sh_pipe_smem_bytes(int HF)
+{
+    return (size_t)PBLOCK * 4 * (SH_GROUPS * 12 + SH_HR * HF);
+}
+
+// copies of one group item: rows (4g+jj)*3+ch, jj < 4, ch < 3
+__device__ __forceinline__ void sh_prefetch_group(float *ring, int tid, const float *coeffs, int64_t N, int64_t n, int g)
+{
+    const float *src = coeffs + (int64_t)g * 12 * N + n;
+    float *dst = ring + g * 12 * PBLOCK + tid;
+#pragma unroll
+    for (int r = 0; r < 12; ++r) cp_async4(dst + r * PBLOCK, src + (int64_t)r * N);
+}
+
+template <int CT>
+__device__ __forceinline__ void sh_directions(const float *campos, int C, float mx, float my, float mz,
+                                              float (&dx)[CT], float (&dy)[CT], float (&dz)[CT], float (&idist)[CT])
+{
+#pragma unroll
+    for (int t = 0; t < CT; ++t) {
+        const int c = t < C ? t : 0;
+        const float ex = mx - __ldg(campos + 3 * c), ey = my - __ldg(campos + 3 * c + 1), ez = mz - __ldg(campos + 3 * c + 2);
+        const float r2 = fmaf(ex, ex, fmaf(ey, ey, ez * ez));
+        float inv = rsqrtf(r2);
+        inv = inv * fmaf(-0.5f * r2, inv * inv, 1.5f);
+        dx[t] = ex * inv; dy[t] = ey * inv; dz[t] = ez * inv; idist[t] = inv;
+    }
+}
+
+// ---- forward: colors[c,n,:] = sum_j coeffs[j,:,n] Y_j(d_cn) -------------------------------------
+template <int G, int CT>
+__device__ __forceinline__ void sh_fwd_group(const float *slot, const float (&dx)[CT], const float (&dy)[CT],
+                                             const float (&dz)[CT], float (&col)[CT][3])
+{
+#pragma unroll
+    for (int jj = 0; jj < 4; ++jj) {
+        const float k0 = slot[(jj * 3 + 0) * PBLOCK], k1 = slot[(jj * 3 + 1) * PBLOCK], k2 = slot[(jj * 3 + 2) * PBLOCK];
+#pragma unroll
+        for (int t = 0; t < CT; ++t) {
+            float Y = 0.f, gx, gy, gz;
+            if (jj == 0) sh_term<4 * G + 0>(dx[t], dy[t], dz[t], Y, gx, gy, gz);
+            if (jj == 1) sh_term<4 * G + 1>(dx[t], dy[t], dz[t], Y, gx, gy, gz);
+            if (jj == 2) sh_term<4 * G + 2>(dx[t], dy[t], dz[t], Y, gx, gy, gz);
+            if (jj == 3) sh_term<4 * G + 3>(dx[t], dy[t], dz[t], Y, gx, gy, gz);
+            col[t][0] = fmaf(k0, Y, col[t][0]); col[t][1] = fmaf(k1, Y, col[t][1]); col[t][2] = fmaf(k2, Y, col[t][2]);
+        }
+    }
+}
+
+template <int CT>
+__global__ void __launch_bounds__(PBLOCK, 4) sh_fwd_pipe_kernel(ShParams p)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int HF = 3;
+    float *ring = reinterpret_cast<float *>(smem_raw);
+    float *hdr = ring + SH_GROUPS * 12 * PBLOCK;
+    const int tid = threadIdx.x;
+    const int64_t N = p.N, stride = (int64_t)gridDim.x * PBLOCK;
+    int64_t n = (int64_t)blockIdx.x * PBLOCK + tid;
+
+    auto prefetch_item = [&](int64_t gn, int g, int hslot) {
+        if (gn < N) {
+            sh_prefetch_group(ring, tid, p.coeffs, N, gn, g);
+            if (g == 0) {
+                float *h = hdr + hslot * HF * PBLOCK + tid;
+                cp_async4(h, p.means + 3 * gn); cp_async4(h + PBLOCK, p.means + 3 * gn + 1);
+                cp_async4(h + 2 * PBLOCK, p.means + 3 * gn + 2);
+            }
+        }
+        cp_async_commit();
+    };
+#pragma unroll
+    for (int j = 0; j < SH_DIST; ++j) prefetch_item(n, j, 0);
+
+    unsigned hs = 0;
+    unsigned mask = load_mask(p.vis, N, n, p.C);
+    for (; n < N; n += stride) {
+        const unsigned mask_next = load_mask(p.vis, N, n + stride, p.C);
+        float dx[CT], dy[CT], dz[CT], idist[CT], col[CT][3];
+#pragma unroll
+        for (int g = 0; g < SH_GROUPS; ++g) {
+            prefetch_item(n + ((g + SH_DIST) / SH_GROUPS) * stride, (g + SH_DIST) % SH_GROUPS, (hs + (g + SH_DIST) / SH_GROUPS) % SH_HR);
+            cp_async_wait<SH_DIST>();
+            if (g == 0) {
+                const float *h = hdr + hs * HF * PBLOCK + tid;
+                sh_directions<CT>(p.campos, p.C, h[0], h[PBLOCK], h[2 * PBLOCK], dx, dy, dz, idist);
+#pragma unroll
+                for (int t = 0; t < CT; ++t) col[t][0] = col[t][1] = col[t][2] = 0.f;
+            }
+            if (mask != 0) {
+                const float *slot = ring + g * 12 * PBLOCK + tid;
+                if (g == 0) sh_fwd_group<0, CT>(slot, dx, dy, dz, col);
+                if (g == 1) sh_fwd_group<1, CT>(slot, dx, dy, dz, col);
+                if (g == 2) sh_fwd_group<2, CT>(slot, dx, dy, dz, col);
+                if (g == 3) sh_fwd_group<3, CT>(slot, dx, dy, dz, col);
+            }
+        }
+#pragma unroll
+        for (int t = 0; t < CT; ++t) {
+            if (t < p.C) {
+                const bool on = mask & (1u << t);
+                float *o = p.colors + ((int64_t)t * N + n) * 3;
+                st_cs(o, on ? col[t][0] : 0.f); st_cs(o + 1, on ? col[t][1] : 0.f); st_cs(o + 2, on ? col[t][2] : 0.f);
+            }
+        }
+        hs = (hs + 1) % SH_HR;
+        mask = mask_next;
+    }
+    cp_async_wait<0>();
+}
+
+// ---- backward: g_coeffs[j,:,n] = sum_c Y_j(d_c) g_col_c;  g_d = sum_j grad Y_j (coeff_j . g_col) ----
+template <int G, int CT>
+__device__ __forceinline__ void sh_bwd_group(const float *slot, bool live, float *g_coeffs, int64_t N, int64_t n,
+                                             const float (&dx)[CT], const float (&dy)[CT], const float (&dz)[CT],
+                                             const float (&gc)[CT][3], float (&gd)[CT][3])
+{
+#pragma unroll
+    for (int jj = 0; jj < 4; ++jj) {
+        float a0 = 0.f, a1 = 0.f, a2 = 0.f;
+        if (live) {
+            const float k0 = slot[(jj * 3 + 0) * PBLOCK], k1 = slot[(jj * 3 + 1) * PBLOCK], k2 = slot[(jj * 3 + 2) * PBLOCK];
+#pragma unroll
+            for (int t = 0; t < CT; ++t) {
+                float Y = 0.f, gx = 0.f, gy = 0.f, gz = 0.f;
+                if (jj == 0) sh_term<4 * G + 0>(dx[t], dy[t], dz[t], Y, gx, gy, gz);
+                if (jj == 1) sh_term<4 * G + 1>(dx[t], dy[t], dz[t], Y, gx, gy, gz);
+                if (jj == 2) sh_term<4 * G + 2>(dx[t], dy[t], dz[t], Y, gx, gy, gz);
+                if (jj == 3) sh_term<4 * G + 3>(dx[t], dy[t], dz[t], Y, gx, gy, gz);
+                a0 = fmaf(gc[t][0], Y, a0); a1 = fmaf(gc[t][1], Y, a1); a2 = fmaf(gc[t][2], Y, a2);     // gc = 0 when culled
+                const float s = fmaf(k0, gc[t][0], fmaf(k1, gc[t][1], k2 * gc[t][2]));
+                gd[t][0] = fmaf(s, gx, gd[t][0]); gd[t][1] = fmaf(s, gy, gd[t][1]); gd[t][2] = fmaf(s, gz, gd[t][2]);
+            }
+        }
+        if (g_coeffs) {
+            float *o = g_coeffs + (int64_t)((4 * G + jj) * 3) * N + n;
+            st_cs(o, a0); st_cs(o + N, a1); st_cs(o + 2 * N, a2);
+        }
+    }
+}
+
+template <int CT>
+__global__ void __launch_bounds__(PBLOCK, 2) sh_bwd_pipe_kernel(ShParams p)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int HF = 3 + 3 * CT;
+    float *ring = reinterpret_cast<float *>(smem_raw);
+    float *hdr = ring + SH_GROUPS * 12 * PBLOCK;
+    const int tid = threadIdx.x;
+    const int C = p.C;
+    const int64_t N = p.N, stride = (int64_t)gridDim.x * PBLOCK;
+    int64_t n = (int64_t)blockIdx.x * PBLOCK + tid;
+
+    auto prefetch_item = [&](int64_t gn, int g, int hslot) {
+        if (gn < N) {
+            sh_prefetch_group(ring, tid, p.coeffs, N, gn, g);
+            if (g == 0) {
+                float *h = hdr + hslot * HF * PBLOCK + tid;
+                cp_async4(h, p.means + 3 * gn); cp_async4(h + PBLOCK, p.means + 3 * gn + 1);
+                cp_async4(h + 2 * PBLOCK, p.means + 3 * gn + 2);
+#pragma unroll
+                for (int t = 0; t < CT; ++t) {
+                    if (t < C) {
+                        const float *g3 = p.g_colors + ((int64_t)t * N + gn) * 3;
+                        cp_async4(h + (3 + 3 * t) * PBLOCK, g3); cp_async4(h + (4 + 3 * t) * PBLOCK, g3 + 1);
+                        cp_async4(h + (5 + 3 * t) * PBLOCK, g3 + 2);
+                    }
+                }
+            }
+        }
+        cp_async_commit();
+    };
+#pragma unroll
+    for (int j = 0; j < SH_DIST; ++j) prefetch_item(n, j, 0);
+
+    unsigned hs = 0;
+    unsigned mask = load_mask(p.vis, N, n, C);
+    for (; n < N; n += stride) {
+        const unsigned mask_next = load_mask(p.vis, N, n + stride, C);
+        float dx[CT], dy[CT], dz[CT], idist[CT], gc[CT][3], gd[CT][3];
+#pragma unroll
+        for (int g = 0; g < SH_GROUPS; ++g) {
+            prefetch_item(n + ((g + SH_DIST) / SH_GROUPS) * stride, (g + SH_DIST) % SH_GROUPS, (hs + (g + SH_DIST) / SH_GROUPS) % SH_HR);
+            cp_async_wait<SH_DIST>();
+            if (g == 0) {
+                const float *h = hdr + hs * HF * PBLOCK + tid;
+                sh_directions<CT>(p.campos, C, h[0], h[PBLOCK], h[2 * PBLOCK], dx, dy, dz, idist);
+#pragma unroll
+                for (int t = 0; t < CT; ++t) {
+                    const bool on = mask & (1u << t);
+                    gc[t][0] = on ? h[(3 + 3 * t) * PBLOCK] : 0.f;
+                    gc[t][1] = on ? h[(4 + 3 * t) * PBLOCK] : 0.f;
+                    gc[t][2] = on ? h[(5 + 3 * t) * PBLOCK] : 0.f;
+                    idist[t] = on ? idist[t] : 0.f;
+                    gd[t][0] = gd[t][1] = gd[t][2] = 0.f;
+                }
+            }
+            const float *slot = ring + g * 12 * PBLOCK + tid;
+            const bool live = mask != 0;
+            if (g == 0) sh_bwd_group<0, CT>(slot, live, p.g_coeffs, N, n, dx, dy, dz, gc, gd);
+            if (g == 1) sh_bwd_group<1, CT>(slot, live, p.g_coeffs, N, n, dx, dy, dz, gc, gd);
+            if (g == 2) sh_bwd_group<2, CT>(slot, live, p.g_coeffs, N, n, dx, dy, dz, gc, gd);
+            if (g == 3) sh_bwd_group<3, CT>(slot, live, p.g_coeffs, N, n, dx, dy, dz, gc, gd);
+        }
+        if (p.g_means) {        // through d = Delta/|Delta|: (I - d d^T)/|Delta|
+            float gm0 = 0.f, gm1 = 0.f, gm2 = 0.f;
+#pragma unroll
+            for (int t = 0; t < CT; ++t) {
+                const float dg = fmaf(dx[t], gd[t][0], fmaf(dy[t], gd[t][1], dz[t] * gd[t][2]));
+                gm0 = fmaf(gd[t][0] - dx[t] * dg, idist[t], gm0);
+                gm1 = fmaf(gd[t][1] - dy[t] * dg, idist[t], gm1);
+                gm2 = fmaf(gd[t][2] - dz[t] * dg, idist[t], gm2);
+            }
+            float *o = p.g_means + 3 * n;
+            st_cs(o, gm0); st_cs(o + 1, gm1); st_cs(o + 2, gm2);
+        }
+        hs = (hs + 1) % SH_HR;
+        mask = mask_next;
+    }
+    cp_async_wait<0>();
+}
+
+// ---- launchers --------------------------------------------------------------------------------
+template <int CT>
+static cudaError_t launch_sh_fwd_pipe_c(const ShParams &p, cudaStream_t st)
+{
+    constexpr size_t smem = sh_pipe_smem_bytes(3);
+    static int cache[64] = {0};
+    sh_fwd_pipe_kernel<CT><<<pipe_grid(sh_fwd_pipe_kernel<CT>, smem, p.N, cache), PBLOCK, smem, st>>>(p);
+    return cudaGetLastError();
+}
+cudaError_t launch_sh_fwd_pipe(const ShParams &p, cudaStream_t st)
+{
+    switch (p.C) {
+    case 1: return launch_sh_fwd_pipe_c<1>(p, st);
+    case 2: return launch_sh_fwd_pipe_c<2>(p, st);
+    case 3: return launch_sh_fwd_pipe_c<3>(p, st);
+    case 4: return launch_sh_fwd_pipe_c<4>(p, st);
+    default: return cudaErrorInvalidValue;
+    }
+}
+template <int CT>
+static cudaError_t launch_sh_bwd_pipe_c(const ShParams &p, cudaStream_t st)
+{
+    constexpr size_t smem = sh_pipe_smem_bytes(3 + 3 * CT);
+    static int cache[64] = {0};
+    sh_bwd_pipe_kernel<CT><<<pipe_grid(sh_bwd_pipe_kernel<CT>, smem, p.N, cache), PBLOCK, smem, st>>>(p);
+    return cudaGetLastError();
+}
+cudaError_t launch_sh_bwd_pipe(const ShParams &p, cudaStream_t st)
+{
+    switch (p.C) {
+    case 1: return launch_sh_bwd_pipe_c<1>(p, st);
+    case 2: return launch_sh_bwd_pipe_c<2>(p, st);
+    case 3: return launch_sh_bwd_pipe_c<3>(p, st);
+    case 4: return launch_sh_bwd_pipe_c<4>(p, st);
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+} // namespace nasg
