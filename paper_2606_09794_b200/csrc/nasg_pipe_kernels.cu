@@ -151,6 +151,97 @@ __global__ void __launch_bounds__(PBLOCK, CT >= 3 ? 3 : 4) nasg_fwd_pipe_kernel(
     cp_async_wait<0>();
 }
 
+// forward, two cameras per packed f32x2 instruction (CT >= 2)
+template <int K, int CT, bool EXACT>
+__global__ void __launch_bounds__(PBLOCK, CT >= 3 ? 3 : 4) nasg_fwd_pipe2_kernel(FwdParams p)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int HR = PipeCfg<K>::HR, HF = 6;
+    const Ring r = carve(smem_raw);
+    const int tid = threadIdx.x;
+    const int64_t N = p.N, stride = (int64_t)gridDim.x * PBLOCK;
+    int64_t n = (int64_t)blockIdx.x * PBLOCK + tid;
+
+    auto prefetch_item = [&](int64_t gn, int l, int slot, int hslot) {
+        prefetch_lobe(r, slot, tid, p.quat, p.shape, p.amp, N, gn, l);
+        if (l == 0 && gn < N) {
+            float *h = r.h + (hslot * HF) * PBLOCK + tid;
+            cp_async4(h, p.means + 3 * gn); cp_async4(h + PBLOCK, p.means + 3 * gn + 1);
+            cp_async4(h + 2 * PBLOCK, p.means + 3 * gn + 2);
+            cp_async4(h + 3 * PBLOCK, p.dc + gn); cp_async4(h + 4 * PBLOCK, p.dc + N + gn);
+            cp_async4(h + 5 * PBLOCK, p.dc + 2 * N + gn);
+        }
+        cp_async_commit();
+    };
+#pragma unroll
+    for (int j = 0; j < DIST; ++j) prefetch_item(n + (j / K) * stride, j % K, j % RING, (j / K) % HR);
+
+    unsigned sbase = 0, hs = 0;                  // ring slot of lobe 0 / header slot of the current Gaussian
+    unsigned mask = load_mask(p.vis, N, n, p.C);
+    for (; n < N; n += stride) {
+        const unsigned mask_next = load_mask(p.vis, N, n + stride, p.C);     // lands during this Gaussian
+        // camera slots live in pairs (x = slot 2j, y = slot 2j+1) so that the evaluation runs on packed
+        // f32x2 arithmetic; a slot beyond C repeats camera 0 and is never stored
+        constexpr int NP = (CT + 1) / 2;
+        float2 dx[NP], dy[NP], dz[NP], col[NP][3];
+#pragma unroll
+        for (int l = 0; l < K; ++l) {
+            prefetch_item(n + ((l + DIST) / K) * stride, (l + DIST) % K, ((PipeCfg<K>::STATIC_SLOTS ? 0u : sbase) + (l + DIST) % RING) % RING,
+                          (hs + (l + DIST) / K) % HR);
+            cp_async_wait<DIST>();
+            if (l == 0) {
+                const float *h = r.h + (hs * HF) * PBLOCK + tid;
+                const float2 mx = splat(h[0]), my = splat(h[PBLOCK]), mz = splat(h[2 * PBLOCK]);
+                const float2 dc0 = splat(h[3 * PBLOCK]), dc1 = splat(h[4 * PBLOCK]), dc2 = splat(h[5 * PBLOCK]);
+#pragma unroll
+                for (int j = 0; j < NP; ++j) {
+                    const int c0 = 2 * j < p.C ? 2 * j : 0, c1 = 2 * j + 1 < p.C ? 2 * j + 1 : 0;
+                    const float2 ex = sub2(mx, make_float2(__ldg(p.campos + 3 * c0), __ldg(p.campos + 3 * c1)));
+                    const float2 ey = sub2(my, make_float2(__ldg(p.campos + 3 * c0 + 1), __ldg(p.campos + 3 * c1 + 1)));
+                    const float2 ez = sub2(mz, make_float2(__ldg(p.campos + 3 * c0 + 2), __ldg(p.campos + 3 * c1 + 2)));
+                    const float2 r2 = fma2(ex, ex, fma2(ey, ey, mul2(ez, ez)));
+                    float2 inv = make_float2(f_rsqrt(r2.x), f_rsqrt(r2.y));
+                    inv = mul2(inv, fma2(mul2(splat(-0.5f), r2), mul2(inv, inv), splat(1.5f)));     // one Newton step
+                    dx[j] = mul2(ex, inv); dy[j] = mul2(ey, inv); dz[j] = mul2(ez, inv);
+                    col[j][0] = dc0; col[j][1] = dc1; col[j][2] = dc2;
+                }
+            }
+            if (mask != 0) {
+                const int slot = ((PipeCfg<K>::STATIC_SLOTS ? 0u : sbase) + l) % RING;
+                const float4 q = r.q[slot * PBLOCK + tid];
+                const float4 sp = r.s[slot * PBLOCK + tid];
+                const float2 w0 = splat(r.w[(slot * 3 + 0) * PBLOCK + tid]), w1 = splat(r.w[(slot * 3 + 1) * PBLOCK + tid]),
+                             w2 = splat(r.w[(slot * 3 + 2) * PBLOCK + tid]);
+                Lobe L; LobeBwd B;
+                lobe_setup<EXACT, false>(q, sp, L, B);
+#pragma unroll
+                for (int j = 0; j < NP; ++j) {
+                    // every camera slot is evaluated: culled slots are zeroed at the store
+                    EvalTerms2 T;
+                    const float2 G = lobe_eval2<false>(L, dx[j], dy[j], dz[j], splat(0.f), T);
+                    col[j][0] = fma2(w0, G, col[j][0]);
+                    col[j][1] = fma2(w1, G, col[j][1]);
+                    col[j][2] = fma2(w2, G, col[j][2]);
+                }
+            }
+        }
+#pragma unroll
+        for (int t = 0; t < CT; ++t) {
+            if (t < p.C) {
+                const bool on = mask & (1u << t);
+                float *o = p.colors + ((int64_t)t * N + n) * 3;
+                const float c0 = (t & 1) ? col[t / 2][0].y : col[t / 2][0].x, c1 = (t & 1) ? col[t / 2][1].y : col[t / 2][1].x,
+                            c2 = (t & 1) ? col[t / 2][2].y : col[t / 2][2].x;
+                st_cs(o, on ? c0 : 0.f); st_cs(o + 1, on ? c1 : 0.f); st_cs(o + 2, on ? c2 : 0.f);
+            }
+        }
+        sbase = (sbase + K) % RING;
+        hs = (hs + 1) % HR;
+        mask = mask_next;
+    }
+    cp_async_wait<0>();
+}
+
 // ---------------------------------------------------------------------------------------------
 // backward (no g_campos: that optional reduction stays on the generic kernel)
 // ---------------------------------------------------------------------------------------------
@@ -296,6 +387,184 @@ __global__ void __launch_bounds__(PBLOCK, 2) nasg_bwd_pipe_kernel(BwdParams p)
 }
 
 // ---------------------------------------------------------------------------------------------
+// backward, two cameras per packed f32x2 instruction (CT >= 2)
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ float hsum(float2 a) { return a.x + a.y; }
+
+#ifndef NASG_BWD2_MINB
+#define NASG_BWD2_MINB 2
+#endif
+// raw visibility bytes of one Gaussian, combined into a bit mask one iteration after the loads were issued
+struct RawMask { unsigned b[4]; };
+__device__ __forceinline__ RawMask load_raw_mask(const uint8_t *vis, int64_t N, int64_t n, int C)
+{
+    RawMask m;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) m.b[c] = (n < N) ? ((c < C) ? (vis ? vis[(int64_t)c * N + n] : 1u) : 0u) : 0u;
+    return m;
+}
+__device__ __forceinline__ unsigned combine_mask(const RawMask &m)
+{
+    return (m.b[0] ? 1u : 0u) | (m.b[1] ? 2u : 0u) | (m.b[2] ? 4u : 0u) | (m.b[3] ? 8u : 0u);
+}
+
+template <int K, int CT, bool EXACT>
+__global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(BwdParams p)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int HR = PipeCfg<K>::HR, HF = 3 + 3 * CT, NP = (CT + 1) / 2;
+    const Ring r = carve(smem_raw);
+    const int tid = threadIdx.x;
+    const int64_t N = p.N, stride = (int64_t)gridDim.x * PBLOCK;
+    int64_t n = (int64_t)blockIdx.x * PBLOCK + tid;
+    const int C = p.C;
+
+    auto prefetch_item = [&](int64_t gn, int l, int slot, int hslot) {
+        prefetch_lobe(r, slot, tid, p.quat, p.shape, p.amp, N, gn, l);
+        if (l == 0 && gn < N) {
+            float *h = r.h + (hslot * HF) * PBLOCK + tid;
+            cp_async4(h, p.means + 3 * gn); cp_async4(h + PBLOCK, p.means + 3 * gn + 1);
+            cp_async4(h + 2 * PBLOCK, p.means + 3 * gn + 2);
+#pragma unroll
+            for (int t = 0; t < CT; ++t) {
+                if (t < C) {
+                    const float *g = p.g_colors + ((int64_t)t * N + gn) * 3;
+                    cp_async4(h + (3 + 3 * t) * PBLOCK, g); cp_async4(h + (4 + 3 * t) * PBLOCK, g + 1);
+                    cp_async4(h + (5 + 3 * t) * PBLOCK, g + 2);
+                }
+            }
+        }
+        cp_async_commit();
+    };
+#pragma unroll
+    for (int j = 0; j < DIST; ++j) prefetch_item(n + (j / K) * stride, j % K, j % RING, (j / K) % HR);
+
+    unsigned sbase = 0, hs = 0;
+    unsigned mask = combine_mask(load_raw_mask(p.vis, N, n, C));
+    for (; n < N; n += stride) {
+        const RawMask raw_next = load_raw_mask(p.vis, N, n + stride, C);       // consumed at the end of this iteration
+        // camera slots in pairs (x = slot 2j, y = slot 2j+1). A culled or padding slot gets an exponent bias of
+        // -1e30: its lobe value and with it every gradient contribution is exactly 0.
+        float2 dx[NP], dy[NP], dz[NP], idist[NP], bias[NP], gd[NP][3];
+        const float *h = r.h + (hs * HF) * PBLOCK + tid;                        // header of this Gaussian (valid after lobe 0 landed)
+#pragma unroll 1
+        for (int l = 0; l < K; ++l) {
+            prefetch_item(n + ((l + DIST) / K) * stride, (l + DIST) % K, (sbase + l + DIST) % RING, (hs + (l + DIST) / K) % HR);
+            cp_async_wait<DIST>();
+            if (l == 0) {
+                const float2 mx = splat(h[0]), my = splat(h[PBLOCK]), mz = splat(h[2 * PBLOCK]);
+                float gdc0 = 0.f, gdc1 = 0.f, gdc2 = 0.f;
+#pragma unroll
+                for (int j = 0; j < NP; ++j) {
+                    const int t0 = 2 * j, t1 = 2 * j + 1;
+                    const int c0 = t0 < C ? t0 : 0, c1 = t1 < C ? t1 : 0;
+                    const bool on0 = mask & (1u << t0), on1 = (t1 < CT) && (mask & (1u << t1));
+                    const float2 ex = sub2(mx, make_float2(__ldg(p.campos + 3 * c0), __ldg(p.campos + 3 * c1)));
+                    const float2 ey = sub2(my, make_float2(__ldg(p.campos + 3 * c0 + 1), __ldg(p.campos + 3 * c1 + 1)));
+                    const float2 ez = sub2(mz, make_float2(__ldg(p.campos + 3 * c0 + 2), __ldg(p.campos + 3 * c1 + 2)));
+                    const float2 r2 = fma2(ex, ex, fma2(ey, ey, mul2(ez, ez)));
+                    float2 inv = make_float2(f_rsqrt(r2.x), f_rsqrt(r2.y));
+                    inv = mul2(inv, fma2(mul2(splat(-0.5f), r2), mul2(inv, inv), splat(1.5f)));
+                    dx[j] = mul2(ex, inv); dy[j] = mul2(ey, inv); dz[j] = mul2(ez, inv);
+                    idist[j] = inv;
+                    bias[j] = make_float2(on0 ? 0.f : -1e30f, on1 ? 0.f : -1e30f);
+                    if (on0) { gdc0 += h[(3 + 3 * t0) * PBLOCK]; gdc1 += h[(4 + 3 * t0) * PBLOCK]; gdc2 += h[(5 + 3 * t0) * PBLOCK]; }
+                    if (t1 < CT && on1) { gdc0 += h[(3 + 3 * t1) * PBLOCK]; gdc1 += h[(4 + 3 * t1) * PBLOCK]; gdc2 += h[(5 + 3 * t1) * PBLOCK]; }
+                    gd[j][0] = gd[j][1] = gd[j][2] = splat(0.f);
+                }
+                if (p.g_dc) { st_cs(p.g_dc + n, gdc0); st_cs(p.g_dc + N + n, gdc1); st_cs(p.g_dc + 2 * N + n, gdc2); }
+            }
+            const int64_t ln = (int64_t)l * N + n;
+            float4 gq = make_float4(0.f, 0.f, 0.f, 0.f), gs = make_float4(0.f, 0.f, 0.f, 0.f);
+            float gw0 = 0.f, gw1 = 0.f, gw2 = 0.f;
+            if (mask != 0) {
+                const int slot = (sbase + l) % RING;
+                const float4 sp = r.s[slot * PBLOCK + tid];
+                const float2 w0 = splat(r.w[(slot * 3 + 0) * PBLOCK + tid]), w1 = splat(r.w[(slot * 3 + 1) * PBLOCK + tid]),
+                             w2 = splat(r.w[(slot * 3 + 2) * PBLOCK + tid]);
+                Lobe L; LobeBwd B;
+                lobe_setup<EXACT, true>(r.q[slot * PBLOCK + tid], sp, L, B);
+                const float2 z2 = splat(0.f);
+                float2 pw0 = z2, pw1 = z2, pw2 = z2;                             // packed accumulators, halves summed below
+                float2 gX0 = z2, gX1 = z2, gX2 = z2, gZ0 = z2, gZ1 = z2, gZ2 = z2;
+                float2 S0 = z2, S1 = z2, S2 = z2, Sk = z2, Sp = z2;
+                const float2 lam2 = splat(B.lam2), a2 = splat(L.a), nk2 = splat(-sp.z);
+#pragma unroll
+                for (int j = 0; j < NP; ++j) {
+                    const int t0 = 2 * j, t1 = (2 * j + 1 < CT) ? 2 * j + 1 : 2 * j;
+                    const float2 gc0 = make_float2(h[(3 + 3 * t0) * PBLOCK], h[(3 + 3 * t1) * PBLOCK]);     // g_colors of the pair
+                    const float2 gc1 = make_float2(h[(4 + 3 * t0) * PBLOCK], h[(4 + 3 * t1) * PBLOCK]);
+                    const float2 gc2 = make_float2(h[(5 + 3 * t0) * PBLOCK], h[(5 + 3 * t1) * PBLOCK]);
+                    EvalTerms2 T;
+                    const float2 G = lobe_eval2<true>(L, dx[j], dy[j], dz[j], bias[j], T);
+                    const float2 gG = fma2(gc0, w0, fma2(gc1, w1, mul2(gc2, w2)));                      // dL/dG, eq.(6)
+                    pw0 = fma2(gc0, G, pw0); pw1 = fma2(gc1, G, pw1); pw2 = fma2(gc2, G, pw2);
+                    const float2 gGG = mul2(gG, G);
+                    const float2 A_tau = mul2(T.Lk, fma2(lam2, T.kp, splat(1.0f)));                     // d ln(pE)/d tau
+                    const float2 A_kap2 = mul2(fma2(mul2(lam2, add2(T.tau, splat(1.0f))), T.kp, T.tau), T.inv_2kappa);  // (d ln(pE)/d kappa)/2
+                    const float2 B1 = mul2(mul2(add2(gGG, gGG), A_tau), T.inv_s2);
+                    const float2 hs_ = mul2(mul2(gG, T.Gh), T.sn);                                      // carrier, eqs.(59),(65)
+                    const float2 gu = fma2(mul2(B1, a2), T.u, mul2(hs_, nk2));                          // gG dG/du (eqs.57-60)
+                    const float2 gv = fma2(mul2(B1, T.tau), T.v, mul2(gGG, A_kap2));                    // gG dG/dv (eqs.61-64)
+                    S0 = add2(S0, gGG);
+                    S1 = fma2(gGG, T.em1, S1);
+                    S2 = fma2(B1, T.uu, S2);
+                    Sk = fma2(hs_, T.u, Sk);
+                    Sp = add2(Sp, hs_);
+                    gX0 = fma2(gu, dx[j], gX0); gX1 = fma2(gu, dy[j], gX1); gX2 = fma2(gu, dz[j], gX2);
+                    gZ0 = fma2(gv, dx[j], gZ0); gZ1 = fma2(gv, dy[j], gZ1); gZ2 = fma2(gv, dz[j], gZ2);
+                    gd[j][0] = fma2(gu, splat(L.Xx), fma2(gv, splat(L.Zx), gd[j][0]));
+                    gd[j][1] = fma2(gu, splat(L.Xy), fma2(gv, splat(L.Zy), gd[j][1]));
+                    gd[j][2] = fma2(gu, splat(L.Xz), fma2(gv, splat(L.Zz), gd[j][2]));
+                }
+                gw0 = hsum(pw0); gw1 = hsum(pw1); gw2 = hsum(pw2);
+                const float s0 = hsum(S0), s1 = hsum(S1), s2 = hsum(S2), sk = hsum(Sk), sp_ = hsum(Sp);
+                const float X0 = hsum(gX0), X1 = hsum(gX1), X2 = hsum(gX2), Z0 = hsum(gZ0), Z1 = hsum(gZ1), Z2 = hsum(gZ2);
+                gs.x = fmaf(0.5f * s2, L.a + 1.0f, -s0 * B.nA);          // (lambda, a) = (e^{l2}, e^{l1-l2} - 1)
+                gs.y = fmaf(B.lam2, s1, -s0 * B.nL) - gs.x;
+                gs.z = -fmaf(s0, B.nk, sk);
+                gs.w = -sp_;
+                // J^T of columns X, Z of R(qhat), qhat = q/|q| (re-normalised here: cheaper than keeping it live)
+                const float4 q = r.q[slot * PBLOCK + tid];
+                const float qq = q.x * q.x + q.y * q.y + q.z * q.z + q.w * q.w;
+                float inv_qn = f_rsqrt(qq);
+                inv_qn = inv_qn * fmaf(-0.5f * qq, inv_qn * inv_qn, 1.5f);
+                const float w = q.x * inv_qn, x = q.y * inv_qn, y = q.z * inv_qn, z = q.w * inv_qn;
+                const float a0 = 2.0f * (z * X1 - y * X2 + y * Z0 - x * Z1);
+                const float a1 = 2.0f * (y * X1 + z * X2 + z * Z0 - w * Z1) - 4.0f * x * Z2;
+                const float a2_ = 2.0f * (x * X1 - w * X2 + w * Z0 + z * Z1) - 4.0f * y * (X0 + Z2);
+                const float a3 = 2.0f * (w * X1 + x * X2 + x * Z0 + y * Z1) - 4.0f * z * X0;
+                const float dot = w * a0 + x * a1 + y * a2_ + z * a3;
+                gq.x = (a0 - w * dot) * inv_qn; gq.y = (a1 - x * dot) * inv_qn;
+                gq.z = (a2_ - y * dot) * inv_qn; gq.w = (a3 - z * dot) * inv_qn;
+            }
+            if (p.g_quat) st_cs4(p.g_quat + 4 * ln, gq);
+            if (p.g_shape) st_cs4(p.g_shape + 4 * ln, gs);
+            if (p.g_amp) {
+                float *o = p.g_amp + (int64_t)l * 3 * N + n;
+                st_cs(o, gw0); st_cs(o + N, gw1); st_cs(o + 2 * N, gw2);
+            }
+        }
+        if (p.g_means) {        // through d = Delta/|Delta|: (I - d d^T)/|Delta|   (gd of a culled slot is exactly 0)
+            float2 gm0 = splat(0.f), gm1 = splat(0.f), gm2 = splat(0.f);
+#pragma unroll
+            for (int j = 0; j < NP; ++j) {
+                const float2 dg = fma2(dx[j], gd[j][0], fma2(dy[j], gd[j][1], mul2(dz[j], gd[j][2])));
+                gm0 = fma2(sub2(gd[j][0], mul2(dx[j], dg)), idist[j], gm0);
+                gm1 = fma2(sub2(gd[j][1], mul2(dy[j], dg)), idist[j], gm1);
+                gm2 = fma2(sub2(gd[j][2], mul2(dz[j], dg)), idist[j], gm2);
+            }
+            float *o = p.g_means + 3 * n;
+            st_cs(o, hsum(gm0)); st_cs(o + 1, hsum(gm1)); st_cs(o + 2, hsum(gm2));
+        }
+        sbase = (sbase + K) % RING;
+        hs = (hs + 1) % HR;
+        mask = combine_mask(raw_next);
+    }
+    cp_async_wait<0>();
+}
+
+// ---------------------------------------------------------------------------------------------
 // launchers: persistent grid, 2 blocks per SM
 // ---------------------------------------------------------------------------------------------
 template <int K, int CT>
@@ -304,8 +573,13 @@ static cudaError_t launch_fwd_pipe_kc(const FwdParams &p, bool exact, cudaStream
     constexpr size_t smem = pipe_smem_bytes(PipeCfg<K>::HR, 6);
     const dim3 block(PBLOCK);
     static int cache[2][64] = {{0}};        // per (K, CT, norm mode) instantiation and device
-    if (exact) nasg_fwd_pipe_kernel<K, CT, true><<<pipe_grid(nasg_fwd_pipe_kernel<K, CT, true>, smem, p.N, cache[1]), block, smem, st>>>(p);
-    else nasg_fwd_pipe_kernel<K, CT, false><<<pipe_grid(nasg_fwd_pipe_kernel<K, CT, false>, smem, p.N, cache[0]), block, smem, st>>>(p);
+    if constexpr (CT >= 2) {
+        if (exact) nasg_fwd_pipe2_kernel<K, CT, true><<<pipe_grid(nasg_fwd_pipe2_kernel<K, CT, true>, smem, p.N, cache[1]), block, smem, st>>>(p);
+        else nasg_fwd_pipe2_kernel<K, CT, false><<<pipe_grid(nasg_fwd_pipe2_kernel<K, CT, false>, smem, p.N, cache[0]), block, smem, st>>>(p);
+    } else {
+        if (exact) nasg_fwd_pipe_kernel<K, CT, true><<<pipe_grid(nasg_fwd_pipe_kernel<K, CT, true>, smem, p.N, cache[1]), block, smem, st>>>(p);
+        else nasg_fwd_pipe_kernel<K, CT, false><<<pipe_grid(nasg_fwd_pipe_kernel<K, CT, false>, smem, p.N, cache[0]), block, smem, st>>>(p);
+    }
     return cudaGetLastError();
 }
 template <int K>
@@ -335,8 +609,13 @@ static cudaError_t launch_bwd_pipe_kc(const BwdParams &p, bool exact, cudaStream
     constexpr size_t smem = pipe_smem_bytes(PipeCfg<K>::HR, 3 + 3 * CT);
     const dim3 block(PBLOCK);
     static int cache[2][64] = {{0}};        // per (K, CT, norm mode) instantiation and device
-    if (exact) nasg_bwd_pipe_kernel<K, CT, true><<<pipe_grid(nasg_bwd_pipe_kernel<K, CT, true>, smem, p.N, cache[1]), block, smem, st>>>(p);
-    else nasg_bwd_pipe_kernel<K, CT, false><<<pipe_grid(nasg_bwd_pipe_kernel<K, CT, false>, smem, p.N, cache[0]), block, smem, st>>>(p);
+    if constexpr (CT >= 2) {
+        if (exact) nasg_bwd_pipe2_kernel<K, CT, true><<<pipe_grid(nasg_bwd_pipe2_kernel<K, CT, true>, smem, p.N, cache[1]), block, smem, st>>>(p);
+        else nasg_bwd_pipe2_kernel<K, CT, false><<<pipe_grid(nasg_bwd_pipe2_kernel<K, CT, false>, smem, p.N, cache[0]), block, smem, st>>>(p);
+    } else {
+        if (exact) nasg_bwd_pipe_kernel<K, CT, true><<<pipe_grid(nasg_bwd_pipe_kernel<K, CT, true>, smem, p.N, cache[1]), block, smem, st>>>(p);
+        else nasg_bwd_pipe_kernel<K, CT, false><<<pipe_grid(nasg_bwd_pipe_kernel<K, CT, false>, smem, p.N, cache[0]), block, smem, st>>>(p);
+    }
     return cudaGetLastError();
 }
 template <int K>

@@ -7,7 +7,10 @@
 
 namespace nasg {
 
-constexpr int PBLOCK = 256;
+#ifndef NASG_PBLOCK
+#define NASG_PBLOCK 256
+#endif
+constexpr int PBLOCK = NASG_PBLOCK;
 
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
 {

@@ -147,7 +147,13 @@ def test_optional_gradient_pointers_and_determinism(B, W):
     only = {"g_shape": torch.full_like(g_all["g_shape"], 7.0)}
     B.nasg_eval_bwd(d["means"], d["quat"], d["shape"], d["amp"], d["dc"], d["campos"], d["g_colors"], d["vis"], 1, out=only)
     torch.cuda.synchronize()
-    assert torch.equal(only["g_shape"], g_all["g_shape"])
+    # (g_all came from the generic kernels, which g_campos selects; `only` from the fast path: same numbers up
+    # to summation order over the cameras, and the fast path is itself bit-reproducible)
+    assert (only["g_shape"] - g_all["g_shape"]).abs().max() <= 1e-5 * g_all["g_shape"].abs().max()
+    again = {"g_shape": torch.full_like(g_all["g_shape"], 7.0)}
+    B.nasg_eval_bwd(d["means"], d["quat"], d["shape"], d["amp"], d["dc"], d["campos"], d["g_colors"], d["vis"], 1, out=again)
+    torch.cuda.synchronize()
+    assert torch.equal(only["g_shape"], again["g_shape"])
 
 
 def test_direction_on_the_lobe_axis_is_finite(B, oracle):
