@@ -312,7 +312,8 @@ __device__ __forceinline__ float2 lobe_eval2(const Lobe &L, float2 dx, float2 dy
     const float2 sw = mul2(s2, w2);
     const float2 rw = make_float2(f_rcp(sw.x), f_rcp(sw.y));
     const float2 inv_s2 = mul2(rw, w2);
-    const float2 q = mul2(s2, mul2(s2, rw));                       // (1 - |v|)/2
+    const float2 s2rw = mul2(s2, rw);                              // 1/(2 (1 + |v|))
+    const float2 q = mul2(s2, s2rw);                               // (1 - |v|)/2
     const float2 tau = mul2(mul2(splat(L.a), uu), inv_s2);
     const bool up0 = v.x > 0.0f, up1 = v.y > 0.0f;
     // log2 kappa (log2_kappa)
@@ -346,7 +347,7 @@ __device__ __forceinline__ float2 lobe_eval2(const Lobe &L, float2 dx, float2 dy
     if (FULL) {
         T.u = u; T.v = v; T.uu = uu; T.inv_s2 = inv_s2; T.tau = tau; T.Lk = mul2(splat(LN2), L2);
         T.kp = add2(em1, splat(1.0f)); T.em1 = em1;
-        const float2 hi = mul2(add2(s2, s2), rw), lo = mul2(mul2(splat(0.5f), w2), inv_s2);   // 1/(1+v)
+        const float2 hi = add2(s2rw, s2rw), lo = mul2(mul2(splat(0.5f), w2), inv_s2);   // 1/(1+v) on the lobe side / far side
         T.inv_2kappa = make_float2(up0 ? hi.x : lo.x, up1 ? hi.y : lo.y);
         T.Gh = Gh; T.sn = make_float2(f_sin(ang.x), f_sin(ang.y));
     }

@@ -38,6 +38,47 @@ __host__ __device__ constexpr size_t pipe_smem_bytes(int HR, int HF)
 {
     return (size_t)PBLOCK * (RING * (16 + 16 + 12) + HR * HF * 4);
 }
+// the packed kernels stage the visibility bytes of a Gaussian next to its header: [HR][4][PBLOCK] bytes
+__host__ __device__ constexpr size_t pipe2_smem_bytes(int HR, int HF) { return pipe_smem_bytes(HR, HF) + (size_t)HR * 4 * PBLOCK; }
+
+// Visibility mask of the packed kernels. A byte load from global memory that is consumed in the same
+// iteration stalls the warp for a DRAM latency (ncu: 11% of all stall samples sat on it), and the compiler
+// places the consumer wherever it likes. When vis rows are 4-byte aligned (N % 4 == 0) every fourth lane
+// copies the 4 bytes of its quad with cp.async into the header slot instead, SH_DIST-style ahead of use;
+// the bytes are read back from shared memory after the wait + __syncwarp. Otherwise (vis == NULL or an
+// unaligned N) the raw bytes are loaded one Gaussian ahead into registers.
+struct RawMask { unsigned b[4]; };
+__device__ __forceinline__ RawMask load_raw_mask(const uint8_t *vis, int64_t N, int64_t n, int C)
+{
+    RawMask m;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) m.b[c] = (n < N) ? ((c < C) ? (vis ? vis[(int64_t)c * N + n] : 1u) : 0u) : 0u;
+    return m;
+}
+__device__ __forceinline__ unsigned combine_mask(const RawMask &m)
+{
+    return (m.b[0] ? 1u : 0u) | (m.b[1] ? 2u : 0u) | (m.b[2] ? 4u : 0u) | (m.b[3] ? 8u : 0u);
+}
+__device__ __forceinline__ bool vis_rows_aligned(const uint8_t *vis, int64_t N)
+{
+    return vis != nullptr && (N & 3) == 0 && (reinterpret_cast<uintptr_t>(vis) & 3u) == 0;
+}
+__device__ __forceinline__ void prefetch_vis(unsigned char *vm, int hslot, int tid, const uint8_t *vis, int64_t N, int64_t gn, int C)
+{
+    if ((tid & 3) == 0) {
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+            if (c < C) cp_async4(vm + (hslot * 4 + c) * PBLOCK + tid, vis + (int64_t)c * N + gn);
+    }
+}
+__device__ __forceinline__ unsigned staged_mask(const unsigned char *vm, int hslot, int tid, int C, bool valid)
+{
+    unsigned m = 0;
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+        if (c < C) m |= (vm[(hslot * 4 + c) * PBLOCK + tid] != 0 ? 1u : 0u) << c;
+    return valid ? m : 0u;
+}
 __device__ __forceinline__ Ring carve(unsigned char *raw)
 {
     Ring r;
@@ -161,6 +202,8 @@ __global__ void __launch_bounds__(PBLOCK, CT >= 3 ? 3 : 4) nasg_fwd_pipe2_kernel
     const int tid = threadIdx.x;
     const int64_t N = p.N, stride = (int64_t)gridDim.x * PBLOCK;
     int64_t n = (int64_t)blockIdx.x * PBLOCK + tid;
+    unsigned char *vm = smem_raw + pipe_smem_bytes(HR, HF);
+    const bool vis_cp = vis_rows_aligned(p.vis, N);
 
     auto prefetch_item = [&](int64_t gn, int l, int slot, int hslot) {
         prefetch_lobe(r, slot, tid, p.quat, p.shape, p.amp, N, gn, l);
@@ -170,6 +213,7 @@ __global__ void __launch_bounds__(PBLOCK, CT >= 3 ? 3 : 4) nasg_fwd_pipe2_kernel
             cp_async4(h + 2 * PBLOCK, p.means + 3 * gn + 2);
             cp_async4(h + 3 * PBLOCK, p.dc + gn); cp_async4(h + 4 * PBLOCK, p.dc + N + gn);
             cp_async4(h + 5 * PBLOCK, p.dc + 2 * N + gn);
+            if (vis_cp) prefetch_vis(vm, hslot, tid, p.vis, N, gn, p.C);
         }
         cp_async_commit();
     };
@@ -177,19 +221,25 @@ __global__ void __launch_bounds__(PBLOCK, CT >= 3 ? 3 : 4) nasg_fwd_pipe2_kernel
     for (int j = 0; j < DIST; ++j) prefetch_item(n + (j / K) * stride, j % K, j % RING, (j / K) % HR);
 
     unsigned sbase = 0, hs = 0;                  // ring slot of lobe 0 / header slot of the current Gaussian
-    unsigned mask = load_mask(p.vis, N, n, p.C);
-    for (; n < N; n += stride) {
-        const unsigned mask_next = load_mask(p.vis, N, n + stride, p.C);     // lands during this Gaussian
+    RawMask raw = {{0u, 0u, 0u, 0u}};
+    if (!vis_cp) raw = load_raw_mask(p.vis, N, n, p.C);
+    for (; n - (tid & 31) < N; n += stride) {       // warp-uniform trip count: lanes past N idle (mask 0, no stores)
+        const bool valid = n < N;
+        RawMask raw_next = {{0u, 0u, 0u, 0u}};
+        if (!vis_cp) raw_next = load_raw_mask(p.vis, N, n + stride, p.C);
+        unsigned mask = 0;
         // camera slots live in pairs (x = slot 2j, y = slot 2j+1) so that the evaluation runs on packed
         // f32x2 arithmetic; a slot beyond C repeats camera 0 and is never stored
         constexpr int NP = (CT + 1) / 2;
         float2 dx[NP], dy[NP], dz[NP], col[NP][3];
 #pragma unroll
         for (int l = 0; l < K; ++l) {
-            prefetch_item(n + ((l + DIST) / K) * stride, (l + DIST) % K, ((PipeCfg<K>::STATIC_SLOTS ? 0u : sbase) + (l + DIST) % RING) % RING,
+            prefetch_item(n + ((l + DIST) / K) * stride, (l + DIST) % K, (sbase + (l + DIST) % RING) % RING,
                           (hs + (l + DIST) / K) % HR);
             cp_async_wait<DIST>();
             if (l == 0) {
+                if (vis_cp) { __syncwarp(); mask = staged_mask(vm, hs, tid, p.C, valid); }
+                else mask = combine_mask(raw);
                 const float *h = r.h + (hs * HF) * PBLOCK + tid;
                 const float2 mx = splat(h[0]), my = splat(h[PBLOCK]), mz = splat(h[2 * PBLOCK]);
                 const float2 dc0 = splat(h[3 * PBLOCK]), dc1 = splat(h[4 * PBLOCK]), dc2 = splat(h[5 * PBLOCK]);
@@ -207,7 +257,7 @@ __global__ void __launch_bounds__(PBLOCK, CT >= 3 ? 3 : 4) nasg_fwd_pipe2_kernel
                 }
             }
             if (mask != 0) {
-                const int slot = ((PipeCfg<K>::STATIC_SLOTS ? 0u : sbase) + l) % RING;
+                const int slot = (sbase + l) % RING;
                 const float4 q = r.q[slot * PBLOCK + tid];
                 const float4 sp = r.s[slot * PBLOCK + tid];
                 const float2 w0 = splat(r.w[(slot * 3 + 0) * PBLOCK + tid]), w1 = splat(r.w[(slot * 3 + 1) * PBLOCK + tid]),
@@ -227,7 +277,7 @@ __global__ void __launch_bounds__(PBLOCK, CT >= 3 ? 3 : 4) nasg_fwd_pipe2_kernel
         }
 #pragma unroll
         for (int t = 0; t < CT; ++t) {
-            if (t < p.C) {
+            if (t < p.C && valid) {
                 const bool on = mask & (1u << t);
                 float *o = p.colors + ((int64_t)t * N + n) * 3;
                 const float c0 = (t & 1) ? col[t / 2][0].y : col[t / 2][0].x, c1 = (t & 1) ? col[t / 2][1].y : col[t / 2][1].x,
@@ -237,7 +287,7 @@ __global__ void __launch_bounds__(PBLOCK, CT >= 3 ? 3 : 4) nasg_fwd_pipe2_kernel
         }
         sbase = (sbase + K) % RING;
         hs = (hs + 1) % HR;
-        mask = mask_next;
+        raw = raw_next;
     }
     cp_async_wait<0>();
 }
@@ -394,20 +444,6 @@ __device__ __forceinline__ float hsum(float2 a) { return a.x + a.y; }
 #ifndef NASG_BWD2_MINB
 #define NASG_BWD2_MINB 2
 #endif
-// raw visibility bytes of one Gaussian, combined into a bit mask one iteration after the loads were issued
-struct RawMask { unsigned b[4]; };
-__device__ __forceinline__ RawMask load_raw_mask(const uint8_t *vis, int64_t N, int64_t n, int C)
-{
-    RawMask m;
-#pragma unroll
-    for (int c = 0; c < 4; ++c) m.b[c] = (n < N) ? ((c < C) ? (vis ? vis[(int64_t)c * N + n] : 1u) : 0u) : 0u;
-    return m;
-}
-__device__ __forceinline__ unsigned combine_mask(const RawMask &m)
-{
-    return (m.b[0] ? 1u : 0u) | (m.b[1] ? 2u : 0u) | (m.b[2] ? 4u : 0u) | (m.b[3] ? 8u : 0u);
-}
-
 template <int K, int CT, bool EXACT>
 __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(BwdParams p)
 {
@@ -418,6 +454,8 @@ __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(
     const int64_t N = p.N, stride = (int64_t)gridDim.x * PBLOCK;
     int64_t n = (int64_t)blockIdx.x * PBLOCK + tid;
     const int C = p.C;
+    unsigned char *vm = smem_raw + pipe_smem_bytes(HR, HF);
+    const bool vis_cp = vis_rows_aligned(p.vis, N);
 
     auto prefetch_item = [&](int64_t gn, int l, int slot, int hslot) {
         prefetch_lobe(r, slot, tid, p.quat, p.shape, p.amp, N, gn, l);
@@ -433,6 +471,7 @@ __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(
                     cp_async4(h + (5 + 3 * t) * PBLOCK, g + 2);
                 }
             }
+            if (vis_cp) prefetch_vis(vm, hslot, tid, p.vis, N, gn, C);
         }
         cp_async_commit();
     };
@@ -440,9 +479,13 @@ __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(
     for (int j = 0; j < DIST; ++j) prefetch_item(n + (j / K) * stride, j % K, j % RING, (j / K) % HR);
 
     unsigned sbase = 0, hs = 0;
-    unsigned mask = combine_mask(load_raw_mask(p.vis, N, n, C));
-    for (; n < N; n += stride) {
-        const RawMask raw_next = load_raw_mask(p.vis, N, n + stride, C);       // consumed at the end of this iteration
+    RawMask raw = {{0u, 0u, 0u, 0u}};
+    if (!vis_cp) raw = load_raw_mask(p.vis, N, n, C);
+    for (; n - (tid & 31) < N; n += stride) {       // warp-uniform trip count: lanes past N idle (mask 0, no stores)
+        const bool valid = n < N;
+        RawMask raw_next = {{0u, 0u, 0u, 0u}};
+        if (!vis_cp) raw_next = load_raw_mask(p.vis, N, n + stride, C);
+        unsigned mask = 0;
         // camera slots in pairs (x = slot 2j, y = slot 2j+1). A culled or padding slot gets an exponent bias of
         // -1e30: its lobe value and with it every gradient contribution is exactly 0.
         float2 dx[NP], dy[NP], dz[NP], idist[NP], bias[NP], gd[NP][3];
@@ -452,6 +495,8 @@ __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(
             prefetch_item(n + ((l + DIST) / K) * stride, (l + DIST) % K, (sbase + l + DIST) % RING, (hs + (l + DIST) / K) % HR);
             cp_async_wait<DIST>();
             if (l == 0) {
+                if (vis_cp) { __syncwarp(); mask = staged_mask(vm, hs, tid, C, valid); }
+                else mask = combine_mask(raw);
                 const float2 mx = splat(h[0]), my = splat(h[PBLOCK]), mz = splat(h[2 * PBLOCK]);
                 float gdc0 = 0.f, gdc1 = 0.f, gdc2 = 0.f;
 #pragma unroll
@@ -472,7 +517,7 @@ __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(
                     if (t1 < CT && on1) { gdc0 += h[(3 + 3 * t1) * PBLOCK]; gdc1 += h[(4 + 3 * t1) * PBLOCK]; gdc2 += h[(5 + 3 * t1) * PBLOCK]; }
                     gd[j][0] = gd[j][1] = gd[j][2] = splat(0.f);
                 }
-                if (p.g_dc) { st_cs(p.g_dc + n, gdc0); st_cs(p.g_dc + N + n, gdc1); st_cs(p.g_dc + 2 * N + n, gdc2); }
+                if (p.g_dc && valid) { st_cs(p.g_dc + n, gdc0); st_cs(p.g_dc + N + n, gdc1); st_cs(p.g_dc + 2 * N + n, gdc2); }
             }
             const int64_t ln = (int64_t)l * N + n;
             float4 gq = make_float4(0.f, 0.f, 0.f, 0.f), gs = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -538,14 +583,14 @@ __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(
                 gq.x = (a0 - w * dot) * inv_qn; gq.y = (a1 - x * dot) * inv_qn;
                 gq.z = (a2_ - y * dot) * inv_qn; gq.w = (a3 - z * dot) * inv_qn;
             }
-            if (p.g_quat) st_cs4(p.g_quat + 4 * ln, gq);
-            if (p.g_shape) st_cs4(p.g_shape + 4 * ln, gs);
-            if (p.g_amp) {
+            if (p.g_quat && valid) st_cs4(p.g_quat + 4 * ln, gq);
+            if (p.g_shape && valid) st_cs4(p.g_shape + 4 * ln, gs);
+            if (p.g_amp && valid) {
                 float *o = p.g_amp + (int64_t)l * 3 * N + n;
                 st_cs(o, gw0); st_cs(o + N, gw1); st_cs(o + 2 * N, gw2);
             }
         }
-        if (p.g_means) {        // through d = Delta/|Delta|: (I - d d^T)/|Delta|   (gd of a culled slot is exactly 0)
+        if (p.g_means && valid) {        // through d = Delta/|Delta|: (I - d d^T)/|Delta|   (gd of a culled slot is exactly 0)
             float2 gm0 = splat(0.f), gm1 = splat(0.f), gm2 = splat(0.f);
 #pragma unroll
             for (int j = 0; j < NP; ++j) {
@@ -559,7 +604,7 @@ __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(
         }
         sbase = (sbase + K) % RING;
         hs = (hs + 1) % HR;
-        mask = combine_mask(raw_next);
+        raw = raw_next;
     }
     cp_async_wait<0>();
 }
@@ -570,7 +615,7 @@ __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(
 template <int K, int CT>
 static cudaError_t launch_fwd_pipe_kc(const FwdParams &p, bool exact, cudaStream_t st)
 {
-    constexpr size_t smem = pipe_smem_bytes(PipeCfg<K>::HR, 6);
+    constexpr size_t smem = CT >= 2 ? pipe2_smem_bytes(PipeCfg<K>::HR, 6) : pipe_smem_bytes(PipeCfg<K>::HR, 6);
     const dim3 block(PBLOCK);
     static int cache[2][64] = {{0}};        // per (K, CT, norm mode) instantiation and device
     if constexpr (CT >= 2) {
@@ -606,7 +651,7 @@ cudaError_t launch_nasg_fwd_pipe(const FwdParams &p, int K, bool exact, cudaStre
 template <int K, int CT>
 static cudaError_t launch_bwd_pipe_kc(const BwdParams &p, bool exact, cudaStream_t st)
 {
-    constexpr size_t smem = pipe_smem_bytes(PipeCfg<K>::HR, 3 + 3 * CT);
+    constexpr size_t smem = CT >= 2 ? pipe2_smem_bytes(PipeCfg<K>::HR, 3 + 3 * CT) : pipe_smem_bytes(PipeCfg<K>::HR, 3 + 3 * CT);
     const dim3 block(PBLOCK);
     static int cache[2][64] = {{0}};        // per (K, CT, norm mode) instantiation and device
     if constexpr (CT >= 2) {
