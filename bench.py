@@ -174,8 +174,8 @@ def run_ours(args, W, cfg):
 
     # each rank owns a shard of independent Gaussians (weak scaling: the per-GPU shard is the config's N;
     # rank r draws its shard from seed + 1000 r). No data-path collective: the path is per-Gaussian.
-    import dataclasses
-    rcfg = dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank)
+    from paper_2606_09794_b200 import sharding as S
+    rcfg = S.weak_scaling_config(cfg, rank)
     inp = W.make_sh(rcfg) if cfg.kind == "sh" else W.make_nasg(rcfg)
     N, C, K = inp["N"], inp["C"], inp.get("K", 0)
     keys = ("means", "coeffs", "campos", "vis", "g_colors") if cfg.kind == "sh" else \
@@ -226,10 +226,7 @@ def run_ours(args, W, cfg):
     total_ms = ev[0][0].elapsed_time(ev[-1][2])
     fwd_ms = sum(e[0].elapsed_time(e[1]) for e in ev) / args.steps
     bwd_ms = sum(e[1].elapsed_time(e[2]) for e in ev) / args.steps
-    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
+    total_ms = S.max_over_ranks(total_ms, "cuda")
     value = world * N * args.steps / (total_ms * 1e-3)
 
     # ---- end to end through the host-buffer C-ABI entry point (pinned host memory) -----------------
@@ -255,10 +252,7 @@ def run_ours(args, W, cfg):
         e2e_call()
     e1.record(stream)
     barrier()
-    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_value = world * N * e2e_steps / (float(t.item()) * 1e-3)
+    e2e_value = world * N * e2e_steps / (S.max_over_ranks(e0.elapsed_time(e1), "cuda") * 1e-3)
 
     if rank == 0:
         fb, bb = algorithmic_bytes(cfg.kind, K, C, d["vis"] is not None)
