@@ -110,8 +110,15 @@ size_t nasg_workspace_bytes(int64_t N, int32_t K, int32_t C);
  * Same computation, forward then backward, but every array pointer in `in`, `colors`, `g_colors`
  * and `out` is a HOST pointer (pinned memory makes the copies asynchronous and fast; pageable works).
  * The call copies the inputs to `dev_scratch` (a DEVICE buffer of >= *_host_scratch_bytes), runs the
- * two kernels, copies colours and gradients back, all on cuda_stream, and returns without
- * synchronising. out->workspace is ignored (carved from dev_scratch). */
+ * two kernels and copies colours and gradients back. Gaussians are independent, so a large call is cut
+ * into chunks of contiguous n-ranges that run as a three-stage pipeline (H2D of chunk i+1, kernels on
+ * chunk i, D2H of chunk i-1) on three streams the library creates once per device on first use: PCIe is
+ * full duplex, so the copies in the two directions overlap. Ordering is that of cuda_stream: the work
+ * starts after what is already queued there, cuda_stream waits for the last copy, and the call returns
+ * without synchronising; host buffers must stay valid until cuda_stream reaches that point.
+ * A call that asks for g_campos (a sum over all Gaussians) runs as one chunk. Not CUDA-graph capturable.
+ * Calls on one device are serialised while they enqueue. out->workspace is ignored (carved from
+ * dev_scratch). */
 size_t nasg_host_scratch_bytes(int64_t N, int32_t K, int32_t C);
 int nasg_eval_fwd_bwd_host(const nasg_inputs *in, const float *g_colors, float *colors,
                            const nasg_grads *out, int norm_mode, void *dev_scratch,

@@ -37,6 +37,7 @@ struct ShParams {
 };
 
 int64_t grid_blocks(int64_t N);
+int api_cuda_fail(cudaError_t e);     // remembers e for nasg_strerror(), returns NASG_ERR_CUDA (nasg_api.cu)
 cudaError_t launch_nasg_fwd(const FwdParams &p, int K, bool exact, cudaStream_t st);
 cudaError_t launch_nasg_bwd(const BwdParams &p, int K, bool exact, cudaStream_t st);
 // fast path (nasg_pipe_kernels.cu): C <= 4, persistent threads, cp.async lobe ring; no g_campos

@@ -209,6 +209,41 @@ def test_host_entry_point_matches_device_path(B, W):
     assert torch.equal(out["g_means"], g["g_means"].cpu()) and torch.equal(out["g_campos"], g["g_campos"].cpu())
 
 
+def test_host_entry_point_chunked_pipeline(B, W):
+    """Large enough to be cut into several chunks (ragged last chunk): bit-identical to the device path."""
+    inp = W.make(2, 3 * 131072 + 4099)
+    d = to_dev(inp, NASG_KEYS)
+    col, g = run_nasg(B, d, 1)
+    host = {k: torch.from_numpy(np.ascontiguousarray(inp[k])).pin_memory() for k in NASG_KEYS}
+    N, K, C = inp["N"], inp["K"], inp["C"]
+    out = dict(colors=torch.empty((C, N, 3)).pin_memory(), g_means=torch.empty((N, 3)).pin_memory(),
+               g_quat=torch.empty((K, N, 4)).pin_memory(), g_shape=torch.empty((K, N, 4)).pin_memory(),
+               g_amp=torch.empty((K, 3, N)).pin_memory(), g_dc=torch.empty((3, N)).pin_memory())
+    scratch = torch.empty(B.nasg_host_scratch_bytes(N, K, C), dtype=torch.uint8, device="cuda")
+    side = torch.cuda.Stream()
+    for _ in range(2):                                   # twice: the internal streams/events are reused
+        for v in out.values():
+            v.fill_(7.0)
+        with torch.cuda.stream(side):
+            B.nasg_eval_fwd_bwd_host(host, out, scratch, 1, stream=side)
+        side.synchronize()                               # the caller's stream alone orders the call
+        assert torch.equal(out["colors"], col.cpu())
+        for k in ("g_means", "g_quat", "g_shape", "g_amp", "g_dc"):
+            assert torch.equal(out[k], g[k].cpu()), k
+    inp = W.make(3, 2 * 131072 + 777)
+    d = to_dev(inp, SH_KEYS)
+    col, g = run_sh(B, d)
+    host = {k: torch.from_numpy(np.ascontiguousarray(inp[k])).pin_memory() for k in SH_KEYS}
+    N, C = inp["N"], inp["C"]
+    out = dict(colors=torch.empty((C, N, 3)).pin_memory(), g_means=torch.empty((N, 3)).pin_memory(),
+               g_coeffs=torch.empty((16, 3, N)).pin_memory())
+    scratch = torch.empty(B.sh_host_scratch_bytes(N, C), dtype=torch.uint8, device="cuda")
+    B.sh_eval_fwd_bwd_host(host, out, scratch)
+    torch.cuda.synchronize()
+    assert torch.equal(out["colors"], col.cpu()) and torch.equal(out["g_coeffs"], g["g_coeffs"].cpu())
+    assert torch.equal(out["g_means"], g["g_means"].cpu())
+
+
 def test_runs_on_a_side_stream_and_in_a_cuda_graph(B, W):
     inp = W.make(1, 40_000)
     d = to_dev(inp, NASG_KEYS)
