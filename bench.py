@@ -49,6 +49,16 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
+def alu_floor_ms(workload: str, N: int, sms: int, sm_hz: float):
+    """Issue-side floor of the dominant kernel from the committed ncu counts (None if not recorded)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            cyc = json.load(f).get("alu_cycles_per_warp_gaussian_bwd", {}).get(workload)
+        return None if cyc is None else 1e3 * (N / 32.0) * cyc / (sms * 4 * sm_hz)
+    except Exception:
+        return None
+
+
 def recorded_traffic(workload: str):
     """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture."""
     try:
@@ -280,6 +290,11 @@ def run_ours(args, W, cfg):
                     "api": "sh_eval_fwd_bwd_host" if cfg.kind == "sh" else "nasg_eval_fwd_bwd_host"},
             "gpu_launches": int(launches),
         }
+        props = torch.cuda.get_device_properties(local)
+        alu_ms = alu_floor_ms(cfg.name, N, props.multi_processor_count, 1.965e9)
+        if alu_ms is not None:      # C = 4: the kernel is FP32-pipe/issue-bound, not HBM-bound
+            line["roofline"]["alu"] = {"floor_ms": alu_ms, "frac": alu_ms / bwd_ms,
+                                       "note": "warp-instruction issue floor at 1965 MHz from the committed ncu counts"}
         if not args.no_cpu and world == 1:
             line["cpu_baseline"] = cpu_baseline(W, cfg)
         print(json.dumps(line), flush=True)

@@ -41,44 +41,6 @@ __host__ __device__ constexpr size_t pipe_smem_bytes(int HR, int HF)
 // the packed kernels stage the visibility bytes of a Gaussian next to its header: [HR][4][PBLOCK] bytes
 __host__ __device__ constexpr size_t pipe2_smem_bytes(int HR, int HF) { return pipe_smem_bytes(HR, HF) + (size_t)HR * 4 * PBLOCK; }
 
-// Visibility mask of the packed kernels. A byte load from global memory that is consumed in the same
-// iteration stalls the warp for a DRAM latency (ncu: 11% of all stall samples sat on it), and the compiler
-// places the consumer wherever it likes. When vis rows are 4-byte aligned (N % 4 == 0) every fourth lane
-// copies the 4 bytes of its quad with cp.async into the header slot instead, SH_DIST-style ahead of use;
-// the bytes are read back from shared memory after the wait + __syncwarp. Otherwise (vis == NULL or an
-// unaligned N) the raw bytes are loaded one Gaussian ahead into registers.
-struct RawMask { unsigned b[4]; };
-__device__ __forceinline__ RawMask load_raw_mask(const uint8_t *vis, int64_t N, int64_t n, int C)
-{
-    RawMask m;
-#pragma unroll
-    for (int c = 0; c < 4; ++c) m.b[c] = (n < N) ? ((c < C) ? (vis ? vis[(int64_t)c * N + n] : 1u) : 0u) : 0u;
-    return m;
-}
-__device__ __forceinline__ unsigned combine_mask(const RawMask &m)
-{
-    return (m.b[0] ? 1u : 0u) | (m.b[1] ? 2u : 0u) | (m.b[2] ? 4u : 0u) | (m.b[3] ? 8u : 0u);
-}
-__device__ __forceinline__ bool vis_rows_aligned(const uint8_t *vis, int64_t N)
-{
-    return vis != nullptr && (N & 3) == 0 && (reinterpret_cast<uintptr_t>(vis) & 3u) == 0;
-}
-__device__ __forceinline__ void prefetch_vis(unsigned char *vm, int hslot, int tid, const uint8_t *vis, int64_t N, int64_t gn, int C)
-{
-    if ((tid & 3) == 0) {
-#pragma unroll
-        for (int c = 0; c < 4; ++c)
-            if (c < C) cp_async4(vm + (hslot * 4 + c) * PBLOCK + tid, vis + (int64_t)c * N + gn);
-    }
-}
-__device__ __forceinline__ unsigned staged_mask(const unsigned char *vm, int hslot, int tid, int C, bool valid)
-{
-    unsigned m = 0;
-#pragma unroll
-    for (int c = 0; c < 4; ++c)
-        if (c < C) m |= (vm[(hslot * 4 + c) * PBLOCK + tid] != 0 ? 1u : 0u) << c;
-    return valid ? m : 0u;
-}
 __device__ __forceinline__ Ring carve(unsigned char *raw)
 {
     Ring r;

@@ -40,6 +40,44 @@ __device__ __forceinline__ unsigned load_mask(const uint8_t *vis, int64_t N, int
     return m;
 }
 
+// Visibility mask staging (packed NASGabor kernels, SH kernels). A byte load from global memory that is consumed in the same
+// iteration stalls the warp for a DRAM latency (ncu: 11% of all stall samples sat on it), and the compiler
+// places the consumer wherever it likes. When vis rows are 4-byte aligned (N % 4 == 0) every fourth lane
+// copies the 4 bytes of its quad with cp.async into the header slot instead, a few items ahead of use;
+// the bytes are read back from shared memory after the wait + __syncwarp. Otherwise (vis == NULL or an
+// unaligned N) the raw bytes are loaded one Gaussian ahead into registers.
+struct RawMask { unsigned b[4]; };
+__device__ __forceinline__ RawMask load_raw_mask(const uint8_t *vis, int64_t N, int64_t n, int C)
+{
+    RawMask m;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) m.b[c] = (n < N) ? ((c < C) ? (vis ? vis[(int64_t)c * N + n] : 1u) : 0u) : 0u;
+    return m;
+}
+__device__ __forceinline__ unsigned combine_mask(const RawMask &m)
+{
+    return (m.b[0] ? 1u : 0u) | (m.b[1] ? 2u : 0u) | (m.b[2] ? 4u : 0u) | (m.b[3] ? 8u : 0u);
+}
+__device__ __forceinline__ bool vis_rows_aligned(const uint8_t *vis, int64_t N)
+{
+    return vis != nullptr && (N & 3) == 0 && (reinterpret_cast<uintptr_t>(vis) & 3u) == 0;
+}
+__device__ __forceinline__ void prefetch_vis(unsigned char *vm, int hslot, int tid, const uint8_t *vis, int64_t N, int64_t gn, int C)
+{
+    if ((tid & 3) == 0) {
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+            if (c < C) cp_async4(vm + (hslot * 4 + c) * PBLOCK + tid, vis + (int64_t)c * N + gn);
+    }
+}
+__device__ __forceinline__ unsigned staged_mask(const unsigned char *vm, int hslot, int tid, int C, bool valid)
+{
+    unsigned m = 0;
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+        if (c < C) m |= (vm[(hslot * 4 + c) * PBLOCK + tid] != 0 ? 1u : 0u) << c;
+    return valid ? m : 0u;
+}
 // Resident-grid size of a persistent kernel; the occupancy query and the shared-memory opt-in are done
 // once per (kernel instantiation, device) and cached (benign, idempotent state).
 template <typename Kernel>

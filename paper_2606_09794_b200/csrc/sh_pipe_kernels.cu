@@ -1,12 +1,22 @@
 // sh_pipe_kernels.cu — fast path of the SH degree-3 comparison kernels for C <= 4 cameras (sm_100a),
 // built the same way as the NASGabor fast path (nasg_pipe_kernels.cu): persistent threads, one thread per
-// Gaussian, parameters streamed through a private shared-memory ring filled by cp.async (LDGSTS)
-// SH_DIST items ahead of use, gradients written once with streaming stores, no atomics.
+// Gaussian, parameters streamed through a shared-memory ring filled by cp.async (LDGSTS) ahead of use,
+// gradients written once with streaming stores, no atomics.
 //
-// Item stream of a thread: (Gaussian i, group g), g = 0..3; group g holds the 4 basis functions
-// j = 4g..4g+3, i.e. 12 planar coefficient rows = 48 B per Gaussian (a NASGabor lobe is 44 B), and always
-// lives in ring slot g. The per-Gaussian header (mean, and g_colors in the backward) travels with
-// group 0 into header slot i % 2. A thread only reads slots it filled itself: no block barrier.
+// Item stream: (Gaussian i, group g), g = 0..3; group g holds the 4 basis functions j = 4g..4g+3, i.e.
+// 12 planar coefficient rows = 48 B per Gaussian (a NASGabor lobe is 44 B), and always lives in ring
+// slot g. The per-Gaussian header (mean, g_colors in the backward, visibility bytes) travels with
+// group 0 into header slot i % 2.
+//
+// The SH path has almost no arithmetic, so the load/store unit is what limits it (ncu: mio_throttle):
+// 51 four-byte LDGSTS per Gaussian and thread. When the rows are 16-byte aligned (N % 4 == 0, aligned
+// base pointers) the four lanes of a quad therefore share the work: lane j copies rows j, j+4, j+8 of
+// the group for all four Gaussians of the quad with ONE 16-byte LDGSTS each (4x fewer copy
+// instructions), and the [N,3] mean / g_colors records of the quad (48 contiguous bytes) with three
+// 16-byte copies. Data is then read by a lane that did not copy it, so every step is:
+// wait (own copies of the item landed) -> __syncwarp (quad's copies visible; everyone is done with the
+// slot about to be refilled) -> prefetch -> compute. The loop has a warp-uniform trip count for this.
+// Otherwise every thread copies its own 4-byte elements (same loop).
 #include "nasg_internal.h"
 #include "pipe_common.cuh"
 #include "sh_math.cuh"
@@ -17,18 +27,43 @@ constexpr int SH_GROUPS = 4;    // groups of 4 basis functions
 constexpr int SH_DIST = 3;      // prefetch distance in groups
 constexpr int SH_HR = 2;        // header slots
 
+// ring [4][12][PBLOCK] floats, header [SH_HR][HF][PBLOCK] floats, visibility bytes [SH_HR][4][PBLOCK]
 __host__ __device__ constexpr size_t sh_pipe_smem_bytes(int HF)
 {
-    return (size_t)PBLOCK * 4 * (SH_GROUPS * 12 + SH_HR * HF);
+    return (size_t)PBLOCK * 4 * (SH_GROUPS * 12 + SH_HR * HF) + (size_t)SH_HR * 4 * PBLOCK;
 }
+static inline bool ptr_aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
-// copies of one group item: rows (4g+jj)*3+ch, jj < 4, ch < 3
-__device__ __forceinline__ void sh_prefetch_group(float *ring, int tid, const float *coeffs, int64_t N, int64_t n, int g)
+// copies of one group item: rows 12g + r, r < 12
+__device__ __forceinline__ void sh_prefetch_group(float *ring, int tid, bool coop, const float *coeffs, int64_t N, int64_t n, int g)
 {
-    const float *src = coeffs + (int64_t)g * 12 * N + n;
-    float *dst = ring + g * 12 * PBLOCK + tid;
+    if (coop) {
+        const int j = tid & 3, q0 = tid & ~3;
+        const float *src = coeffs + ((int64_t)g * 12 + j) * N + (n - j);
+        float *dst = ring + (g * 12 + j) * PBLOCK + q0;
 #pragma unroll
-    for (int r = 0; r < 12; ++r) cp_async4(dst + r * PBLOCK, src + (int64_t)r * N);
+        for (int r = 0; r < 3; ++r) cp_async16(dst + 4 * r * PBLOCK, src + (int64_t)4 * r * N);
+    } else {
+        const float *src = coeffs + (int64_t)g * 12 * N + n;
+        float *dst = ring + g * 12 * PBLOCK + tid;
+#pragma unroll
+        for (int r = 0; r < 12; ++r) cp_async4(dst + r * PBLOCK, src + (int64_t)r * N);
+    }
+}
+// a [N,3] record of the quad (mean or one camera's g_colors) into a 3*PBLOCK-float header area:
+// cooperative: the tile's records stay interleaved (thread t reads h[3t+i]); else planar (h[i*PBLOCK+t])
+__device__ __forceinline__ void sh_prefetch_rec3(float *area, int tid, bool coop, const float *src3 /* record of Gaussian n */)
+{
+    if (coop) {
+        const int j = tid & 3;
+        if (j < 3) cp_async16(area + 3 * (tid & ~3) + 4 * j, src3 - 3 * j + 4 * j);     // record base of the quad + 4j floats
+    } else {
+        cp_async4(area + tid, src3); cp_async4(area + PBLOCK + tid, src3 + 1); cp_async4(area + 2 * PBLOCK + tid, src3 + 2);
+    }
+}
+__device__ __forceinline__ float sh_rec3(const float *area, int tid, bool coop, int i)
+{
+    return coop ? area[3 * tid + i] : area[i * PBLOCK + tid];
 }
 
 template <int CT>
@@ -66,24 +101,26 @@ __device__ __forceinline__ void sh_fwd_group(const float *slot, const float (&dx
     }
 }
 
-template <int CT>
+template <int CT, bool COOP>
 __global__ void __launch_bounds__(PBLOCK, 4) sh_fwd_pipe_kernel(ShParams p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int HF = 3;
     float *ring = reinterpret_cast<float *>(smem_raw);
     float *hdr = ring + SH_GROUPS * 12 * PBLOCK;
+    unsigned char *vm = reinterpret_cast<unsigned char *>(hdr + SH_HR * HF * PBLOCK);
     const int tid = threadIdx.x;
     const int64_t N = p.N, stride = (int64_t)gridDim.x * PBLOCK;
     int64_t n = (int64_t)blockIdx.x * PBLOCK + tid;
+    constexpr bool coop = COOP;      // rows 16-byte aligned (checked by the launcher)
+    const bool vis_cp = vis_rows_aligned(p.vis, N);
 
     auto prefetch_item = [&](int64_t gn, int g, int hslot) {
         if (gn < N) {
-            sh_prefetch_group(ring, tid, p.coeffs, N, gn, g);
+            sh_prefetch_group(ring, tid, coop, p.coeffs, N, gn, g);
             if (g == 0) {
-                float *h = hdr + hslot * HF * PBLOCK + tid;
-                cp_async4(h, p.means + 3 * gn); cp_async4(h + PBLOCK, p.means + 3 * gn + 1);
-                cp_async4(h + 2 * PBLOCK, p.means + 3 * gn + 2);
+                sh_prefetch_rec3(hdr + hslot * HF * PBLOCK, tid, coop, p.means + 3 * gn);
+                if (vis_cp) prefetch_vis(vm, hslot, tid, p.vis, N, gn, p.C);
             }
         }
         cp_async_commit();
@@ -92,17 +129,24 @@ __global__ void __launch_bounds__(PBLOCK, 4) sh_fwd_pipe_kernel(ShParams p)
     for (int j = 0; j < SH_DIST; ++j) prefetch_item(n, j, 0);
 
     unsigned hs = 0;
-    unsigned mask = load_mask(p.vis, N, n, p.C);
-    for (; n < N; n += stride) {
-        const unsigned mask_next = load_mask(p.vis, N, n + stride, p.C);
+    RawMask raw = {{0u, 0u, 0u, 0u}};
+    if (!vis_cp) raw = load_raw_mask(p.vis, N, n, p.C);
+    for (; n - (tid & 31) < N; n += stride) {       // warp-uniform trip count: lanes past N idle (mask 0, no stores)
+        const bool valid = n < N;
+        RawMask raw_next = {{0u, 0u, 0u, 0u}};
+        if (!vis_cp) raw_next = load_raw_mask(p.vis, N, n + stride, p.C);
+        unsigned mask = 0;
         float dx[CT], dy[CT], dz[CT], idist[CT], col[CT][3];
 #pragma unroll
         for (int g = 0; g < SH_GROUPS; ++g) {
+            cp_async_wait<SH_DIST - 1>();       // item g (own copies) landed
+            __syncwarp();                       // ... and the quad's; slot (g+3)%4 is free in every lane
             prefetch_item(n + ((g + SH_DIST) / SH_GROUPS) * stride, (g + SH_DIST) % SH_GROUPS, (hs + (g + SH_DIST) / SH_GROUPS) % SH_HR);
-            cp_async_wait<SH_DIST>();
             if (g == 0) {
-                const float *h = hdr + hs * HF * PBLOCK + tid;
-                sh_directions<CT>(p.campos, p.C, h[0], h[PBLOCK], h[2 * PBLOCK], dx, dy, dz, idist);
+                mask = vis_cp ? staged_mask(vm, hs, tid, p.C, valid) : combine_mask(raw);
+                const float *h = hdr + hs * HF * PBLOCK;
+                sh_directions<CT>(p.campos, p.C, sh_rec3(h, tid, coop, 0), sh_rec3(h, tid, coop, 1), sh_rec3(h, tid, coop, 2),
+                                  dx, dy, dz, idist);
 #pragma unroll
                 for (int t = 0; t < CT; ++t) col[t][0] = col[t][1] = col[t][2] = 0.f;
             }
@@ -116,21 +160,21 @@ __global__ void __launch_bounds__(PBLOCK, 4) sh_fwd_pipe_kernel(ShParams p)
         }
 #pragma unroll
         for (int t = 0; t < CT; ++t) {
-            if (t < p.C) {
+            if (t < p.C && valid) {
                 const bool on = mask & (1u << t);
                 float *o = p.colors + ((int64_t)t * N + n) * 3;
                 st_cs(o, on ? col[t][0] : 0.f); st_cs(o + 1, on ? col[t][1] : 0.f); st_cs(o + 2, on ? col[t][2] : 0.f);
             }
         }
         hs = (hs + 1) % SH_HR;
-        mask = mask_next;
+        raw = raw_next;
     }
     cp_async_wait<0>();
 }
 
 // ---- backward: g_coeffs[j,:,n] = sum_c Y_j(d_c) g_col_c;  g_d = sum_j grad Y_j (coeff_j . g_col) ----
 template <int G, int CT>
-__device__ __forceinline__ void sh_bwd_group(const float *slot, bool live, float *g_coeffs, int64_t N, int64_t n,
+__device__ __forceinline__ void sh_bwd_group(const float *slot, bool live, bool valid, float *g_coeffs, int64_t N, int64_t n,
                                              const float (&dx)[CT], const float (&dy)[CT], const float (&dz)[CT],
                                              const float (&gc)[CT][3], float (&gd)[CT][3])
 {
@@ -151,40 +195,38 @@ __device__ __forceinline__ void sh_bwd_group(const float *slot, bool live, float
                 gd[t][0] = fmaf(s, gx, gd[t][0]); gd[t][1] = fmaf(s, gy, gd[t][1]); gd[t][2] = fmaf(s, gz, gd[t][2]);
             }
         }
-        if (g_coeffs) {
+        if (g_coeffs && valid) {
             float *o = g_coeffs + (int64_t)((4 * G + jj) * 3) * N + n;
             st_cs(o, a0); st_cs(o + N, a1); st_cs(o + 2 * N, a2);
         }
     }
 }
 
-template <int CT>
+template <int CT, bool COOP>
 __global__ void __launch_bounds__(PBLOCK, 2) sh_bwd_pipe_kernel(ShParams p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int HF = 3 + 3 * CT;
     float *ring = reinterpret_cast<float *>(smem_raw);
     float *hdr = ring + SH_GROUPS * 12 * PBLOCK;
+    unsigned char *vm = reinterpret_cast<unsigned char *>(hdr + SH_HR * HF * PBLOCK);
     const int tid = threadIdx.x;
     const int C = p.C;
     const int64_t N = p.N, stride = (int64_t)gridDim.x * PBLOCK;
     int64_t n = (int64_t)blockIdx.x * PBLOCK + tid;
+    constexpr bool coop = COOP;      // rows 16-byte aligned (checked by the launcher)
+    const bool vis_cp = vis_rows_aligned(p.vis, N);
 
     auto prefetch_item = [&](int64_t gn, int g, int hslot) {
         if (gn < N) {
-            sh_prefetch_group(ring, tid, p.coeffs, N, gn, g);
+            sh_prefetch_group(ring, tid, coop, p.coeffs, N, gn, g);
             if (g == 0) {
-                float *h = hdr + hslot * HF * PBLOCK + tid;
-                cp_async4(h, p.means + 3 * gn); cp_async4(h + PBLOCK, p.means + 3 * gn + 1);
-                cp_async4(h + 2 * PBLOCK, p.means + 3 * gn + 2);
+                float *h = hdr + hslot * HF * PBLOCK;
+                sh_prefetch_rec3(h, tid, coop, p.means + 3 * gn);
 #pragma unroll
-                for (int t = 0; t < CT; ++t) {
-                    if (t < C) {
-                        const float *g3 = p.g_colors + ((int64_t)t * N + gn) * 3;
-                        cp_async4(h + (3 + 3 * t) * PBLOCK, g3); cp_async4(h + (4 + 3 * t) * PBLOCK, g3 + 1);
-                        cp_async4(h + (5 + 3 * t) * PBLOCK, g3 + 2);
-                    }
-                }
+                for (int t = 0; t < CT; ++t)
+                    if (t < C) sh_prefetch_rec3(h + (3 + 3 * t) * PBLOCK, tid, coop, p.g_colors + ((int64_t)t * N + gn) * 3);
+                if (vis_cp) prefetch_vis(vm, hslot, tid, p.vis, N, gn, C);
             }
         }
         cp_async_commit();
@@ -193,35 +235,43 @@ __global__ void __launch_bounds__(PBLOCK, 2) sh_bwd_pipe_kernel(ShParams p)
     for (int j = 0; j < SH_DIST; ++j) prefetch_item(n, j, 0);
 
     unsigned hs = 0;
-    unsigned mask = load_mask(p.vis, N, n, C);
-    for (; n < N; n += stride) {
-        const unsigned mask_next = load_mask(p.vis, N, n + stride, C);
+    RawMask raw = {{0u, 0u, 0u, 0u}};
+    if (!vis_cp) raw = load_raw_mask(p.vis, N, n, C);
+    for (; n - (tid & 31) < N; n += stride) {
+        const bool valid = n < N;
+        RawMask raw_next = {{0u, 0u, 0u, 0u}};
+        if (!vis_cp) raw_next = load_raw_mask(p.vis, N, n + stride, C);
+        unsigned mask = 0;
         float dx[CT], dy[CT], dz[CT], idist[CT], gc[CT][3], gd[CT][3];
 #pragma unroll
         for (int g = 0; g < SH_GROUPS; ++g) {
+            cp_async_wait<SH_DIST - 1>();
+            __syncwarp();
             prefetch_item(n + ((g + SH_DIST) / SH_GROUPS) * stride, (g + SH_DIST) % SH_GROUPS, (hs + (g + SH_DIST) / SH_GROUPS) % SH_HR);
-            cp_async_wait<SH_DIST>();
             if (g == 0) {
-                const float *h = hdr + hs * HF * PBLOCK + tid;
-                sh_directions<CT>(p.campos, C, h[0], h[PBLOCK], h[2 * PBLOCK], dx, dy, dz, idist);
+                mask = vis_cp ? staged_mask(vm, hs, tid, C, valid) : combine_mask(raw);
+                const float *h = hdr + hs * HF * PBLOCK;
+                sh_directions<CT>(p.campos, C, sh_rec3(h, tid, coop, 0), sh_rec3(h, tid, coop, 1), sh_rec3(h, tid, coop, 2),
+                                  dx, dy, dz, idist);
 #pragma unroll
                 for (int t = 0; t < CT; ++t) {
                     const bool on = mask & (1u << t);
-                    gc[t][0] = on ? h[(3 + 3 * t) * PBLOCK] : 0.f;
-                    gc[t][1] = on ? h[(4 + 3 * t) * PBLOCK] : 0.f;
-                    gc[t][2] = on ? h[(5 + 3 * t) * PBLOCK] : 0.f;
+                    const float *hg = h + (3 + 3 * t) * PBLOCK;
+                    gc[t][0] = on ? sh_rec3(hg, tid, coop, 0) : 0.f;
+                    gc[t][1] = on ? sh_rec3(hg, tid, coop, 1) : 0.f;
+                    gc[t][2] = on ? sh_rec3(hg, tid, coop, 2) : 0.f;
                     idist[t] = on ? idist[t] : 0.f;
                     gd[t][0] = gd[t][1] = gd[t][2] = 0.f;
                 }
             }
             const float *slot = ring + g * 12 * PBLOCK + tid;
             const bool live = mask != 0;
-            if (g == 0) sh_bwd_group<0, CT>(slot, live, p.g_coeffs, N, n, dx, dy, dz, gc, gd);
-            if (g == 1) sh_bwd_group<1, CT>(slot, live, p.g_coeffs, N, n, dx, dy, dz, gc, gd);
-            if (g == 2) sh_bwd_group<2, CT>(slot, live, p.g_coeffs, N, n, dx, dy, dz, gc, gd);
-            if (g == 3) sh_bwd_group<3, CT>(slot, live, p.g_coeffs, N, n, dx, dy, dz, gc, gd);
+            if (g == 0) sh_bwd_group<0, CT>(slot, live, valid, p.g_coeffs, N, n, dx, dy, dz, gc, gd);
+            if (g == 1) sh_bwd_group<1, CT>(slot, live, valid, p.g_coeffs, N, n, dx, dy, dz, gc, gd);
+            if (g == 2) sh_bwd_group<2, CT>(slot, live, valid, p.g_coeffs, N, n, dx, dy, dz, gc, gd);
+            if (g == 3) sh_bwd_group<3, CT>(slot, live, valid, p.g_coeffs, N, n, dx, dy, dz, gc, gd);
         }
-        if (p.g_means) {        // through d = Delta/|Delta|: (I - d d^T)/|Delta|
+        if (p.g_means && valid) {        // through d = Delta/|Delta|: (I - d d^T)/|Delta|
             float gm0 = 0.f, gm1 = 0.f, gm2 = 0.f;
 #pragma unroll
             for (int t = 0; t < CT; ++t) {
@@ -234,7 +284,7 @@ __global__ void __launch_bounds__(PBLOCK, 2) sh_bwd_pipe_kernel(ShParams p)
             st_cs(o, gm0); st_cs(o + 1, gm1); st_cs(o + 2, gm2);
         }
         hs = (hs + 1) % SH_HR;
-        mask = mask_next;
+        raw = raw_next;
     }
     cp_async_wait<0>();
 }
@@ -244,8 +294,10 @@ template <int CT>
 static cudaError_t launch_sh_fwd_pipe_c(const ShParams &p, cudaStream_t st)
 {
     constexpr size_t smem = sh_pipe_smem_bytes(3);
-    static int cache[64] = {0};
-    sh_fwd_pipe_kernel<CT><<<pipe_grid(sh_fwd_pipe_kernel<CT>, smem, p.N, cache), PBLOCK, smem, st>>>(p);
+    static int cache[2][64] = {{0}};
+    const bool coop = (p.N & 3) == 0 && ptr_aligned16(p.coeffs) && ptr_aligned16(p.means);
+    if (coop) sh_fwd_pipe_kernel<CT, true><<<pipe_grid(sh_fwd_pipe_kernel<CT, true>, smem, p.N, cache[1]), PBLOCK, smem, st>>>(p);
+    else sh_fwd_pipe_kernel<CT, false><<<pipe_grid(sh_fwd_pipe_kernel<CT, false>, smem, p.N, cache[0]), PBLOCK, smem, st>>>(p);
     return cudaGetLastError();
 }
 cudaError_t launch_sh_fwd_pipe(const ShParams &p, cudaStream_t st)
@@ -262,8 +314,10 @@ template <int CT>
 static cudaError_t launch_sh_bwd_pipe_c(const ShParams &p, cudaStream_t st)
 {
     constexpr size_t smem = sh_pipe_smem_bytes(3 + 3 * CT);
-    static int cache[64] = {0};
-    sh_bwd_pipe_kernel<CT><<<pipe_grid(sh_bwd_pipe_kernel<CT>, smem, p.N, cache), PBLOCK, smem, st>>>(p);
+    static int cache[2][64] = {{0}};
+    const bool coop = (p.N & 3) == 0 && ptr_aligned16(p.coeffs) && ptr_aligned16(p.means) && ptr_aligned16(p.g_colors);
+    if (coop) sh_bwd_pipe_kernel<CT, true><<<pipe_grid(sh_bwd_pipe_kernel<CT, true>, smem, p.N, cache[1]), PBLOCK, smem, st>>>(p);
+    else sh_bwd_pipe_kernel<CT, false><<<pipe_grid(sh_bwd_pipe_kernel<CT, false>, smem, p.N, cache[0]), PBLOCK, smem, st>>>(p);
     return cudaGetLastError();
 }
 cudaError_t launch_sh_bwd_pipe(const ShParams &p, cudaStream_t st)
