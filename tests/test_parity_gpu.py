@@ -39,7 +39,7 @@ def test_sh_config_small(B, W, oracle):
 
 
 @pytest.mark.parametrize("K", [1, 2, 3, 4, 5, 8])
-@pytest.mark.parametrize("C", [1, 3, 4, 5, 9])
+@pytest.mark.parametrize("C", [1, 2, 3, 4, 5, 9])
 def test_all_lobe_counts_and_camera_tiles(B, W, oracle, K, C):
     """Every compiled K, and camera counts that exercise the C==1 path, a partial tile, a full tile and
     the multi-tile read-modify-write path (C > 4)."""
@@ -48,7 +48,7 @@ def test_all_lobe_counts_and_camera_tiles(B, W, oracle, K, C):
     check_nasg(B, oracle, inp, 1, want_campos=True, label=f"K={K} C={C}")
 
 
-@pytest.mark.parametrize("C", [1, 2, 6])
+@pytest.mark.parametrize("C", [1, 2, 3, 4, 6])
 def test_sh_camera_tiles(B, W, oracle, C):
     cfg = dataclasses.replace(W.CONFIGS[3], seed=70 + C, C=C)
     inp = W.make_sh(cfg, N=3_011)
@@ -176,6 +176,34 @@ def test_unnormalised_quaternions(B, W, oracle):
     inp = W.make(1, 5_000)
     scale = np.random.default_rng(3).uniform(0.1, 10.0, size=inp["quat"].shape[:2] + (1,)).astype(np.float32)
     check_nasg(B, oracle, dict(inp, quat=inp["quat"] * scale), 1, label="unnormalised q")
+
+
+@pytest.mark.parametrize("N", [4096, 8200])
+def test_aligned_and_misaligned_row_pointers(B, W, oracle, N):
+    """N % 4 == 0 takes the cooperative 16-byte copies / cp.async-staged mask; views that start 1 element
+    into a larger allocation break the 16-byte (4-byte for vis) alignment and must take the fallback."""
+    inp = W.make(2, N)
+    rc, rg = oracle.nasg_fwd(inp, 1), oracle.nasg_bwd(inp, 1)
+    d = to_dev(inp, NASG_KEYS)
+
+    def shifted(t):                       # same values, storage offset by one element
+        buf = torch.empty(t.numel() + 1, dtype=t.dtype, device=t.device)
+        buf[1:] = t.reshape(-1)
+        return buf[1:].view(t.shape)
+    for label, dd in (("aligned", d), ("vis+means shifted", dict(d, vis=shifted(d["vis"]), means=shifted(d["means"]),
+                                                                   g_colors=shifted(d["g_colors"])))):
+        col, g = run_nasg(B, dd, 1)
+        assert rel_err(col, rc) <= FWD_TOL, label
+        for k in ("g_means", "g_quat", "g_shape", "g_amp", "g_dc"):
+            assert rel_err(g[k], rg[k]) <= BWD_TOL, (label, k)
+    inp = W.make(3, N)
+    rc, rg = oracle.sh_fwd(inp), oracle.sh_bwd(inp)
+    d = to_dev(inp, SH_KEYS)
+    for label, dd in (("aligned", d), ("shifted", dict(d, vis=shifted(d["vis"]), means=shifted(d["means"]),
+                                                        coeffs=shifted(d["coeffs"]), g_colors=shifted(d["g_colors"])))):
+        col, g = run_sh(B, dd)
+        assert rel_err(col, rc) <= FWD_TOL, label
+        assert rel_err(g["g_means"], rg["g_means"]) <= BWD_TOL and rel_err(g["g_coeffs"], rg["g_coeffs"]) <= BWD_TOL, label
 
 
 def test_host_entry_point_matches_device_path(B, W):
