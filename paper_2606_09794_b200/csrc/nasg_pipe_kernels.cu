@@ -23,7 +23,7 @@ constexpr int RING = 4;     // lobe slots per thread
 constexpr int DIST = 3;     // prefetch distance in lobes
 
 template <int K> struct PipeCfg {
-    static constexpr int HR = (K <= 2) ? 4 : 2;          // header slots: ceil(DIST/K)+1 rounded to a power of 2
+    static constexpr int HR = (K == 1) ? 4 : (K == 2) ? 3 : 2;   // header slots: Gaussians spanned by DIST lobes ahead, + 1
     static constexpr bool STATIC_SLOTS = (K % RING) == 0; // lobe l always lives in ring slot l % RING
 };
 
@@ -450,7 +450,10 @@ __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(
         unsigned mask = 0;
         // camera slots in pairs (x = slot 2j, y = slot 2j+1). A culled or padding slot gets an exponent bias of
         // -1e30: its lobe value and with it every gradient contribution is exactly 0.
-        float2 dx[NP], dy[NP], dz[NP], idist[NP], bias[NP], gd[NP][3];
+        float2 dx[NP], dy[NP], dz[NP], gd[NP][3];
+        // per-thread scratch behind the staged visibility bytes: 1/|Delta| per camera is parked here instead of
+        // in registers until the end of the Gaussian (parking the directions too costs more than it frees)
+        float *hi = reinterpret_cast<float *>(vm + HR * 4 * PBLOCK) + tid;
         const float *h = r.h + (hs * HF) * PBLOCK + tid;                        // header of this Gaussian (valid after lobe 0 landed)
 #pragma unroll 1
         for (int l = 0; l < K; ++l) {
@@ -473,8 +476,7 @@ __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(
                     float2 inv = make_float2(f_rsqrt(r2.x), f_rsqrt(r2.y));
                     inv = mul2(inv, fma2(mul2(splat(-0.5f), r2), mul2(inv, inv), splat(1.5f)));
                     dx[j] = mul2(ex, inv); dy[j] = mul2(ey, inv); dz[j] = mul2(ez, inv);
-                    idist[j] = inv;
-                    bias[j] = make_float2(on0 ? 0.f : -1e30f, on1 ? 0.f : -1e30f);
+                    hi[t0 * PBLOCK] = inv.x; hi[t1 * PBLOCK] = inv.y;
                     if (on0) { gdc0 += h[(3 + 3 * t0) * PBLOCK]; gdc1 += h[(4 + 3 * t0) * PBLOCK]; gdc2 += h[(5 + 3 * t0) * PBLOCK]; }
                     if (t1 < CT && on1) { gdc0 += h[(3 + 3 * t1) * PBLOCK]; gdc1 += h[(4 + 3 * t1) * PBLOCK]; gdc2 += h[(5 + 3 * t1) * PBLOCK]; }
                     gd[j][0] = gd[j][1] = gd[j][2] = splat(0.f);
@@ -502,8 +504,11 @@ __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(
                     const float2 gc0 = make_float2(h[(3 + 3 * t0) * PBLOCK], h[(3 + 3 * t1) * PBLOCK]);     // g_colors of the pair
                     const float2 gc1 = make_float2(h[(4 + 3 * t0) * PBLOCK], h[(4 + 3 * t1) * PBLOCK]);
                     const float2 gc2 = make_float2(h[(5 + 3 * t0) * PBLOCK], h[(5 + 3 * t1) * PBLOCK]);
+                    const float2 dxj = dx[j], dyj = dy[j], dzj = dz[j];
                     EvalTerms2 T;
-                    const float2 G = lobe_eval2<true>(L, dx[j], dy[j], dz[j], bias[j], T);
+                    const float2 bias = make_float2((mask & (1u << t0)) ? 0.f : -1e30f,
+                                                    (2 * j + 1 < CT && (mask & (1u << t1))) ? 0.f : -1e30f);   // (re-derived: 4 fewer live registers)
+                    const float2 G = lobe_eval2<true>(L, dxj, dyj, dzj, bias, T);
                     const float2 gG = fma2(gc0, w0, fma2(gc1, w1, mul2(gc2, w2)));                      // dL/dG, eq.(6)
                     pw0 = fma2(gc0, G, pw0); pw1 = fma2(gc1, G, pw1); pw2 = fma2(gc2, G, pw2);
                     const float2 gGG = mul2(gG, G);
@@ -518,8 +523,8 @@ __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(
                     S2 = fma2(B1, T.uu, S2);
                     Sk = fma2(hs_, T.u, Sk);
                     Sp = add2(Sp, hs_);
-                    gX0 = fma2(gu, dx[j], gX0); gX1 = fma2(gu, dy[j], gX1); gX2 = fma2(gu, dz[j], gX2);
-                    gZ0 = fma2(gv, dx[j], gZ0); gZ1 = fma2(gv, dy[j], gZ1); gZ2 = fma2(gv, dz[j], gZ2);
+                    gX0 = fma2(gu, dxj, gX0); gX1 = fma2(gu, dyj, gX1); gX2 = fma2(gu, dzj, gX2);
+                    gZ0 = fma2(gv, dxj, gZ0); gZ1 = fma2(gv, dyj, gZ1); gZ2 = fma2(gv, dzj, gZ2);
                     gd[j][0] = fma2(gu, splat(L.Xx), fma2(gv, splat(L.Zx), gd[j][0]));
                     gd[j][1] = fma2(gu, splat(L.Xy), fma2(gv, splat(L.Zy), gd[j][1]));
                     gd[j][2] = fma2(gu, splat(L.Xz), fma2(gv, splat(L.Zz), gd[j][2]));
@@ -556,10 +561,12 @@ __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(
             float2 gm0 = splat(0.f), gm1 = splat(0.f), gm2 = splat(0.f);
 #pragma unroll
             for (int j = 0; j < NP; ++j) {
-                const float2 dg = fma2(dx[j], gd[j][0], fma2(dy[j], gd[j][1], mul2(dz[j], gd[j][2])));
-                gm0 = fma2(sub2(gd[j][0], mul2(dx[j], dg)), idist[j], gm0);
-                gm1 = fma2(sub2(gd[j][1], mul2(dy[j], dg)), idist[j], gm1);
-                gm2 = fma2(sub2(gd[j][2], mul2(dz[j], dg)), idist[j], gm2);
+                const float2 dxj = dx[j], dyj = dy[j], dzj = dz[j];
+                const float2 dg = fma2(dxj, gd[j][0], fma2(dyj, gd[j][1], mul2(dzj, gd[j][2])));
+                const float2 idist = make_float2(hi[(2 * j) * PBLOCK], hi[(2 * j + 1) * PBLOCK]);
+                gm0 = fma2(sub2(gd[j][0], mul2(dxj, dg)), idist, gm0);
+                gm1 = fma2(sub2(gd[j][1], mul2(dyj, dg)), idist, gm1);
+                gm2 = fma2(sub2(gd[j][2], mul2(dzj, dg)), idist, gm2);
             }
             float *o = p.g_means + 3 * n;
             st_cs(o, hsum(gm0)); st_cs(o + 1, hsum(gm1)); st_cs(o + 2, hsum(gm2));
@@ -613,7 +620,7 @@ cudaError_t launch_nasg_fwd_pipe(const FwdParams &p, int K, bool exact, cudaStre
 template <int K, int CT>
 static cudaError_t launch_bwd_pipe_kc(const BwdParams &p, bool exact, cudaStream_t st)
 {
-    constexpr size_t smem = CT >= 2 ? pipe2_smem_bytes(PipeCfg<K>::HR, 3 + 3 * CT) : pipe_smem_bytes(PipeCfg<K>::HR, 3 + 3 * CT);
+    constexpr size_t smem = CT >= 2 ? pipe2_smem_bytes(PipeCfg<K>::HR, 3 + 3 * CT) + (size_t)PBLOCK * 4 * 2 * ((CT + 1) / 2) : pipe_smem_bytes(PipeCfg<K>::HR, 3 + 3 * CT);
     const dim3 block(PBLOCK);
     static int cache[2][64] = {{0}};        // per (K, CT, norm mode) instantiation and device
     if constexpr (CT >= 2) {
