@@ -116,11 +116,14 @@ class ClockSampler:
 
 
 # ---- the oracle legs (cpu_baseline and --impl reference): the ONLY places bench.py runs oracle/ ------
+NORM_MODE = 1      # set from --norm-mode in main()
+
+
 def oracle_step(ref, W, inp, kind):
     if kind == "sh":
         ref.sh_fwd(inp); ref.sh_bwd(inp)
     else:
-        ref.nasg_fwd(inp, 1); ref.nasg_bwd(inp, 1)
+        ref.nasg_fwd(inp, NORM_MODE); ref.nasg_bwd(inp, NORM_MODE)
 
 
 def oracle_sample(W, cfg, target_s: float):
@@ -204,7 +207,7 @@ def run_ours(args, W, cfg):
         if cfg.kind == "sh":
             B.sh_eval_fwd(d["means"], d["coeffs"], d["campos"], d["vis"], out=colors, stream=stream)
         else:
-            B.nasg_eval_fwd(d["means"], d["quat"], d["shape"], d["amp"], d["dc"], d["campos"], d["vis"], 1,
+            B.nasg_eval_fwd(d["means"], d["quat"], d["shape"], d["amp"], d["dc"], d["campos"], d["vis"], args.norm_mode,
                             out=colors, stream=stream)
 
     def bwd():
@@ -212,7 +215,7 @@ def run_ours(args, W, cfg):
             B.sh_eval_bwd(d["means"], d["coeffs"], d["campos"], d["g_colors"], d["vis"], out=grads, stream=stream)
         else:
             B.nasg_eval_bwd(d["means"], d["quat"], d["shape"], d["amp"], d["dc"], d["campos"], d["g_colors"],
-                            d["vis"], 1, out=grads, stream=stream)
+                            d["vis"], args.norm_mode, out=grads, stream=stream)
 
     def barrier():
         if world > 1:
@@ -256,7 +259,7 @@ def run_ours(args, W, cfg):
                     g_quat=torch.empty((K, N, 4)).pin_memory(), g_shape=torch.empty((K, N, 4)).pin_memory(),
                     g_amp=torch.empty((K, 3, N)).pin_memory(), g_dc=torch.empty((3, N)).pin_memory())
         scratch = torch.empty(B.nasg_host_scratch_bytes(N, K, C), dtype=torch.uint8, device="cuda")
-        e2e_call = lambda: B.nasg_eval_fwd_bwd_host(host, hout, scratch, 1, stream=stream)
+        e2e_call = lambda: B.nasg_eval_fwd_bwd_host(host, hout, scratch, args.norm_mode, stream=stream)
     h2d = sum(v.numel() * v.element_size() for v in host.values() if v is not None)
     d2h = sum(v.numel() * v.element_size() for v in hout.values())
     e2e_steps = max(1, min(args.steps, 5))
@@ -280,7 +283,7 @@ def run_ours(args, W, cfg):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": cfg.name, "N_per_gpu": N, "K": K, "C": C, "norm_mode": "exact (eq.10)",
+            "config": {"workload": cfg.name, "N_per_gpu": N, "K": K, "C": C, "norm_mode": {1: "exact (eq.10)", 0: "approximate (NASG normaliser, PAPER.md:223)", 2: "pure NASG, no carrier (PAPER.md:423)"}[args.norm_mode],
                        "l2": "inputs (%.2f GB/step) larger than the 126 MB L2; no flush" % ((fb + bb) * N / 1e9),
                        "parallelism": f"{world} x independent N-shards, no collective"},
             "fwd_ms": fwd_ms, "bwd_ms": bwd_ms,
@@ -314,8 +317,12 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (default 2 = headline)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--norm-mode", type=int, default=1, choices=[0, 1, 2],
+                    help="1 = exact normaliser eq.(10) (default, the metric's configuration); 0 = the NASG normaliser the paper trained with; 2 = pure NASG lobe (no carrier)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
     args = ap.parse_args()
+    global NORM_MODE
+    NORM_MODE = 0 if args.norm_mode == 2 else args.norm_mode    # (the oracle has no carrier-free mode: same cost)
     from paper_2606_09794_b200 import workloads as W
     cfg = W.CONFIGS[args.config]
     if args.impl == "reference":

@@ -51,12 +51,15 @@ extern "C" {
 #define NASG_ERR_ALIGN          -4  /* quat/shape (or their gradients) not 16-byte aligned          */
 #define NASG_ERR_WORKSPACE      -5  /* g_campos requested but workspace NULL or too small           */
 #define NASG_ERR_CUDA           -6  /* launch / copy failed: cudaGetLastError()                     */
-#define NASG_ERR_NORM_MODE      -7  /* norm_mode not 0 or 1                                         */
+#define NASG_ERR_NORM_MODE      -7  /* norm_mode not 0, 1 or 2                                      */
 
 #define NASG_MAX_CAMERAS 64
 
 #define NASG_NORM_APPROX 0          /* NASG normaliser, carrier ignored              */
 #define NASG_NORM_EXACT  1          /* eq.(10) as printed                        */
+#define NASG_NORM_NASG   2          /* pure NASG lobe: no Gabor carrier. k and phi   */
+                                    /* (shape[...,2:4]) are ignored = taken as 0, their gradients   */
+                                    /* are written as 0; at k = 0 both normalisers above coincide   */
 
 /* Inputs of one evaluation: N Gaussians, K lobes each, C cameras. */
 typedef struct {

@@ -17,7 +17,7 @@ import torch
 
 from . import build as _build
 
-NORM_APPROX, NORM_EXACT = 0, 1
+NORM_APPROX, NORM_EXACT, NORM_NASG = 0, 1, 2
 MAX_CAMERAS = 64
 SYMBOLS = ("nasg_eval_fwd", "nasg_eval_bwd", "sh_eval_fwd", "sh_eval_bwd", "nasg_workspace_bytes",
            "nasg_host_scratch_bytes", "nasg_eval_fwd_bwd_host", "sh_host_scratch_bytes",

@@ -50,14 +50,13 @@ int nasg_eval_fwd(const nasg_inputs *in, float *colors, int norm_mode, void *cud
 {
     int rc = check_inputs(in);
     if (rc != NASG_OK) return rc;
-    if (norm_mode != NASG_NORM_APPROX && norm_mode != NASG_NORM_EXACT) return NASG_ERR_NORM_MODE;
+    if (norm_mode != NASG_NORM_APPROX && norm_mode != NASG_NORM_EXACT && norm_mode != NASG_NORM_NASG) return NASG_ERR_NORM_MODE;
     if (in->N == 0) return NASG_OK;
     if (!colors) return NASG_ERR_NULL;
     if (!aligned16(in->quat) || !aligned16(in->shape)) return NASG_ERR_ALIGN;
     nasg::FwdParams p{in->N, in->C, in->means, in->quat, in->shape, in->amp, in->dc, in->campos, in->vis, colors};
-    const bool exact = norm_mode == NASG_NORM_EXACT;
-    cudaError_t e = use_pipe(in->C) ? nasg::launch_nasg_fwd_pipe(p, in->K, exact, (cudaStream_t)cuda_stream)
-                                    : nasg::launch_nasg_fwd(p, in->K, exact, (cudaStream_t)cuda_stream);
+    cudaError_t e = use_pipe(in->C) ? nasg::launch_nasg_fwd_pipe(p, in->K, norm_mode, (cudaStream_t)cuda_stream)
+                                    : nasg::launch_nasg_fwd(p, in->K, norm_mode, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return cuda_fail(e);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     return NASG_OK;
@@ -68,7 +67,7 @@ int nasg_eval_bwd(const nasg_inputs *in, const float *g_colors, const nasg_grads
 {
     int rc = check_inputs(in);
     if (rc != NASG_OK) return rc;
-    if (norm_mode != NASG_NORM_APPROX && norm_mode != NASG_NORM_EXACT) return NASG_ERR_NORM_MODE;
+    if (norm_mode != NASG_NORM_APPROX && norm_mode != NASG_NORM_EXACT && norm_mode != NASG_NORM_NASG) return NASG_ERR_NORM_MODE;
     if (!out) return NASG_ERR_NULL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (in->N == 0) {
@@ -88,9 +87,8 @@ int nasg_eval_bwd(const nasg_inputs *in, const float *g_colors, const nasg_grads
     }
     nasg::BwdParams p{in->N, in->C, in->means, in->quat, in->shape, in->amp, in->campos, in->vis, g_colors,
                       out->g_means, out->g_quat, out->g_shape, out->g_amp, out->g_dc, partial};
-    const bool exact = norm_mode == NASG_NORM_EXACT;
-    cudaError_t e = (use_pipe(in->C) && !partial) ? nasg::launch_nasg_bwd_pipe(p, in->K, exact, st)
-                                                  : nasg::launch_nasg_bwd(p, in->K, exact, st);
+    cudaError_t e = (use_pipe(in->C) && !partial) ? nasg::launch_nasg_bwd_pipe(p, in->K, norm_mode, st)
+                                                  : nasg::launch_nasg_bwd(p, in->K, norm_mode, st);
     if (e != cudaSuccess) return cuda_fail(e);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     if (partial) {
@@ -162,7 +160,7 @@ const char *nasg_strerror(int code)
     case NASG_ERR_ALIGN: return "quat/shape (or their gradients) must be 16-byte aligned";
     case NASG_ERR_WORKSPACE: return "workspace/scratch missing, misaligned or too small";
     case NASG_ERR_CUDA: return cudaGetErrorString(t_last_cuda);
-    case NASG_ERR_NORM_MODE: return "norm_mode must be 0 (approximate) or 1 (exact, eq.10)";
+    case NASG_ERR_NORM_MODE: return "norm_mode must be 0 (approximate), 1 (exact, eq.10) or 2 (pure NASG, no carrier)";
     default: return "unknown error code";
     }
 }

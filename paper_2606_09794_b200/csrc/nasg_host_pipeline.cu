@@ -166,7 +166,7 @@ int nasg_eval_fwd_bwd_host(const nasg_inputs *in, const float *g_colors, float *
     if (!in || !out) return NASG_ERR_NULL;
     if (in->N < 0 || in->C < 1 || in->C > NASG_MAX_CAMERAS) return NASG_ERR_SHAPE;
     if (!(in->K == 1 || in->K == 2 || in->K == 3 || in->K == 4 || in->K == 5 || in->K == 8)) return NASG_ERR_UNSUPPORTED_K;
-    if (norm_mode != NASG_NORM_APPROX && norm_mode != NASG_NORM_EXACT) return NASG_ERR_NORM_MODE;
+    if (norm_mode != NASG_NORM_APPROX && norm_mode != NASG_NORM_EXACT && norm_mode != NASG_NORM_NASG) return NASG_ERR_NORM_MODE;
     if (in->N == 0) return NASG_OK;
     if (!in->means || !in->quat || !in->shape || !in->amp || !in->dc || !in->campos || !g_colors || !colors || !dev_scratch)
         return NASG_ERR_NULL;

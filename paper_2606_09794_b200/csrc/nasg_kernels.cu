@@ -21,7 +21,7 @@ __device__ __forceinline__ float4 ldg4(const float *base, int64_t idx)
 // ---------------------------------------------------------------------------------------------
 // forward: colors[c,n,:] = c0 + sum_l w_l G_l(d_cn)           eq.(6), eq.(9), eq.(10)
 // ---------------------------------------------------------------------------------------------
-template <int K, int CT, bool EXACT>
+template <int K, int CT, int MODE>
 __global__ void __launch_bounds__(BLOCK, 2) nasg_fwd_kernel(FwdParams p)
 {
     const int64_t N = p.N;
@@ -60,12 +60,12 @@ __global__ void __launch_bounds__(BLOCK, 2) nasg_fwd_kernel(FwdParams p)
                 const float w1 = __ldg(p.amp + ((int64_t)l * 3 + 1) * N + n);
                 const float w2 = __ldg(p.amp + ((int64_t)l * 3 + 2) * N + n);
                 Lobe L; LobeBwd B;
-                lobe_setup<EXACT, false>(q, sp, L, B);
+                lobe_setup<MODE, false>(q, sp, L, B);
 #pragma unroll
                 for (int t = 0; t < CT; ++t) {
                     if (mask & (1u << t)) {
                         EvalTerms T;
-                        const float G = lobe_eval<false>(L, dx[t], dy[t], dz[t], T);
+                        const float G = lobe_eval<false, MODE != 2>(L, dx[t], dy[t], dz[t], T);
                         col[t][0] = fmaf(w0, G, col[t][0]);
                         col[t][1] = fmaf(w1, G, col[t][1]);
                         col[t][2] = fmaf(w2, G, col[t][2]);
@@ -105,7 +105,7 @@ __device__ __forceinline__ void block_sum_store(float v, float *smem, float *dst
     }
 }
 
-template <int K, int CT, bool EXACT, bool CAMGRAD>
+template <int K, int CT, int MODE, bool CAMGRAD>
 __global__ void __launch_bounds__(BLOCK, 2) nasg_bwd_kernel(BwdParams p)
 {
     __shared__ float red[BLOCK / 32];
@@ -160,14 +160,14 @@ __global__ void __launch_bounds__(BLOCK, 2) nasg_bwd_kernel(BwdParams p)
                     const float w1 = __ldg(p.amp + ((int64_t)l * 3 + 1) * N + n);
                     const float w2 = __ldg(p.amp + ((int64_t)l * 3 + 2) * N + n);
                     Lobe L; LobeBwd B;
-                    lobe_setup<EXACT, true>(q, sp, L, B);
+                    lobe_setup<MODE, true>(q, sp, L, B);
                     float gX0 = 0.f, gX1 = 0.f, gX2 = 0.f, gZ0 = 0.f, gZ1 = 0.f, gZ2 = 0.f;
                     float S0 = 0.f, S1 = 0.f, S2 = 0.f, Sk = 0.f, Sp = 0.f;
 #pragma unroll
                     for (int t = 0; t < CT; ++t) {
                         if (mask & (1u << t)) {
                             EvalTerms T;
-                            const float G = lobe_eval<true>(L, dx[t], dy[t], dz[t], T);
+                            const float G = lobe_eval<true, MODE != 2>(L, dx[t], dy[t], dz[t], T);
                             const float gG = fmaf(gc[t][0], w0, fmaf(gc[t][1], w1, gc[t][2] * w2)); // dL/dG, eq.(6)
                             gw[0] = fmaf(gc[t][0], G, gw[0]);
                             gw[1] = fmaf(gc[t][1], G, gw[1]);
@@ -280,55 +280,57 @@ __global__ void __launch_bounds__(BLOCK) campos_reduce_kernel(const float *parti
 int64_t grid_blocks(int64_t N) { return (N + BLOCK - 1) / BLOCK; }
 
 template <int K, int CT>
-static cudaError_t launch_fwd_kc(const FwdParams &p, bool exact, cudaStream_t st)
+static cudaError_t launch_fwd_kc(const FwdParams &p, int mode, cudaStream_t st)
 {
     const dim3 grid((unsigned)grid_blocks(p.N)), block(BLOCK);
-    if (exact) nasg_fwd_kernel<K, CT, true><<<grid, block, 0, st>>>(p);
-    else nasg_fwd_kernel<K, CT, false><<<grid, block, 0, st>>>(p);
+    if (mode == 1) nasg_fwd_kernel<K, CT, 1><<<grid, block, 0, st>>>(p);
+    else if (mode == 0) nasg_fwd_kernel<K, CT, 0><<<grid, block, 0, st>>>(p);
+    else nasg_fwd_kernel<K, CT, 2><<<grid, block, 0, st>>>(p);
     return cudaGetLastError();
 }
 template <int K>
-static cudaError_t launch_fwd_k(const FwdParams &p, bool exact, cudaStream_t st)
+static cudaError_t launch_fwd_k(const FwdParams &p, int mode, cudaStream_t st)
 {
-    return p.C == 1 ? launch_fwd_kc<K, 1>(p, exact, st) : launch_fwd_kc<K, 4>(p, exact, st);
+    return p.C == 1 ? launch_fwd_kc<K, 1>(p, mode, st) : launch_fwd_kc<K, 4>(p, mode, st);
 }
-cudaError_t launch_nasg_fwd(const FwdParams &p, int K, bool exact, cudaStream_t st)
+cudaError_t launch_nasg_fwd(const FwdParams &p, int K, int mode, cudaStream_t st)
 {
     switch (K) {
-    case 1: return launch_fwd_k<1>(p, exact, st);
-    case 2: return launch_fwd_k<2>(p, exact, st);
-    case 3: return launch_fwd_k<3>(p, exact, st);
-    case 4: return launch_fwd_k<4>(p, exact, st);
-    case 5: return launch_fwd_k<5>(p, exact, st);
-    case 8: return launch_fwd_k<8>(p, exact, st);
+    case 1: return launch_fwd_k<1>(p, mode, st);
+    case 2: return launch_fwd_k<2>(p, mode, st);
+    case 3: return launch_fwd_k<3>(p, mode, st);
+    case 4: return launch_fwd_k<4>(p, mode, st);
+    case 5: return launch_fwd_k<5>(p, mode, st);
+    case 8: return launch_fwd_k<8>(p, mode, st);
     default: return cudaErrorInvalidValue;
     }
 }
 
 template <int K, int CT, bool CAMGRAD>
-static cudaError_t launch_bwd_kcg(const BwdParams &p, bool exact, cudaStream_t st)
+static cudaError_t launch_bwd_kcg(const BwdParams &p, int mode, cudaStream_t st)
 {
     const dim3 grid((unsigned)grid_blocks(p.N)), block(BLOCK);
-    if (exact) nasg_bwd_kernel<K, CT, true, CAMGRAD><<<grid, block, 0, st>>>(p);
-    else nasg_bwd_kernel<K, CT, false, CAMGRAD><<<grid, block, 0, st>>>(p);
+    if (mode == 1) nasg_bwd_kernel<K, CT, 1, CAMGRAD><<<grid, block, 0, st>>>(p);
+    else if (mode == 0) nasg_bwd_kernel<K, CT, 0, CAMGRAD><<<grid, block, 0, st>>>(p);
+    else nasg_bwd_kernel<K, CT, 2, CAMGRAD><<<grid, block, 0, st>>>(p);
     return cudaGetLastError();
 }
 template <int K>
-static cudaError_t launch_bwd_k(const BwdParams &p, bool exact, cudaStream_t st)
+static cudaError_t launch_bwd_k(const BwdParams &p, int mode, cudaStream_t st)
 {
     const bool cam = p.cam_partial != nullptr;
-    if (p.C == 1) return cam ? launch_bwd_kcg<K, 1, true>(p, exact, st) : launch_bwd_kcg<K, 1, false>(p, exact, st);
-    return cam ? launch_bwd_kcg<K, 4, true>(p, exact, st) : launch_bwd_kcg<K, 4, false>(p, exact, st);
+    if (p.C == 1) return cam ? launch_bwd_kcg<K, 1, true>(p, mode, st) : launch_bwd_kcg<K, 1, false>(p, mode, st);
+    return cam ? launch_bwd_kcg<K, 4, true>(p, mode, st) : launch_bwd_kcg<K, 4, false>(p, mode, st);
 }
-cudaError_t launch_nasg_bwd(const BwdParams &p, int K, bool exact, cudaStream_t st)
+cudaError_t launch_nasg_bwd(const BwdParams &p, int K, int mode, cudaStream_t st)
 {
     switch (K) {
-    case 1: return launch_bwd_k<1>(p, exact, st);
-    case 2: return launch_bwd_k<2>(p, exact, st);
-    case 3: return launch_bwd_k<3>(p, exact, st);
-    case 4: return launch_bwd_k<4>(p, exact, st);
-    case 5: return launch_bwd_k<5>(p, exact, st);
-    case 8: return launch_bwd_k<8>(p, exact, st);
+    case 1: return launch_bwd_k<1>(p, mode, st);
+    case 2: return launch_bwd_k<2>(p, mode, st);
+    case 3: return launch_bwd_k<3>(p, mode, st);
+    case 4: return launch_bwd_k<4>(p, mode, st);
+    case 5: return launch_bwd_k<5>(p, mode, st);
+    case 8: return launch_bwd_k<8>(p, mode, st);
     default: return cudaErrorInvalidValue;
     }
 }

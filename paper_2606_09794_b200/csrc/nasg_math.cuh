@@ -211,7 +211,9 @@ NASG_HD void normaliser(float l1, float l2, float Lam, float lam, float k, float
     }
 }
 
-template <bool EXACT, bool GRAD>
+// MODE: 0 = NASG normaliser (approximate), 1 = eq.(10) (exact), 2 = pure NASG: no carrier (k = phi = 0 assumed,
+// shape.z/.w ignored), for which both normalisers coincide (Psi(k=0) = 1)
+template <int MODE, bool GRAD>
 NASG_HD void lobe_setup(const float4 q, const float4 sp, Lobe &L, LobeBwd &B)
 {
     const float qq = q.x * q.x + q.y * q.y + q.z * q.z + q.w * q.w;
@@ -228,9 +230,9 @@ NASG_HD void lobe_setup(const float4 q, const float4 sp, Lobe &L, LobeBwd &B)
     const float Lam = lam * one_pa;
     L.a = fmaxf(one_pa - 1.0f, 0.0f);
     L.lam2e = 2.0f * LOG2E * lam;
-    L.kt = sp.z * INV_TWO_PI; L.pt = sp.w * INV_TWO_PI;
+    L.kt = MODE == 2 ? 0.f : sp.z * INV_TWO_PI; L.pt = MODE == 2 ? 0.f : sp.w * INV_TWO_PI;
     float nA = 0.f, nL = 0.f, nk = 0.f;
-    normaliser<EXACT, GRAD>(sp.x, sp.y, Lam, lam, sp.z, L.lgI, nA, nL, nk);
+    normaliser<MODE == 1, GRAD>(sp.x, sp.y, Lam, lam, sp.z, L.lgI, nA, nL, nk);
     if (GRAD) {
         B.qw = w; B.qx = x; B.qy = y; B.qz = z; B.inv_qn = inv_qn;
         B.lam2 = 2.0f * lam; B.k = sp.z;
@@ -247,7 +249,7 @@ struct EvalTerms {      // what the backward needs from the recomputed forward
 
 // G = H p E / I at direction (dx,dy,dz) (eq.(9) over eq.(10)). With FULL also fills the terms the
 // backward needs. MUFU count: rcp, lg2, ex2, ex2, cos (+ sin with FULL).
-template <bool FULL>
+template <bool FULL, bool CARRIER = true>
 NASG_HD float lobe_eval(const Lobe &L, float dx, float dy, float dz, EvalTerms &T)
 {
     const float u = fmaf(dx, L.Xx, fmaf(dy, L.Xy, dz * L.Xz));
@@ -268,12 +270,12 @@ NASG_HD float lobe_eval(const Lobe &L, float dx, float dy, float dz, EvalTerms &
     const float arg = fmaf(L.lam2e, em1, fmaf(tau, L2, L.lgI));   // log2( p E / (2 I) )
     float Gh = f_ex2(arg);
     Gh = (s2 <= TINY && !upper) ? 0.0f : Gh;                 // d = -z: G = 0 (eq.(9), third case)
-    const float ang = reduce_turns(fmaf(L.kt, u, L.pt));     // k d.x + phi  (mod 2 pi)
-    const float G = fmaf(Gh, f_cos(ang), Gh);                // (1 + cos)/2 * p E / I
+    const float ang = CARRIER ? reduce_turns(fmaf(L.kt, u, L.pt)) : 0.f;     // k d.x + phi  (mod 2 pi)
+    const float G = CARRIER ? fmaf(Gh, f_cos(ang), Gh) : Gh + Gh;            // (1 + cos)/2 * p E / I   (no carrier: H = 1)
     if (FULL) {
         T.u = u; T.v = v; T.uu = uu; T.inv_s2 = inv_s2; T.tau = tau; T.Lk = LN2 * L2; T.kp = kp; T.em1 = em1;
         T.inv_2kappa = upper ? 2.0f * s2 * rw : 0.5f * w2 * inv_s2;      // 1/(1+v)
-        T.Gh = Gh; T.sn = f_sin(ang);
+        T.Gh = Gh; T.sn = CARRIER ? f_sin(ang) : 0.f;
     }
     return G;
 }
@@ -299,7 +301,7 @@ struct EvalTerms2 {
 // lobe_eval for a pair of directions (dx.x,dy.x,dz.x), (dx.y,dy.y,dz.y)
 // `bias` is added to the base-2 exponent of each half: 0 for a live camera slot, -1e30 for a culled one
 // (then p E / I = 0 and every gradient contribution of the slot vanishes without a select).
-template <bool FULL>
+template <bool FULL, bool CARRIER = true>
 __device__ __forceinline__ float2 lobe_eval2(const Lobe &L, float2 dx, float2 dy, float2 dz, float2 bias, EvalTerms2 &T)
 {
     const float2 u = fma2(dx, splat(L.Xx), fma2(dy, splat(L.Xy), mul2(dz, splat(L.Xz))));
@@ -339,17 +341,22 @@ __device__ __forceinline__ float2 lobe_eval2(const Lobe &L, float2 dx, float2 dy
     float2 Gh = make_float2(f_ex2(arg.x), f_ex2(arg.y));
     Gh.x = (s2.x <= TINY && !up0) ? 0.0f : Gh.x;                   // d = -z: G = 0 (eq.(9), third case)
     Gh.y = (s2.y <= TINY && !up1) ? 0.0f : Gh.y;
-    // carrier: angle in turns, exact reduction to [-1/2, 1/2] (reduce_turns)
-    const float2 t = fma2(splat(L.kt), u, splat(L.pt));
-    const float2 n = add2(add2(t, splat(12582912.0f)), splat(-12582912.0f));
-    const float2 ang = mul2(sub2(t, n), splat(TWO_PI));
-    const float2 G = fma2(Gh, make_float2(f_cos(ang.x), f_cos(ang.y)), Gh);
+    // carrier: angle in turns, exact reduction to [-1/2, 1/2] (reduce_turns); without carrier H = 1
+    float2 ang = splat(0.f), G;
+    if (CARRIER) {
+        const float2 t = fma2(splat(L.kt), u, splat(L.pt));
+        const float2 n = add2(add2(t, splat(12582912.0f)), splat(-12582912.0f));
+        ang = mul2(sub2(t, n), splat(TWO_PI));
+        G = fma2(Gh, make_float2(f_cos(ang.x), f_cos(ang.y)), Gh);
+    } else {
+        G = add2(Gh, Gh);
+    }
     if (FULL) {
         T.u = u; T.v = v; T.uu = uu; T.inv_s2 = inv_s2; T.tau = tau; T.Lk = mul2(splat(LN2), L2);
         T.kp = add2(em1, splat(1.0f)); T.em1 = em1;
         const float2 hi = add2(s2rw, s2rw), lo = mul2(mul2(splat(0.5f), w2), inv_s2);   // 1/(1+v) on the lobe side / far side
         T.inv_2kappa = make_float2(up0 ? hi.x : lo.x, up1 ? hi.y : lo.y);
-        T.Gh = Gh; T.sn = make_float2(f_sin(ang.x), f_sin(ang.y));
+        T.Gh = Gh; T.sn = CARRIER ? make_float2(f_sin(ang.x), f_sin(ang.y)) : splat(0.f);
     }
     return G;
 }

@@ -69,7 +69,7 @@ __device__ __forceinline__ void prefetch_lobe(const Ring &r, int slot, int tid, 
 // ---------------------------------------------------------------------------------------------
 // forward
 // ---------------------------------------------------------------------------------------------
-template <int K, int CT, bool EXACT>
+template <int K, int CT, int MODE>
 __global__ void __launch_bounds__(PBLOCK, CT >= 3 ? 3 : 4) nasg_fwd_pipe_kernel(FwdParams p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -126,12 +126,12 @@ __global__ void __launch_bounds__(PBLOCK, CT >= 3 ? 3 : 4) nasg_fwd_pipe_kernel(
                 const float w0 = r.w[(slot * 3 + 0) * PBLOCK + tid], w1 = r.w[(slot * 3 + 1) * PBLOCK + tid],
                             w2 = r.w[(slot * 3 + 2) * PBLOCK + tid];
                 Lobe L; LobeBwd B;
-                lobe_setup<EXACT, false>(q, sp, L, B);
+                lobe_setup<MODE, false>(q, sp, L, B);
 #pragma unroll
                 for (int t = 0; t < CT; ++t) {
                     {   // every camera slot is evaluated: culled slots carry g_colors = 0 / are zeroed at the store
                         EvalTerms T;
-                        const float G = lobe_eval<false>(L, dx[t], dy[t], dz[t], T);
+                        const float G = lobe_eval<false, MODE != 2>(L, dx[t], dy[t], dz[t], T);
                         col[t][0] = fmaf(w0, G, col[t][0]);
                         col[t][1] = fmaf(w1, G, col[t][1]);
                         col[t][2] = fmaf(w2, G, col[t][2]);
@@ -155,7 +155,7 @@ __global__ void __launch_bounds__(PBLOCK, CT >= 3 ? 3 : 4) nasg_fwd_pipe_kernel(
 }
 
 // forward, two cameras per packed f32x2 instruction (CT >= 2)
-template <int K, int CT, bool EXACT>
+template <int K, int CT, int MODE>
 __global__ void __launch_bounds__(PBLOCK, CT >= 3 ? 3 : 4) nasg_fwd_pipe2_kernel(FwdParams p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -225,12 +225,12 @@ __global__ void __launch_bounds__(PBLOCK, CT >= 3 ? 3 : 4) nasg_fwd_pipe2_kernel
                 const float2 w0 = splat(r.w[(slot * 3 + 0) * PBLOCK + tid]), w1 = splat(r.w[(slot * 3 + 1) * PBLOCK + tid]),
                              w2 = splat(r.w[(slot * 3 + 2) * PBLOCK + tid]);
                 Lobe L; LobeBwd B;
-                lobe_setup<EXACT, false>(q, sp, L, B);
+                lobe_setup<MODE, false>(q, sp, L, B);
 #pragma unroll
                 for (int j = 0; j < NP; ++j) {
                     // every camera slot is evaluated: culled slots are zeroed at the store
                     EvalTerms2 T;
-                    const float2 G = lobe_eval2<false>(L, dx[j], dy[j], dz[j], splat(0.f), T);
+                    const float2 G = lobe_eval2<false, MODE != 2>(L, dx[j], dy[j], dz[j], splat(0.f), T);
                     col[j][0] = fma2(w0, G, col[j][0]);
                     col[j][1] = fma2(w1, G, col[j][1]);
                     col[j][2] = fma2(w2, G, col[j][2]);
@@ -257,7 +257,7 @@ __global__ void __launch_bounds__(PBLOCK, CT >= 3 ? 3 : 4) nasg_fwd_pipe2_kernel
 // ---------------------------------------------------------------------------------------------
 // backward (no g_campos: that optional reduction stays on the generic kernel)
 // ---------------------------------------------------------------------------------------------
-template <int K, int CT, bool EXACT>
+template <int K, int CT, int MODE>
 __global__ void __launch_bounds__(PBLOCK, 2) nasg_bwd_pipe_kernel(BwdParams p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -330,14 +330,14 @@ __global__ void __launch_bounds__(PBLOCK, 2) nasg_bwd_pipe_kernel(BwdParams p)
                 const float w0 = r.w[(slot * 3 + 0) * PBLOCK + tid], w1 = r.w[(slot * 3 + 1) * PBLOCK + tid],
                             w2 = r.w[(slot * 3 + 2) * PBLOCK + tid];
                 Lobe L; LobeBwd B;
-                lobe_setup<EXACT, true>(q, sp, L, B);
+                lobe_setup<MODE, true>(q, sp, L, B);
                 float gX0 = 0.f, gX1 = 0.f, gX2 = 0.f, gZ0 = 0.f, gZ1 = 0.f, gZ2 = 0.f;
                 float S0 = 0.f, S1 = 0.f, S2 = 0.f, Sk = 0.f, Sp = 0.f;
 #pragma unroll
                 for (int t = 0; t < CT; ++t) {
                     {   // every camera slot is evaluated: culled slots carry g_colors = 0 / are zeroed at the store
                         EvalTerms T;
-                        const float G = lobe_eval<true>(L, dx[t], dy[t], dz[t], T);
+                        const float G = lobe_eval<true, MODE != 2>(L, dx[t], dy[t], dz[t], T);
                         const float gG = fmaf(gc[t][0], w0, fmaf(gc[t][1], w1, gc[t][2] * w2));   // dL/dG, eq.(6)
                         gw0 = fmaf(gc[t][0], G, gw0); gw1 = fmaf(gc[t][1], G, gw1); gw2 = fmaf(gc[t][2], G, gw2);
                         const float gGG = gG * G;
@@ -406,7 +406,7 @@ __device__ __forceinline__ float hsum(float2 a) { return a.x + a.y; }
 #ifndef NASG_BWD2_MINB
 #define NASG_BWD2_MINB 2
 #endif
-template <int K, int CT, bool EXACT>
+template <int K, int CT, int MODE>
 __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(BwdParams p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -492,7 +492,7 @@ __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(
                 const float2 w0 = splat(r.w[(slot * 3 + 0) * PBLOCK + tid]), w1 = splat(r.w[(slot * 3 + 1) * PBLOCK + tid]),
                              w2 = splat(r.w[(slot * 3 + 2) * PBLOCK + tid]);
                 Lobe L; LobeBwd B;
-                lobe_setup<EXACT, true>(r.q[slot * PBLOCK + tid], sp, L, B);
+                lobe_setup<MODE, true>(r.q[slot * PBLOCK + tid], sp, L, B);
                 const float2 z2 = splat(0.f);
                 float2 pw0 = z2, pw1 = z2, pw2 = z2;                             // packed accumulators, halves summed below
                 float2 gX0 = z2, gX1 = z2, gX2 = z2, gZ0 = z2, gZ1 = z2, gZ2 = z2;
@@ -508,7 +508,7 @@ __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(
                     EvalTerms2 T;
                     const float2 bias = make_float2((mask & (1u << t0)) ? 0.f : -1e30f,
                                                     (2 * j + 1 < CT && (mask & (1u << t1))) ? 0.f : -1e30f);   // (re-derived: 4 fewer live registers)
-                    const float2 G = lobe_eval2<true>(L, dxj, dyj, dzj, bias, T);
+                    const float2 G = lobe_eval2<true, MODE != 2>(L, dxj, dyj, dzj, bias, T);
                     const float2 gG = fma2(gc0, w0, fma2(gc1, w1, mul2(gc2, w2)));                      // dL/dG, eq.(6)
                     pw0 = fma2(gc0, G, pw0); pw1 = fma2(gc1, G, pw1); pw2 = fma2(gc2, G, pw2);
                     const float2 gGG = mul2(gG, G);
@@ -582,73 +582,77 @@ __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(
 // launchers: persistent grid, 2 blocks per SM
 // ---------------------------------------------------------------------------------------------
 template <int K, int CT>
-static cudaError_t launch_fwd_pipe_kc(const FwdParams &p, bool exact, cudaStream_t st)
+static cudaError_t launch_fwd_pipe_kc(const FwdParams &p, int mode, cudaStream_t st)
 {
     constexpr size_t smem = CT >= 2 ? pipe2_smem_bytes(PipeCfg<K>::HR, 6) : pipe_smem_bytes(PipeCfg<K>::HR, 6);
     const dim3 block(PBLOCK);
-    static int cache[2][64] = {{0}};        // per (K, CT, norm mode) instantiation and device
+    static int cache[3][64] = {{0}};        // per (K, CT, norm mode) instantiation and device
     if constexpr (CT >= 2) {
-        if (exact) nasg_fwd_pipe2_kernel<K, CT, true><<<pipe_grid(nasg_fwd_pipe2_kernel<K, CT, true>, smem, p.N, cache[1]), block, smem, st>>>(p);
-        else nasg_fwd_pipe2_kernel<K, CT, false><<<pipe_grid(nasg_fwd_pipe2_kernel<K, CT, false>, smem, p.N, cache[0]), block, smem, st>>>(p);
+        if (mode == 1) nasg_fwd_pipe2_kernel<K, CT, 1><<<pipe_grid(nasg_fwd_pipe2_kernel<K, CT, 1>, smem, p.N, cache[1]), block, smem, st>>>(p);
+        else if (mode == 0) nasg_fwd_pipe2_kernel<K, CT, 0><<<pipe_grid(nasg_fwd_pipe2_kernel<K, CT, 0>, smem, p.N, cache[0]), block, smem, st>>>(p);
+        else nasg_fwd_pipe2_kernel<K, CT, 2><<<pipe_grid(nasg_fwd_pipe2_kernel<K, CT, 2>, smem, p.N, cache[2]), block, smem, st>>>(p);
     } else {
-        if (exact) nasg_fwd_pipe_kernel<K, CT, true><<<pipe_grid(nasg_fwd_pipe_kernel<K, CT, true>, smem, p.N, cache[1]), block, smem, st>>>(p);
-        else nasg_fwd_pipe_kernel<K, CT, false><<<pipe_grid(nasg_fwd_pipe_kernel<K, CT, false>, smem, p.N, cache[0]), block, smem, st>>>(p);
+        if (mode == 1) nasg_fwd_pipe_kernel<K, CT, 1><<<pipe_grid(nasg_fwd_pipe_kernel<K, CT, 1>, smem, p.N, cache[1]), block, smem, st>>>(p);
+        else if (mode == 0) nasg_fwd_pipe_kernel<K, CT, 0><<<pipe_grid(nasg_fwd_pipe_kernel<K, CT, 0>, smem, p.N, cache[0]), block, smem, st>>>(p);
+        else nasg_fwd_pipe_kernel<K, CT, 2><<<pipe_grid(nasg_fwd_pipe_kernel<K, CT, 2>, smem, p.N, cache[2]), block, smem, st>>>(p);
     }
     return cudaGetLastError();
 }
 template <int K>
-static cudaError_t launch_fwd_pipe_k(const FwdParams &p, bool exact, cudaStream_t st)
+static cudaError_t launch_fwd_pipe_k(const FwdParams &p, int mode, cudaStream_t st)
 {
-    if (p.C == 1) return launch_fwd_pipe_kc<K, 1>(p, exact, st);
-    if (p.C == 2) return launch_fwd_pipe_kc<K, 2>(p, exact, st);
-    if (p.C == 3) return launch_fwd_pipe_kc<K, 3>(p, exact, st);
-    return launch_fwd_pipe_kc<K, 4>(p, exact, st);
+    if (p.C == 1) return launch_fwd_pipe_kc<K, 1>(p, mode, st);
+    if (p.C == 2) return launch_fwd_pipe_kc<K, 2>(p, mode, st);
+    if (p.C == 3) return launch_fwd_pipe_kc<K, 3>(p, mode, st);
+    return launch_fwd_pipe_kc<K, 4>(p, mode, st);
 }
-cudaError_t launch_nasg_fwd_pipe(const FwdParams &p, int K, bool exact, cudaStream_t st)
+cudaError_t launch_nasg_fwd_pipe(const FwdParams &p, int K, int mode, cudaStream_t st)
 {
     switch (K) {
-    case 1: return launch_fwd_pipe_k<1>(p, exact, st);
-    case 2: return launch_fwd_pipe_k<2>(p, exact, st);
-    case 3: return launch_fwd_pipe_k<3>(p, exact, st);
-    case 4: return launch_fwd_pipe_k<4>(p, exact, st);
-    case 5: return launch_fwd_pipe_k<5>(p, exact, st);
-    case 8: return launch_fwd_pipe_k<8>(p, exact, st);
+    case 1: return launch_fwd_pipe_k<1>(p, mode, st);
+    case 2: return launch_fwd_pipe_k<2>(p, mode, st);
+    case 3: return launch_fwd_pipe_k<3>(p, mode, st);
+    case 4: return launch_fwd_pipe_k<4>(p, mode, st);
+    case 5: return launch_fwd_pipe_k<5>(p, mode, st);
+    case 8: return launch_fwd_pipe_k<8>(p, mode, st);
     default: return cudaErrorInvalidValue;
     }
 }
 
 template <int K, int CT>
-static cudaError_t launch_bwd_pipe_kc(const BwdParams &p, bool exact, cudaStream_t st)
+static cudaError_t launch_bwd_pipe_kc(const BwdParams &p, int mode, cudaStream_t st)
 {
     constexpr size_t smem = CT >= 2 ? pipe2_smem_bytes(PipeCfg<K>::HR, 3 + 3 * CT) + (size_t)PBLOCK * 4 * 2 * ((CT + 1) / 2) : pipe_smem_bytes(PipeCfg<K>::HR, 3 + 3 * CT);
     const dim3 block(PBLOCK);
-    static int cache[2][64] = {{0}};        // per (K, CT, norm mode) instantiation and device
+    static int cache[3][64] = {{0}};        // per (K, CT, norm mode) instantiation and device
     if constexpr (CT >= 2) {
-        if (exact) nasg_bwd_pipe2_kernel<K, CT, true><<<pipe_grid(nasg_bwd_pipe2_kernel<K, CT, true>, smem, p.N, cache[1]), block, smem, st>>>(p);
-        else nasg_bwd_pipe2_kernel<K, CT, false><<<pipe_grid(nasg_bwd_pipe2_kernel<K, CT, false>, smem, p.N, cache[0]), block, smem, st>>>(p);
+        if (mode == 1) nasg_bwd_pipe2_kernel<K, CT, 1><<<pipe_grid(nasg_bwd_pipe2_kernel<K, CT, 1>, smem, p.N, cache[1]), block, smem, st>>>(p);
+        else if (mode == 0) nasg_bwd_pipe2_kernel<K, CT, 0><<<pipe_grid(nasg_bwd_pipe2_kernel<K, CT, 0>, smem, p.N, cache[0]), block, smem, st>>>(p);
+        else nasg_bwd_pipe2_kernel<K, CT, 2><<<pipe_grid(nasg_bwd_pipe2_kernel<K, CT, 2>, smem, p.N, cache[2]), block, smem, st>>>(p);
     } else {
-        if (exact) nasg_bwd_pipe_kernel<K, CT, true><<<pipe_grid(nasg_bwd_pipe_kernel<K, CT, true>, smem, p.N, cache[1]), block, smem, st>>>(p);
-        else nasg_bwd_pipe_kernel<K, CT, false><<<pipe_grid(nasg_bwd_pipe_kernel<K, CT, false>, smem, p.N, cache[0]), block, smem, st>>>(p);
+        if (mode == 1) nasg_bwd_pipe_kernel<K, CT, 1><<<pipe_grid(nasg_bwd_pipe_kernel<K, CT, 1>, smem, p.N, cache[1]), block, smem, st>>>(p);
+        else if (mode == 0) nasg_bwd_pipe_kernel<K, CT, 0><<<pipe_grid(nasg_bwd_pipe_kernel<K, CT, 0>, smem, p.N, cache[0]), block, smem, st>>>(p);
+        else nasg_bwd_pipe_kernel<K, CT, 2><<<pipe_grid(nasg_bwd_pipe_kernel<K, CT, 2>, smem, p.N, cache[2]), block, smem, st>>>(p);
     }
     return cudaGetLastError();
 }
 template <int K>
-static cudaError_t launch_bwd_pipe_k(const BwdParams &p, bool exact, cudaStream_t st)
+static cudaError_t launch_bwd_pipe_k(const BwdParams &p, int mode, cudaStream_t st)
 {
-    if (p.C == 1) return launch_bwd_pipe_kc<K, 1>(p, exact, st);
-    if (p.C == 2) return launch_bwd_pipe_kc<K, 2>(p, exact, st);
-    if (p.C == 3) return launch_bwd_pipe_kc<K, 3>(p, exact, st);
-    return launch_bwd_pipe_kc<K, 4>(p, exact, st);
+    if (p.C == 1) return launch_bwd_pipe_kc<K, 1>(p, mode, st);
+    if (p.C == 2) return launch_bwd_pipe_kc<K, 2>(p, mode, st);
+    if (p.C == 3) return launch_bwd_pipe_kc<K, 3>(p, mode, st);
+    return launch_bwd_pipe_kc<K, 4>(p, mode, st);
 }
-cudaError_t launch_nasg_bwd_pipe(const BwdParams &p, int K, bool exact, cudaStream_t st)
+cudaError_t launch_nasg_bwd_pipe(const BwdParams &p, int K, int mode, cudaStream_t st)
 {
     switch (K) {
-    case 1: return launch_bwd_pipe_k<1>(p, exact, st);
-    case 2: return launch_bwd_pipe_k<2>(p, exact, st);
-    case 3: return launch_bwd_pipe_k<3>(p, exact, st);
-    case 4: return launch_bwd_pipe_k<4>(p, exact, st);
-    case 5: return launch_bwd_pipe_k<5>(p, exact, st);
-    case 8: return launch_bwd_pipe_k<8>(p, exact, st);
+    case 1: return launch_bwd_pipe_k<1>(p, mode, st);
+    case 2: return launch_bwd_pipe_k<2>(p, mode, st);
+    case 3: return launch_bwd_pipe_k<3>(p, mode, st);
+    case 4: return launch_bwd_pipe_k<4>(p, mode, st);
+    case 5: return launch_bwd_pipe_k<5>(p, mode, st);
+    case 8: return launch_bwd_pipe_k<8>(p, mode, st);
     default: return cudaErrorInvalidValue;
     }
 }

@@ -60,7 +60,7 @@ def test_error_codes_without_gpu(B):
     assert fwd(inputs(N=-1)) == -2 and fwd(inputs(Cn=0)) == -2 and fwd(inputs(Cn=65)) == -2   # SHAPE
     assert fwd(inputs(K=6)) == -3 and fwd(inputs(K=0)) == -3                     # UNSUPPORTED_K
     assert fwd(inputs(quat=p + 4)) == -4                                        # ALIGN
-    assert fwd(inputs(), mode=2) == -7                                          # NORM_MODE
+    assert fwd(inputs(), mode=3) == -7                                          # NORM_MODE (0, 1, 2 are valid)
     assert fwd(inputs(N=0, means=None)) == 0                                    # N == 0 is a no-op
     g = B._Grads(p, p, p, p, p, p, None, 0)
     assert lib.nasg_eval_bwd(C.byref(inputs()), C.c_void_p(p), C.byref(g), 1, None) == -5   # WORKSPACE

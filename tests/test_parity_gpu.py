@@ -38,6 +38,27 @@ def test_sh_config_small(B, W, oracle):
     check_sh(B, oracle, inp, want_campos=True, label="cfg3 N=60001")
 
 
+@pytest.mark.parametrize("cfg,N,K,C", [(2, 20_011, 4, 4), (1, 20_000, 4, 1), (2, 3_001, 2, 3), (4, 9_999, 8, 1), (2, 2_048, 3, 6)])
+def test_pure_nasg_mode_ignores_the_carrier(B, W, oracle, cfg, N, K, C):
+    """norm_mode 2: the NASG lobe of PAPER.md:423 — k and phi are taken as 0
+    whatever shape[...,2:4] holds, their gradients are 0. The oracle evaluates the same inputs with k = phi = 0
+    (where eq.(10) and the NASG normaliser coincide: Psi(k=0) = 1, pinned by P4)."""
+    c = dataclasses.replace(W.CONFIGS[cfg], seed=300 + K + C, K=K, C=C)
+    inp = W.make_nasg(c, N=N)
+    zero = dict(inp, shape=inp["shape"].copy())
+    zero["shape"][..., 2:] = 0.0
+    rc, rg = oracle.nasg_fwd(zero, 0), oracle.nasg_bwd(zero, 0)
+    assert np.abs(oracle.nasg_fwd(zero, 1) - rc).max() <= 1e-12 * np.abs(rc).max()
+    d = to_dev(inp, NASG_KEYS)
+    for want_campos in (False, True):                       # fast path, then generic kernels
+        col, g = run_nasg(B, d, 2, want_campos)
+        assert rel_err(col, rc) <= FWD_TOL
+        for k in ("g_means", "g_quat", "g_amp", "g_dc") + (("g_campos",) if want_campos else ()):
+            assert rel_err(g[k], rg[k]) <= BWD_TOL, k
+        assert rel_err(g["g_shape"][..., :2], rg["g_shape"][..., :2]) <= BWD_TOL
+        assert (g["g_shape"][..., 2:] == 0).all()
+
+
 @pytest.mark.parametrize("K", [1, 2, 3, 4, 5, 8])
 @pytest.mark.parametrize("C", [1, 2, 3, 4, 5, 9])
 def test_all_lobe_counts_and_camera_tiles(B, W, oracle, K, C):
