@@ -1,6 +1,6 @@
-// nasg_api.cu — the extern "C" boundary declared in include/nasg.h: argument validation, dispatch
-// to the kernel launchers, and the host-buffer end-to-end entry points. No arithmetic of the
-// method lives here.
+// nasg_api.cu — the extern "C" boundary declared in include/nasg.h: argument validation and dispatch
+// to the kernel launchers (the host-buffer end-to-end entry points live in nasg_host_pipeline.cu).
+// No arithmetic of the method lives here.
 #include "nasg.h"
 #include "nasg_internal.h"
 
@@ -14,7 +14,6 @@ thread_local cudaError_t t_last_cuda = cudaSuccess;
 
 inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 inline bool supported_K(int K) { return K == 1 || K == 2 || K == 3 || K == 4 || K == 5 || K == 8; }
-inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 // C <= 4 runs the persistent cp.async-pipelined kernels; NASG_FORCE_GENERIC=1 (debug/AB testing) or a
 // larger camera batch runs the generic ones.
