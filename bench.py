@@ -313,7 +313,7 @@ def run_ours(args, W, cfg):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=200)   # ~110 ms timed: long enough for the power cap to show
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (default 2 = headline)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
