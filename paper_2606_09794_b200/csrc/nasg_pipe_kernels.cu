@@ -13,6 +13,11 @@
 // (coalesced across the warp: quat/shape rows are float4 groups, amp/dc rows are planar).
 // Item stream of a thread: (Gaussian i, lobe l) in order; item j lives in ring slot j % RING; the
 // per-Gaussian header (mean, dc or g_colors) travels with lobe 0 into header slot i % HR.
+//
+// Two families: nasg_{fwd,bwd}_pipe_kernel (C = 1: scalar arithmetic) and nasg_{fwd,bwd}_pipe2_kernel
+// (C = 2..4: camera slots evaluated in pairs on packed f32x2 arithmetic, visibility bytes staged through
+// shared memory with cp.async, culled slots neutralised without a branch). MODE = normaliser / carrier mode
+// (include/nasg.h: 0 approximate, 1 exact eq.(10), 2 pure NASG), compiled in.
 #include "nasg_internal.h"
 #include "nasg_math.cuh"
 #include "pipe_common.cuh"
