@@ -130,6 +130,68 @@ def test_sh_full_size_sampled(B, W, oracle):
     torch.cuda.empty_cache()
 
 
+def test_indices_beyond_32_bits(B, W, oracle):
+    """Maximum sizes: K = 8, N = 70e6, C = 4 puts 2.24e9 elements (9 GB) in quat/shape — element indices
+    beyond 2^31 and byte offsets beyond 2^32 in every planar array. Inputs are drawn on the device (same
+    distributions as the base recipe); sampled Gaussians, incl. the last ones, are checked against the oracle."""
+    free, _ = torch.cuda.mem_get_info()
+    if free < 90e9:
+        pytest.skip("needs ~70 GB of device memory")
+    N, K, C = 70_000_000, 8, 4
+    gen = torch.Generator(device="cuda").manual_seed(1234)
+    rnd = lambda *shape: torch.rand(*shape, device="cuda", generator=gen)
+    nrm = lambda *shape: torch.randn(*shape, device="cuda", generator=gen)
+    d = {"means": rnd(N, 3) * 2 - 1, "quat": nrm(K, N, 4), "amp": nrm(K, 3, N) * 0.3, "dc": nrm(3, N) * 0.3,
+         "g_colors": nrm(C, N, 3), "vis": (rnd(C, N) < 0.6).to(torch.uint8)}
+    b = rnd(K, N, 2) * 5
+    d["shape"] = torch.stack([b.max(dim=2).values, b.min(dim=2).values, rnd(K, N) * 8, rnd(K, N) * 6.2831853], dim=2).contiguous()
+    del b
+    g3 = torch.randn(C, 3, generator=torch.Generator().manual_seed(7))
+    d["campos"] = (4 * g3 / g3.norm(dim=1, keepdim=True)).cuda()
+    assert d["quat"].numel() > 2**31
+    col, g = run_nasg(B, d, 1)
+    idx = torch.unique(torch.cat([torch.randint(0, N, (3000,)), torch.tensor([0, 1, 2**24, 2**26 + 5, N - 257, N - 2, N - 1])]))
+    ti = idx.cuda()
+    sub = {"N": int(idx.numel()), "K": K, "C": C, "campos": d["campos"].cpu().numpy(),
+           "means": d["means"][ti].cpu().numpy(), "quat": d["quat"][:, ti].cpu().numpy(), "shape": d["shape"][:, ti].cpu().numpy(),
+           "amp": d["amp"][:, :, ti].cpu().numpy(), "dc": d["dc"][:, ti].cpu().numpy(),
+           "g_colors": d["g_colors"][:, ti].cpu().numpy(), "vis": d["vis"][:, ti].cpu().numpy()}
+    sub = {k: (np.ascontiguousarray(v) if isinstance(v, np.ndarray) else v) for k, v in sub.items()}
+    rc, rg = oracle.nasg_fwd(sub, 1), oracle.nasg_bwd(sub, 1)
+    assert rel_err(col[:, ti], rc) <= FWD_TOL
+    assert rel_err(g["g_means"][ti], rg["g_means"]) <= BWD_TOL and rel_err(g["g_dc"][:, ti], rg["g_dc"]) <= BWD_TOL
+    assert rel_err(g["g_quat"][:, ti], rg["g_quat"]) <= BWD_TOL and rel_err(g["g_shape"][:, ti], rg["g_shape"]) <= BWD_TOL
+    assert rel_err(g["g_amp"][:, :, ti], rg["g_amp"]) <= BWD_TOL
+    del d, col, g
+    torch.cuda.empty_cache()
+
+
+def test_sh_indices_beyond_32_bits(B, W, oracle):
+    free, _ = torch.cuda.mem_get_info()
+    if free < 60e9:
+        pytest.skip("needs ~30 GB of device memory")
+    N, C = 50_000_000, 4                                   # coeffs: 2.4e9 elements, 9.6 GB
+    gen = torch.Generator(device="cuda").manual_seed(4321)
+    d = {"means": torch.rand(N, 3, device="cuda", generator=gen) * 2 - 1,
+         "coeffs": torch.randn(16, 3, N, device="cuda", generator=gen) * 0.2,
+         "g_colors": torch.randn(C, N, 3, device="cuda", generator=gen),
+         "vis": (torch.rand(C, N, device="cuda", generator=gen) < 0.6).to(torch.uint8)}
+    g3 = torch.randn(C, 3, generator=torch.Generator().manual_seed(8))
+    d["campos"] = (4 * g3 / g3.norm(dim=1, keepdim=True)).cuda()
+    assert d["coeffs"].numel() > 2**31
+    col, g = run_sh(B, d)
+    idx = torch.unique(torch.cat([torch.randint(0, N, (3000,)), torch.tensor([0, 2**25 + 3, N - 257, N - 1])]))
+    ti = idx.cuda()
+    sub = {"N": int(idx.numel()), "C": C, "campos": d["campos"].cpu().numpy(), "means": d["means"][ti].cpu().numpy(),
+           "coeffs": np.ascontiguousarray(d["coeffs"][:, :, ti].cpu().numpy()),
+           "g_colors": np.ascontiguousarray(d["g_colors"][:, ti].cpu().numpy()), "vis": np.ascontiguousarray(d["vis"][:, ti].cpu().numpy())}
+    rc, rg = oracle.sh_fwd(sub), oracle.sh_bwd(sub)
+    assert rel_err(col[:, ti], rc) <= FWD_TOL
+    assert rel_err(g["g_means"][ti], rg["g_means"]) <= BWD_TOL and rel_err(g["g_coeffs"][:, :, ti], rg["g_coeffs"]) <= BWD_TOL
+    del d, col, g
+    torch.cuda.empty_cache()
+
+
 # ---- edge cases -------------------------------------------------------------------------------
 @pytest.mark.parametrize("N", [1, 31, 255, 256, 257])
 def test_tiny_and_ragged_sizes(B, W, oracle, N):
