@@ -93,8 +93,8 @@ int nasg_eval_fwd(const nasg_inputs *in, float *colors, int norm_mode, void *cud
 
 /* Gradients of sum(g_colors[C,N,3] * colors) (Supplementary F + DESIGN.md §4). Nothing saved by the
  * forward is needed: the lobe values are recomputed. Each gradient element is written exactly once
- * by one thread (no atomics); g_campos is a warp-shuffle -> block -> second-stage reduction through
- * `workspace`, deterministic for a given N. */
+ * by one thread (no atomics); g_campos is a per-thread partial -> warp-shuffle -> block -> second-stage
+ * reduction through `workspace`, in a fixed order: bit-reproducible for a given N and device. */
 int nasg_eval_bwd(const nasg_inputs *in, const float *g_colors, const nasg_grads *out, int norm_mode,
                   void *cuda_stream);
 

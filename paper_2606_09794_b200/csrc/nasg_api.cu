@@ -86,12 +86,14 @@ int nasg_eval_bwd(const nasg_inputs *in, const float *g_colors, const nasg_grads
     }
     nasg::BwdParams p{in->N, in->C, in->means, in->quat, in->shape, in->amp, in->campos, in->vis, g_colors,
                       out->g_means, out->g_quat, out->g_shape, out->g_amp, out->g_dc, partial};
-    cudaError_t e = (use_pipe(in->C) && !partial) ? nasg::launch_nasg_bwd_pipe(p, in->K, norm_mode, st)
-                                                  : nasg::launch_nasg_bwd(p, in->K, norm_mode, st);
+    int pipe_blocks = 0;
+    const bool pipe = use_pipe(in->C);
+    cudaError_t e = pipe ? nasg::launch_nasg_bwd_pipe(p, in->K, norm_mode, st, &pipe_blocks)
+                         : nasg::launch_nasg_bwd(p, in->K, norm_mode, st);
     if (e != cudaSuccess) return cuda_fail(e);
     g_launches.fetch_add(1, std::memory_order_relaxed);
-    if (partial) {
-        e = nasg::launch_campos_reduce(partial, nasg::grid_blocks(in->N), in->C, out->g_campos, st);
+    if (partial) {      // second stage of g_campos: fixed-order sum of the per-block partials
+        e = nasg::launch_campos_reduce(partial, pipe ? pipe_blocks : nasg::grid_blocks(in->N), in->C, out->g_campos, st);
         if (e != cudaSuccess) return cuda_fail(e);
         g_launches.fetch_add(1, std::memory_order_relaxed);
     }

@@ -40,9 +40,9 @@ int64_t grid_blocks(int64_t N);
 int api_cuda_fail(cudaError_t e);     // remembers e for nasg_strerror(), returns NASG_ERR_CUDA (nasg_api.cu)
 cudaError_t launch_nasg_fwd(const FwdParams &p, int K, int mode, cudaStream_t st);
 cudaError_t launch_nasg_bwd(const BwdParams &p, int K, int mode, cudaStream_t st);
-// fast path (nasg_pipe_kernels.cu): C <= 4, persistent threads, cp.async lobe ring; no g_campos
+// fast path (nasg_pipe_kernels.cu): C <= 4, persistent threads, cp.async lobe ring
 cudaError_t launch_nasg_fwd_pipe(const FwdParams &p, int K, int mode, cudaStream_t st);
-cudaError_t launch_nasg_bwd_pipe(const BwdParams &p, int K, int mode, cudaStream_t st);
+cudaError_t launch_nasg_bwd_pipe(const BwdParams &p, int K, int mode, cudaStream_t st, int *grid_out);   // grid_out: blocks launched (= rows of cam_partial)
 cudaError_t launch_campos_reduce(const float *partial, int64_t nblocks, int C, float *out, cudaStream_t st);
 cudaError_t launch_sh_fwd(const ShParams &p, cudaStream_t st);
 cudaError_t launch_sh_bwd(const ShParams &p, cudaStream_t st);

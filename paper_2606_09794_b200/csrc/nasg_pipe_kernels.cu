@@ -260,7 +260,7 @@ __global__ void __launch_bounds__(PBLOCK, CT >= 3 ? 3 : 4) nasg_fwd_pipe2_kernel
 }
 
 // ---------------------------------------------------------------------------------------------
-// backward (no g_campos: that optional reduction stays on the generic kernel)
+// backward (g_campos, if asked for: per-thread partial over the thread's Gaussians -> block sum at the end)
 // ---------------------------------------------------------------------------------------------
 template <int K, int CT, int MODE>
 __global__ void __launch_bounds__(PBLOCK, 2) nasg_bwd_pipe_kernel(BwdParams p)
@@ -294,6 +294,9 @@ __global__ void __launch_bounds__(PBLOCK, 2) nasg_bwd_pipe_kernel(BwdParams p)
     for (int j = 0; j < DIST; ++j) prefetch_item(n + (j / K) * stride, j % K, j % RING, (j / K) % HR);
 
     unsigned sbase = 0, hs = 0;
+    float cam[CT][3];                 // this thread's share of g_campos (only if p.cam_partial): summed over its Gaussians
+#pragma unroll
+    for (int t = 0; t < CT; ++t) cam[t][0] = cam[t][1] = cam[t][2] = 0.f;
     unsigned mask = load_mask(p.vis, N, n, C);
     for (; n < N; n += stride) {
         const unsigned mask_next = load_mask(p.vis, N, n + stride, C);
@@ -384,23 +387,35 @@ __global__ void __launch_bounds__(PBLOCK, 2) nasg_bwd_pipe_kernel(BwdParams p)
                 st_cs(o, gw0); st_cs(o + N, gw1); st_cs(o + 2 * N, gw2);
             }
         }
-        if (p.g_means) {        // through d = Delta/|Delta|: (I - d d^T)/|Delta|
+        if (p.g_means || p.cam_partial) {        // through d = Delta/|Delta|: (I - d d^T)/|Delta|; g_campos gets minus the same
             float gm0 = 0.f, gm1 = 0.f, gm2 = 0.f;
 #pragma unroll
             for (int t = 0; t < CT; ++t) {
                 const float dg = fmaf(dx[t], gd[t][0], fmaf(dy[t], gd[t][1], dz[t] * gd[t][2]));
-                gm0 = fmaf(gd[t][0] - dx[t] * dg, idist[t], gm0);
-                gm1 = fmaf(gd[t][1] - dy[t] * dg, idist[t], gm1);
-                gm2 = fmaf(gd[t][2] - dz[t] * dg, idist[t], gm2);
+                const float t0 = (gd[t][0] - dx[t] * dg) * idist[t], t1 = (gd[t][1] - dy[t] * dg) * idist[t],
+                            t2 = (gd[t][2] - dz[t] * dg) * idist[t];
+                gm0 += t0; gm1 += t1; gm2 += t2;
+                cam[t][0] -= t0; cam[t][1] -= t1; cam[t][2] -= t2;
             }
-            float *o = p.g_means + 3 * n;
-            st_cs(o, gm0); st_cs(o + 1, gm1); st_cs(o + 2, gm2);
+            if (p.g_means) {
+                float *o = p.g_means + 3 * n;
+                st_cs(o, gm0); st_cs(o + 1, gm1); st_cs(o + 2, gm2);
+            }
         }
         sbase = (sbase + K) % RING;
         hs = (hs + 1) % HR;
         mask = mask_next;
     }
     cp_async_wait<0>();
+    if (p.cam_partial) {            // block partial of g_campos: warp shuffle -> shared memory -> fixed-order sum (deterministic)
+        __syncthreads();            // (every thread is done with the ring: reuse its first bytes)
+        float *red = reinterpret_cast<float *>(smem_raw);
+#pragma unroll
+        for (int t = 0; t < CT; ++t)
+            if (t < C)
+                for (int i = 0; i < 3; ++i)
+                    pipe_block_sum_store(cam[t][i], red, p.cam_partial + ((int64_t)blockIdx.x * C + t) * 3 + i);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -411,7 +426,9 @@ __device__ __forceinline__ float hsum(float2 a) { return a.x + a.y; }
 #ifndef NASG_BWD2_MINB
 #define NASG_BWD2_MINB 2
 #endif
-template <int K, int CT, int MODE>
+// CAMGRAD: also produce this block's partial of g_campos (compile-time: the extra code would cost the common
+// no-g_campos instantiation ~2 % through register allocation alone)
+template <int K, int CT, int MODE, bool CAMGRAD>
 __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(BwdParams p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -446,6 +463,14 @@ __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(
     for (int j = 0; j < DIST; ++j) prefetch_item(n + (j / K) * stride, j % K, j % RING, (j / K) % HR);
 
     unsigned sbase = 0, hs = 0;
+    // this thread's share of g_campos, 3 floats per camera slot, kept in shared memory (registers are the scarce
+    // resource here); the area exists only when the launcher was asked for g_campos
+    auto cam_acc = [&]() { return reinterpret_cast<float *>(vm + HR * 4 * PBLOCK) + 2 * NP * PBLOCK + tid; };
+    if (CAMGRAD) {
+        float *hc = cam_acc();
+#pragma unroll
+        for (int i = 0; i < 6 * NP; ++i) hc[i * PBLOCK] = 0.f;
+    }
     RawMask raw = {{0u, 0u, 0u, 0u}};
     if (!vis_cp) raw = load_raw_mask(p.vis, N, n, C);
     for (; n - (tid & 31) < N; n += stride) {       // warp-uniform trip count: lanes past N idle (mask 0, no stores)
@@ -562,7 +587,7 @@ __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(
                 st_cs(o, gw0); st_cs(o + N, gw1); st_cs(o + 2 * N, gw2);
             }
         }
-        if (p.g_means && valid) {        // through d = Delta/|Delta|: (I - d d^T)/|Delta|   (gd of a culled slot is exactly 0)
+        if ((p.g_means || CAMGRAD) && valid) {    // through d = Delta/|Delta|: (I - d d^T)/|Delta|   (gd of a culled slot is exactly 0)
             float2 gm0 = splat(0.f), gm1 = splat(0.f), gm2 = splat(0.f);
 #pragma unroll
             for (int j = 0; j < NP; ++j) {
@@ -572,15 +597,32 @@ __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(
                 gm0 = fma2(sub2(gd[j][0], mul2(dxj, dg)), idist, gm0);
                 gm1 = fma2(sub2(gd[j][1], mul2(dyj, dg)), idist, gm1);
                 gm2 = fma2(sub2(gd[j][2], mul2(dzj, dg)), idist, gm2);
+                if (CAMGRAD) {                                  // g_campos_c -= the same terms, per camera slot
+                    const float2 t0 = mul2(sub2(gd[j][0], mul2(dxj, dg)), idist), t1 = mul2(sub2(gd[j][1], mul2(dyj, dg)), idist),
+                                 t2 = mul2(sub2(gd[j][2], mul2(dzj, dg)), idist);
+                    float *c0 = cam_acc() + (6 * j) * PBLOCK, *c1 = c0 + 3 * PBLOCK;
+                    c0[0] -= t0.x; c0[PBLOCK] -= t1.x; c0[2 * PBLOCK] -= t2.x;
+                    c1[0] -= t0.y; c1[PBLOCK] -= t1.y; c1[2 * PBLOCK] -= t2.y;
+                }
             }
-            float *o = p.g_means + 3 * n;
-            st_cs(o, hsum(gm0)); st_cs(o + 1, hsum(gm1)); st_cs(o + 2, hsum(gm2));
+            if (p.g_means) {
+                float *o = p.g_means + 3 * n;
+                st_cs(o, hsum(gm0)); st_cs(o + 1, hsum(gm1)); st_cs(o + 2, hsum(gm2));
+            }
         }
         sbase = (sbase + K) % RING;
         hs = (hs + 1) % HR;
         raw = raw_next;
     }
     cp_async_wait<0>();
+    if (CAMGRAD) {                  // block partial of g_campos: warp shuffle -> shared memory -> fixed-order sum (deterministic)
+        __syncthreads();            // (every thread is done with the ring: reuse its first bytes)
+        float *red = reinterpret_cast<float *>(smem_raw);
+        const float *hc = cam_acc();
+        for (int t = 0; t < C; ++t)
+            for (int i = 0; i < 3; ++i)
+                pipe_block_sum_store(hc[(3 * t + i) * PBLOCK], red, p.cam_partial + ((int64_t)blockIdx.x * C + t) * 3 + i);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -625,39 +667,53 @@ cudaError_t launch_nasg_fwd_pipe(const FwdParams &p, int K, int mode, cudaStream
 }
 
 template <int K, int CT>
-static cudaError_t launch_bwd_pipe_kc(const BwdParams &p, int mode, cudaStream_t st)
+static cudaError_t launch_bwd_pipe_kc(const BwdParams &p, int mode, cudaStream_t st, int *grid_out)
 {
-    constexpr size_t smem = CT >= 2 ? pipe2_smem_bytes(PipeCfg<K>::HR, 3 + 3 * CT) + (size_t)PBLOCK * 4 * 2 * ((CT + 1) / 2) : pipe_smem_bytes(PipeCfg<K>::HR, 3 + 3 * CT);
+    const bool camgrad = p.cam_partial != nullptr;       // packed kernels: + 3 floats per camera slot and thread for g_campos
+    const size_t smem = CT >= 2 ? pipe2_smem_bytes(PipeCfg<K>::HR, 3 + 3 * CT) + (size_t)PBLOCK * 4 * (camgrad ? 8 : 2) * ((CT + 1) / 2)
+                                : pipe_smem_bytes(PipeCfg<K>::HR, 3 + 3 * CT);
     const dim3 block(PBLOCK);
-    static int cache[3][64] = {{0}};        // per (K, CT, norm mode) instantiation and device
+    static int cache_all[2][3][64] = {{{0}}};   // per (K, CT, g_campos, norm mode) instantiation and device
+    int (*cache)[64] = cache_all[camgrad ? 1 : 0];
     if constexpr (CT >= 2) {
-        if (mode == 1) nasg_bwd_pipe2_kernel<K, CT, 1><<<pipe_grid(nasg_bwd_pipe2_kernel<K, CT, 1>, smem, p.N, cache[1]), block, smem, st>>>(p);
-        else if (mode == 0) nasg_bwd_pipe2_kernel<K, CT, 0><<<pipe_grid(nasg_bwd_pipe2_kernel<K, CT, 0>, smem, p.N, cache[0]), block, smem, st>>>(p);
-        else nasg_bwd_pipe2_kernel<K, CT, 2><<<pipe_grid(nasg_bwd_pipe2_kernel<K, CT, 2>, smem, p.N, cache[2]), block, smem, st>>>(p);
+        if (camgrad) {
+            if (mode == 1) nasg_bwd_pipe2_kernel<K, CT, 1, true><<<pipe_grid(nasg_bwd_pipe2_kernel<K, CT, 1, true>, smem, p.N, cache[1]), block, smem, st>>>(p);
+            else if (mode == 0) nasg_bwd_pipe2_kernel<K, CT, 0, true><<<pipe_grid(nasg_bwd_pipe2_kernel<K, CT, 0, true>, smem, p.N, cache[0]), block, smem, st>>>(p);
+            else nasg_bwd_pipe2_kernel<K, CT, 2, true><<<pipe_grid(nasg_bwd_pipe2_kernel<K, CT, 2, true>, smem, p.N, cache[2]), block, smem, st>>>(p);
+        } else {
+            if (mode == 1) nasg_bwd_pipe2_kernel<K, CT, 1, false><<<pipe_grid(nasg_bwd_pipe2_kernel<K, CT, 1, false>, smem, p.N, cache[1]), block, smem, st>>>(p);
+            else if (mode == 0) nasg_bwd_pipe2_kernel<K, CT, 0, false><<<pipe_grid(nasg_bwd_pipe2_kernel<K, CT, 0, false>, smem, p.N, cache[0]), block, smem, st>>>(p);
+            else nasg_bwd_pipe2_kernel<K, CT, 2, false><<<pipe_grid(nasg_bwd_pipe2_kernel<K, CT, 2, false>, smem, p.N, cache[2]), block, smem, st>>>(p);
+        }
     } else {
         if (mode == 1) nasg_bwd_pipe_kernel<K, CT, 1><<<pipe_grid(nasg_bwd_pipe_kernel<K, CT, 1>, smem, p.N, cache[1]), block, smem, st>>>(p);
         else if (mode == 0) nasg_bwd_pipe_kernel<K, CT, 0><<<pipe_grid(nasg_bwd_pipe_kernel<K, CT, 0>, smem, p.N, cache[0]), block, smem, st>>>(p);
         else nasg_bwd_pipe_kernel<K, CT, 2><<<pipe_grid(nasg_bwd_pipe_kernel<K, CT, 2>, smem, p.N, cache[2]), block, smem, st>>>(p);
     }
+    int dev = 0;
+    cudaGetDevice(&dev);
+    const int64_t need = (p.N + PBLOCK - 1) / PBLOCK;
+    const int resident = cache[mode][(dev >= 0 && dev < 64) ? dev : 0];
+    *grid_out = (int)(need < resident ? need : resident);       // = the grid just launched (blocks of cam_partial written)
     return cudaGetLastError();
 }
 template <int K>
-static cudaError_t launch_bwd_pipe_k(const BwdParams &p, int mode, cudaStream_t st)
+static cudaError_t launch_bwd_pipe_k(const BwdParams &p, int mode, cudaStream_t st, int *grid_out)
 {
-    if (p.C == 1) return launch_bwd_pipe_kc<K, 1>(p, mode, st);
-    if (p.C == 2) return launch_bwd_pipe_kc<K, 2>(p, mode, st);
-    if (p.C == 3) return launch_bwd_pipe_kc<K, 3>(p, mode, st);
-    return launch_bwd_pipe_kc<K, 4>(p, mode, st);
+    if (p.C == 1) return launch_bwd_pipe_kc<K, 1>(p, mode, st, grid_out);
+    if (p.C == 2) return launch_bwd_pipe_kc<K, 2>(p, mode, st, grid_out);
+    if (p.C == 3) return launch_bwd_pipe_kc<K, 3>(p, mode, st, grid_out);
+    return launch_bwd_pipe_kc<K, 4>(p, mode, st, grid_out);
 }
-cudaError_t launch_nasg_bwd_pipe(const BwdParams &p, int K, int mode, cudaStream_t st)
+cudaError_t launch_nasg_bwd_pipe(const BwdParams &p, int K, int mode, cudaStream_t st, int *grid_out)
 {
     switch (K) {
-    case 1: return launch_bwd_pipe_k<1>(p, mode, st);
-    case 2: return launch_bwd_pipe_k<2>(p, mode, st);
-    case 3: return launch_bwd_pipe_k<3>(p, mode, st);
-    case 4: return launch_bwd_pipe_k<4>(p, mode, st);
-    case 5: return launch_bwd_pipe_k<5>(p, mode, st);
-    case 8: return launch_bwd_pipe_k<8>(p, mode, st);
+    case 1: return launch_bwd_pipe_k<1>(p, mode, st, grid_out);
+    case 2: return launch_bwd_pipe_k<2>(p, mode, st, grid_out);
+    case 3: return launch_bwd_pipe_k<3>(p, mode, st, grid_out);
+    case 4: return launch_bwd_pipe_k<4>(p, mode, st, grid_out);
+    case 5: return launch_bwd_pipe_k<5>(p, mode, st, grid_out);
+    case 8: return launch_bwd_pipe_k<8>(p, mode, st, grid_out);
     default: return cudaErrorInvalidValue;
     }
 }

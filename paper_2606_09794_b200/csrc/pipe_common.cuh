@@ -78,6 +78,24 @@ __device__ __forceinline__ unsigned staged_mask(const unsigned char *vm, int hsl
         if (c < C) m |= (vm[(hslot * 4 + c) * PBLOCK + tid] != 0 ? 1u : 0u) << c;
     return valid ? m : 0u;
 }
+// Sum `v` over the block (PBLOCK threads) in a fixed order and let thread 0 store it to *dst.
+// All threads of the block must call; `red` is PBLOCK/32 floats of shared memory.
+__device__ __forceinline__ void pipe_block_sum_store(float v, float *red, float *dst)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __syncthreads();
+    if (lane == 0) red[warp] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float s = 0.f;
+#pragma unroll
+        for (int w = 0; w < PBLOCK / 32; ++w) s += red[w];
+        *dst = s;
+    }
+}
+
 // Resident-grid size of a persistent kernel; the occupancy query and the shared-memory opt-in are done
 // once per (kernel instantiation, device) and cached (benign, idempotent state).
 template <typename Kernel>
