@@ -133,11 +133,13 @@ int sh_eval_bwd(int64_t N, int32_t C, const float *means, const float *coeffs, c
         partial = static_cast<float *>(workspace);
     }
     nasg::ShParams p{N, C, means, coeffs, campos, vis, g_colors, nullptr, g_means, g_coeffs, partial};
-    cudaError_t e = (use_pipe(C) && !partial) ? nasg::launch_sh_bwd_pipe(p, st) : nasg::launch_sh_bwd(p, st);
+    int pipe_blocks = 0;
+    const bool pipe = use_pipe(C);
+    cudaError_t e = pipe ? nasg::launch_sh_bwd_pipe(p, st, &pipe_blocks) : nasg::launch_sh_bwd(p, st);
     if (e != cudaSuccess) return cuda_fail(e);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     if (partial) {
-        e = nasg::launch_campos_reduce(partial, nasg::grid_blocks(N), C, g_campos, st);
+        e = nasg::launch_campos_reduce(partial, pipe ? pipe_blocks : nasg::grid_blocks(N), C, g_campos, st);
         if (e != cudaSuccess) return cuda_fail(e);
         g_launches.fetch_add(1, std::memory_order_relaxed);
     }

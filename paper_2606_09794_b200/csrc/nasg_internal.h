@@ -46,8 +46,8 @@ cudaError_t launch_nasg_bwd_pipe(const BwdParams &p, int K, int mode, cudaStream
 cudaError_t launch_campos_reduce(const float *partial, int64_t nblocks, int C, float *out, cudaStream_t st);
 cudaError_t launch_sh_fwd(const ShParams &p, cudaStream_t st);
 cudaError_t launch_sh_bwd(const ShParams &p, cudaStream_t st);
-// fast path (sh_pipe_kernels.cu): C <= 4, same persistent cp.async skeleton; no g_campos
+// fast path (sh_pipe_kernels.cu): C <= 4, same persistent cp.async skeleton
 cudaError_t launch_sh_fwd_pipe(const ShParams &p, cudaStream_t st);
-cudaError_t launch_sh_bwd_pipe(const ShParams &p, cudaStream_t st);
+cudaError_t launch_sh_bwd_pipe(const ShParams &p, cudaStream_t st, int *grid_out);
 
 } // namespace nasg

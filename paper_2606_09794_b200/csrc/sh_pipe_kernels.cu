@@ -202,7 +202,9 @@ __device__ __forceinline__ void sh_bwd_group(const float *slot, bool live, bool 
     }
 }
 
-template <int CT, bool COOP>
+// CAMGRAD: also produce this block's partial of g_campos (per-thread partial over the persistent loop, kept in
+// shared memory behind the staged visibility bytes; one block sum at the end of the kernel)
+template <int CT, bool COOP, bool CAMGRAD>
 __global__ void __launch_bounds__(PBLOCK, 2) sh_bwd_pipe_kernel(ShParams p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -235,6 +237,11 @@ __global__ void __launch_bounds__(PBLOCK, 2) sh_bwd_pipe_kernel(ShParams p)
     for (int j = 0; j < SH_DIST; ++j) prefetch_item(n, j, 0);
 
     unsigned hs = 0;
+    float *hc = reinterpret_cast<float *>(vm + SH_HR * 4 * PBLOCK) + tid;       // [3 CT][PBLOCK], CAMGRAD only
+    if (CAMGRAD) {
+#pragma unroll
+        for (int i = 0; i < 3 * CT; ++i) hc[i * PBLOCK] = 0.f;
+    }
     RawMask raw = {{0u, 0u, 0u, 0u}};
     if (!vis_cp) raw = load_raw_mask(p.vis, N, n, C);
     for (; n - (tid & 31) < N; n += stride) {
@@ -271,22 +278,38 @@ __global__ void __launch_bounds__(PBLOCK, 2) sh_bwd_pipe_kernel(ShParams p)
             if (g == 2) sh_bwd_group<2, CT>(slot, live, valid, p.g_coeffs, N, n, dx, dy, dz, gc, gd);
             if (g == 3) sh_bwd_group<3, CT>(slot, live, valid, p.g_coeffs, N, n, dx, dy, dz, gc, gd);
         }
-        if (p.g_means && valid) {        // through d = Delta/|Delta|: (I - d d^T)/|Delta|
+        if ((p.g_means || CAMGRAD) && valid) {        // through d = Delta/|Delta|: (I - d d^T)/|Delta|; g_campos gets minus the same
             float gm0 = 0.f, gm1 = 0.f, gm2 = 0.f;
 #pragma unroll
             for (int t = 0; t < CT; ++t) {
                 const float dg = fmaf(dx[t], gd[t][0], fmaf(dy[t], gd[t][1], dz[t] * gd[t][2]));
-                gm0 = fmaf(gd[t][0] - dx[t] * dg, idist[t], gm0);
-                gm1 = fmaf(gd[t][1] - dy[t] * dg, idist[t], gm1);
-                gm2 = fmaf(gd[t][2] - dz[t] * dg, idist[t], gm2);
+                if (CAMGRAD) {
+                    const float t0 = (gd[t][0] - dx[t] * dg) * idist[t], t1 = (gd[t][1] - dy[t] * dg) * idist[t],
+                                t2 = (gd[t][2] - dz[t] * dg) * idist[t];
+                    gm0 += t0; gm1 += t1; gm2 += t2;
+                    hc[(3 * t) * PBLOCK] -= t0; hc[(3 * t + 1) * PBLOCK] -= t1; hc[(3 * t + 2) * PBLOCK] -= t2;
+                } else {
+                    gm0 = fmaf(gd[t][0] - dx[t] * dg, idist[t], gm0);
+                    gm1 = fmaf(gd[t][1] - dy[t] * dg, idist[t], gm1);
+                    gm2 = fmaf(gd[t][2] - dz[t] * dg, idist[t], gm2);
+                }
             }
-            float *o = p.g_means + 3 * n;
-            st_cs(o, gm0); st_cs(o + 1, gm1); st_cs(o + 2, gm2);
+            if (p.g_means) {
+                float *o = p.g_means + 3 * n;
+                st_cs(o, gm0); st_cs(o + 1, gm1); st_cs(o + 2, gm2);
+            }
         }
         hs = (hs + 1) % SH_HR;
         raw = raw_next;
     }
     cp_async_wait<0>();
+    if (CAMGRAD) {                  // block partial: warp shuffle -> shared memory -> fixed-order sum (deterministic)
+        __syncthreads();            // (every thread is done with the ring: reuse its first bytes)
+        float *red = reinterpret_cast<float *>(smem_raw);
+        for (int t = 0; t < C; ++t)
+            for (int i = 0; i < 3; ++i)
+                pipe_block_sum_store(hc[(3 * t + i) * PBLOCK], red, p.cam_partial + ((int64_t)blockIdx.x * C + t) * 3 + i);
+    }
 }
 
 // ---- launchers --------------------------------------------------------------------------------
@@ -311,22 +334,34 @@ cudaError_t launch_sh_fwd_pipe(const ShParams &p, cudaStream_t st)
     }
 }
 template <int CT>
-static cudaError_t launch_sh_bwd_pipe_c(const ShParams &p, cudaStream_t st)
+static cudaError_t launch_sh_bwd_pipe_c(const ShParams &p, cudaStream_t st, int *grid_out)
 {
-    constexpr size_t smem = sh_pipe_smem_bytes(3 + 3 * CT);
-    static int cache[2][64] = {{0}};
+    const bool camgrad = p.cam_partial != nullptr;
+    const size_t smem = sh_pipe_smem_bytes(3 + 3 * CT) + (camgrad ? (size_t)PBLOCK * 4 * 3 * CT : 0);
+    static int cache[4][64] = {{0}};       // per (CT, cooperative copies, g_campos) instantiation and device
     const bool coop = (p.N & 3) == 0 && ptr_aligned16(p.coeffs) && ptr_aligned16(p.means) && ptr_aligned16(p.g_colors);
-    if (coop) sh_bwd_pipe_kernel<CT, true><<<pipe_grid(sh_bwd_pipe_kernel<CT, true>, smem, p.N, cache[1]), PBLOCK, smem, st>>>(p);
-    else sh_bwd_pipe_kernel<CT, false><<<pipe_grid(sh_bwd_pipe_kernel<CT, false>, smem, p.N, cache[0]), PBLOCK, smem, st>>>(p);
+    int *c = cache[(coop ? 1 : 0) + (camgrad ? 2 : 0)];
+    if (camgrad) {
+        if (coop) sh_bwd_pipe_kernel<CT, true, true><<<pipe_grid(sh_bwd_pipe_kernel<CT, true, true>, smem, p.N, c), PBLOCK, smem, st>>>(p);
+        else sh_bwd_pipe_kernel<CT, false, true><<<pipe_grid(sh_bwd_pipe_kernel<CT, false, true>, smem, p.N, c), PBLOCK, smem, st>>>(p);
+    } else {
+        if (coop) sh_bwd_pipe_kernel<CT, true, false><<<pipe_grid(sh_bwd_pipe_kernel<CT, true, false>, smem, p.N, c), PBLOCK, smem, st>>>(p);
+        else sh_bwd_pipe_kernel<CT, false, false><<<pipe_grid(sh_bwd_pipe_kernel<CT, false, false>, smem, p.N, c), PBLOCK, smem, st>>>(p);
+    }
+    int dev = 0;
+    cudaGetDevice(&dev);
+    const int64_t need = (p.N + PBLOCK - 1) / PBLOCK;
+    const int resident = c[(dev >= 0 && dev < 64) ? dev : 0];
+    *grid_out = (int)(need < resident ? need : resident);       // = the grid just launched (rows of cam_partial written)
     return cudaGetLastError();
 }
-cudaError_t launch_sh_bwd_pipe(const ShParams &p, cudaStream_t st)
+cudaError_t launch_sh_bwd_pipe(const ShParams &p, cudaStream_t st, int *grid_out)
 {
     switch (p.C) {
-    case 1: return launch_sh_bwd_pipe_c<1>(p, st);
-    case 2: return launch_sh_bwd_pipe_c<2>(p, st);
-    case 3: return launch_sh_bwd_pipe_c<3>(p, st);
-    case 4: return launch_sh_bwd_pipe_c<4>(p, st);
+    case 1: return launch_sh_bwd_pipe_c<1>(p, st, grid_out);
+    case 2: return launch_sh_bwd_pipe_c<2>(p, st, grid_out);
+    case 3: return launch_sh_bwd_pipe_c<3>(p, st, grid_out);
+    case 4: return launch_sh_bwd_pipe_c<4>(p, st, grid_out);
     default: return cudaErrorInvalidValue;
     }
 }

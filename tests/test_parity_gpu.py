@@ -192,6 +192,30 @@ def test_sh_indices_beyond_32_bits(B, W, oracle):
     torch.cuda.empty_cache()
 
 
+def test_generic_kernels_for_small_camera_counts_in_a_subprocess():
+    """C <= 4 always takes the persistent fast path; NASG_FORCE_GENERIC=1 (read once per process) routes it through
+    the generic one-thread-per-Gaussian kernels, which otherwise only serve C > 4. Same tolerances."""
+    import os, subprocess, sys, textwrap
+    code = textwrap.dedent("""
+        import sys; sys.path.insert(0, "tests"); sys.path.insert(0, ".")
+        from oracle import ref
+        from paper_2606_09794_b200 import binding as B, workloads as W
+        from gpu_util import check_nasg, check_sh
+        for mode in (1, 0, 2):
+            inp = W.make(2, 6001)
+            if mode == 2:
+                inp = dict(inp, shape=inp["shape"].copy()); inp["shape"][..., 2:] = 0
+            check_nasg(B, ref, inp, mode, want_campos=True, label=f"generic mode={mode}")
+        check_nasg(B, ref, W.make(1, 5003), 1, want_campos=True, label="generic C=1")
+        check_sh(B, ref, W.make(3, 6001), want_campos=True, label="generic sh")
+        print("GENERIC-OK")
+    """)
+    env = dict(os.environ, NASG_FORCE_GENERIC="1")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, "-c", code], cwd=root, env=env, capture_output=True, text=True, timeout=600)
+    assert out.returncode == 0 and "GENERIC-OK" in out.stdout, out.stdout[-2000:] + out.stderr[-2000:]
+
+
 # ---- edge cases -------------------------------------------------------------------------------
 @pytest.mark.parametrize("N", [1, 31, 255, 256, 257])
 def test_tiny_and_ragged_sizes(B, W, oracle, N):
