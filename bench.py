@@ -149,8 +149,21 @@ def cpu_baseline(W, cfg, target_s=12.0):
         dt = time.perf_counter() - t0
         if dt >= target_s or reps >= 64:
             break
-    return {"value": n * reps / dt, "unit": UNIT, "cores": ref.num_threads(), "kind": "oracle",
-            "sample": f"{n} Gaussians of {cfg.name} (same seeded recipe), fwd+bwd x {reps}, {dt:.2f} s, fp64 C -O2 OpenMP"}
+    cores = ref.num_threads()
+    # the same oracle on ONE thread, on a 1/16 prefix of the sample (both are reported)
+    n1 = max(1, n // 16)
+    inp1 = W.make(cfg.index, n1)
+    ref.set_num_threads(1)
+    t0 = time.perf_counter(); oracle_step(ref, W, inp1, cfg.kind); dt1 = time.perf_counter() - t0
+    ref.set_num_threads(cores)
+    try:
+        with open("/proc/cpuinfo") as f:
+            model = next((l.split(":", 1)[1].strip() for l in f if l.startswith("model name")), "unknown")
+    except Exception:
+        model = "unknown"
+    return {"value": n * reps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{n} Gaussians of {cfg.name} (same seeded recipe), fwd+bwd x {reps}, {dt:.2f} s, fp64 C -O2 OpenMP",
+            "single_thread_value": n1 / dt1, "cpu_model": model}
 
 
 def run_reference(args, W, cfg):

@@ -206,6 +206,15 @@ int nasg_ref_num_threads(void)
     return 1;
 #endif
 }
+/* timing harness only (bench.py: single-thread vs all-core baseline); no effect on any result */
+void nasg_ref_set_num_threads(int t)
+{
+#ifdef _OPENMP
+    if (t > 0) omp_set_num_threads(t);
+#else
+    (void)t;
+#endif
+}
 
 /* ------------------------------------------------------------------------------------------ */
 /* forward: colors[c,n,:] = c0 + sum_l w_l G_l(d_cn); culled entries 0                          */

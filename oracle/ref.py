@@ -50,6 +50,7 @@ def lib():
         L.nasg_ref_frame.argtypes = [dp, dp, dp]
         L.sh_ref_basis.argtypes = [dp, dp, dp]
         L.nasg_ref_num_threads.restype = i32
+        L.nasg_ref_set_num_threads.argtypes = [i32]
         for f in (L.nasg_ref_fwd, L.nasg_ref_bwd, L.sh_ref_fwd, L.sh_ref_bwd):
             f.restype = i32
         _lib = L
@@ -66,6 +67,11 @@ def _p(a: Optional[np.ndarray]):
 
 def num_threads() -> int:
     return int(lib().nasg_ref_num_threads())
+
+
+def set_num_threads(t: int) -> None:
+    """OpenMP threads of the following calls (timing harness only)."""
+    lib().nasg_ref_set_num_threads(int(t))
 
 
 def nasg_fwd(inp: dict, norm_mode: int = 1) -> np.ndarray:
