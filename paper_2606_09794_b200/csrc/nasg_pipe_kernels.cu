@@ -161,7 +161,7 @@ __global__ void __launch_bounds__(PBLOCK, CT >= 3 ? 3 : 4) nasg_fwd_pipe_kernel(
 
 // forward, two cameras per packed f32x2 instruction (CT >= 2)
 template <int K, int CT, int MODE>
-__global__ void __launch_bounds__(PBLOCK, CT >= 3 ? 3 : 4) nasg_fwd_pipe2_kernel(FwdParams p)
+__global__ void __launch_bounds__(PBLOCK, K <= 2 ? 2 : (CT >= 3 ? 3 : 4)) nasg_fwd_pipe2_kernel(FwdParams p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int HR = PipeCfg<K>::HR, HF = 6;
