@@ -29,8 +29,11 @@
  * overflows fp64 for Lambda > 709 (config 4 reaches Lambda = e^8); it is pinned against the literal
  * formula evaluated with 50-digit mpmath arithmetic.
  *
- * Parity unpinned: only the measure-zero points d = +-z (R11), where the paper's case split is
- * followed for the value and tau-dependent gradient terms are defined as 0.
+ * The measure-zero points d = +-z (R11) follow the paper's case split for the value; tau-dependent
+ * gradient terms are defined as 0 there, which is their limit at +z. Pinned by
+ * tests/test_oracle_pins.py::test_R11_* (case values of eq.(9), continuity of all seven partials at +z
+ * along both meridians, the X-meridian limit 0 and the Y-meridian limit e^{-2 lambda} H/I at -z).
+ * No function of this file is "parity unpinned".
  *
  * All arrays are fp64 host arrays (the harness promotes the fp32 inputs exactly). Layouts:
  *   means [N,3] quat [K,N,4] (w,x,y,z) shape [K,N,4] = (log Lambda, log lambda, k, phi)

@@ -28,7 +28,8 @@ constexpr int RING = 4;     // lobe slots per thread
 constexpr int DIST = 3;     // prefetch distance in lobes
 
 template <int K> struct PipeCfg {
-    static constexpr int HR = (K == 1) ? 4 : (K == 2) ? 3 : 2;   // header slots: Gaussians spanned by DIST lobes ahead, + 1
+    static constexpr int HR = (K == 1) ? 5 : (K <= 3) ? 3 : 2;   // header slots: Gaussians spanned by DIST lobes ahead, + 1 (K = 1, 3: + 1 more so that
+                                                                 // the l == 0 prefetch never targets the slot other lanes still read their visibility bytes from)
     static constexpr bool STATIC_SLOTS = (K % RING) == 0; // lobe l always lives in ring slot l % RING
 };
 
@@ -507,8 +508,15 @@ __global__ void __launch_bounds__(PBLOCK, NASG_BWD2_MINB) nasg_bwd_pipe2_kernel(
                     inv = mul2(inv, fma2(mul2(splat(-0.5f), r2), mul2(inv, inv), splat(1.5f)));
                     dx[j] = mul2(ex, inv); dy[j] = mul2(ey, inv); dz[j] = mul2(ez, inv);
                     hi[t0 * PBLOCK] = inv.x; hi[t1 * PBLOCK] = inv.y;
+                    // g_colors of a culled slot is never used (it may be NaN or uninitialised memory): the staged copy in this
+                    // thread's private header column is zeroed once, so that the per-lobe reads below need no select
+                    float *hw = r.h + (hs * HF) * PBLOCK + tid;
                     if (on0) { gdc0 += h[(3 + 3 * t0) * PBLOCK]; gdc1 += h[(4 + 3 * t0) * PBLOCK]; gdc2 += h[(5 + 3 * t0) * PBLOCK]; }
-                    if (t1 < CT && on1) { gdc0 += h[(3 + 3 * t1) * PBLOCK]; gdc1 += h[(4 + 3 * t1) * PBLOCK]; gdc2 += h[(5 + 3 * t1) * PBLOCK]; }
+                    else { hw[(3 + 3 * t0) * PBLOCK] = 0.f; hw[(4 + 3 * t0) * PBLOCK] = 0.f; hw[(5 + 3 * t0) * PBLOCK] = 0.f; }
+                    if (t1 < CT) {
+                        if (on1) { gdc0 += h[(3 + 3 * t1) * PBLOCK]; gdc1 += h[(4 + 3 * t1) * PBLOCK]; gdc2 += h[(5 + 3 * t1) * PBLOCK]; }
+                        else { hw[(3 + 3 * t1) * PBLOCK] = 0.f; hw[(4 + 3 * t1) * PBLOCK] = 0.f; hw[(5 + 3 * t1) * PBLOCK] = 0.f; }
+                    }
                     gd[j][0] = gd[j][1] = gd[j][2] = splat(0.f);
                 }
                 if (p.g_dc && valid) { st_cs(p.g_dc + n, gdc0); st_cs(p.g_dc + N + n, gdc1); st_cs(p.g_dc + 2 * N + n, gdc2); }

@@ -6,8 +6,8 @@ import numpy as np
 import pytest
 import torch
 
-from gpu_util import (BWD_TOL, FWD_TOL, NASG_KEYS, SH_KEYS, check_nasg, check_sh, rel_err, run_nasg, run_sh,
-                      to_dev)
+from gpu_util import (BWD_TOL, FWD_TOL, NASG_KEYS, SH_KEYS, check_nasg, check_sh, p99_rel, rel_err, run_nasg,
+                      run_sh, to_dev)
 
 pytestmark = pytest.mark.gpu
 
@@ -50,7 +50,7 @@ def test_pure_nasg_mode_ignores_the_carrier(B, W, oracle, cfg, N, K, C):
     rc, rg = oracle.nasg_fwd(zero, 0), oracle.nasg_bwd(zero, 0)
     assert np.abs(oracle.nasg_fwd(zero, 1) - rc).max() <= 1e-12 * np.abs(rc).max()
     d = to_dev(inp, NASG_KEYS)
-    for want_campos in (False, True):                       # fast path, then generic kernels
+    for want_campos in (False, True):                       # plain and g_campos variants (generic kernels for C > 4)
         col, g = run_nasg(B, d, 2, want_campos)
         assert rel_err(col, rc) <= FWD_TOL
         for k in ("g_means", "g_quat", "g_amp", "g_dc") + (("g_campos",) if want_campos else ()):
@@ -76,32 +76,35 @@ def test_sh_camera_tiles(B, W, oracle, C):
     check_sh(B, oracle, inp, want_campos=True, label=f"sh C={C}")
 
 
-# ---- full BASELINE sizes, launch configuration of bench.py: sampled outputs + size-independent properties ----
-def _sampled_check_nasg(B, W, oracle, cfg, n_sample=30_000):
+# ---- full BASELINE sizes, launch configuration of bench.py: EVERY element of EVERY output array ----
+def _report(label, errs, p99):
+    print(label, " ".join(f"{k}={errs[k]:.2e}(p99 {p99[k]:.1e})" for k in errs))
+
+
+def _full_check_nasg(B, W, oracle, cfg):
+    """All N Gaussians of the config against the oracle (seconds on the box's host cores), with g_campos — a global
+    fp32 sum over N terms that cannot be sampled. max-norm asserted at BASELINE's tolerances; the 99th-percentile
+    element-wise relative error is printed beside it."""
     inp = W.make(cfg)
     d = to_dev(inp, NASG_KEYS)
-    col, g = run_nasg(B, d, 1)
+    col, g = run_nasg(B, d, 1, want_campos=True)
+    _, g_nc = run_nasg(B, d, 1, want_campos=False)            # the launch bench.py times (no g_campos)
     N = inp["N"]
-    rng = np.random.default_rng(999 + cfg)
-    idx = np.unique(np.concatenate([rng.integers(0, N, n_sample), [0, 1, 255, 256, N - 257, N - 2, N - 1]]))
-    sub = W.take(inp, idx)
-    rc = oracle.nasg_fwd(sub, 1)
-    rg = oracle.nasg_bwd(sub, 1)
-    ti = torch.from_numpy(idx).cuda()
-    errs = {"colors": rel_err(col[:, ti], rc), "g_means": rel_err(g["g_means"][ti], rg["g_means"]),
-            "g_quat": rel_err(g["g_quat"][:, ti], rg["g_quat"]), "g_shape": rel_err(g["g_shape"][:, ti], rg["g_shape"]),
-            "g_amp": rel_err(g["g_amp"][:, :, ti], rg["g_amp"]), "g_dc": rel_err(g["g_dc"][:, ti], rg["g_dc"])}
-    print(f"cfg{cfg} full N={N} sampled {idx.size}:", " ".join(f"{k}={v:.2e}" for k, v in errs.items()))
+    rc = oracle.nasg_fwd(inp, 1)
+    errs, p99 = {"colors": rel_err(col, rc)}, {"colors": p99_rel(col, rc)}
+    del rc
+    rg = oracle.nasg_bwd(inp, 1)
+    for k in ("g_means", "g_quat", "g_shape", "g_amp", "g_dc", "g_campos"):
+        errs[k], p99[k] = rel_err(g[k], rg[k]), p99_rel(g[k], rg[k])
+        if k != "g_campos":
+            assert rel_err(g_nc[k], rg[k]) <= BWD_TOL, ("no-g_campos launch", k)
+    _report(f"cfg{cfg} full N={N} all elements:", errs, p99)
     assert errs.pop("colors") <= FWD_TOL
     for k, v in errs.items():
         assert v <= BWD_TOL, (k, v)
-    # properties that hold at any size
-    assert torch.isfinite(col).all() and all(torch.isfinite(v).all() for k, v in g.items())
     if d["vis"] is not None:
         v = d["vis"] != 0
         assert (col[~v] == 0).all()                                        # culled pairs are exactly 0
-        want_dc = (d["g_colors"] * v[:, :, None]).sum(0).T.contiguous()    # g_c0 = sum_c vis g_col
-        assert (g["g_dc"] - want_dc).abs().max() <= 1e-5 * want_dc.abs().max()
         dead = ~v.any(0)
         assert (g["g_means"][dead] == 0).all() and (g["g_quat"][:, dead] == 0).all() and (g["g_amp"][:, :, dead] == 0).all()
     else:
@@ -109,23 +112,23 @@ def _sampled_check_nasg(B, W, oracle, cfg, n_sample=30_000):
 
 
 @pytest.mark.parametrize("cfg", [1, 2, 4])
-def test_nasg_full_size_sampled(B, W, oracle, cfg):
-    _sampled_check_nasg(B, W, oracle, cfg)
+def test_nasg_full_size_every_element(B, W, oracle, cfg):
+    _full_check_nasg(B, W, oracle, cfg)
     torch.cuda.empty_cache()
 
 
-def test_sh_full_size_sampled(B, W, oracle):
+def test_sh_full_size_every_element(B, W, oracle):
     inp = W.make(3)
     d = to_dev(inp, SH_KEYS)
-    col, g = run_sh(B, d)
-    N = inp["N"]
-    idx = np.unique(np.concatenate([np.random.default_rng(1002).integers(0, N, 30_000), [0, 255, 256, N - 1]]))
-    sub = W.take(inp, idx)
-    rc, rg = oracle.sh_fwd(sub), oracle.sh_bwd(sub)
-    ti = torch.from_numpy(idx).cuda()
-    assert rel_err(col[:, ti], rc) <= FWD_TOL
-    assert rel_err(g["g_means"][ti], rg["g_means"]) <= BWD_TOL
-    assert rel_err(g["g_coeffs"][:, :, ti], rg["g_coeffs"]) <= BWD_TOL
+    col, g = run_sh(B, d, want_campos=True)
+    rc, rg = oracle.sh_fwd(inp), oracle.sh_bwd(inp)
+    errs, p99 = {"colors": rel_err(col, rc)}, {"colors": p99_rel(col, rc)}
+    for k in ("g_means", "g_coeffs", "g_campos"):
+        errs[k], p99[k] = rel_err(g[k], rg[k]), p99_rel(g[k], rg[k])
+    _report(f"cfg3 full N={inp['N']} all elements:", errs, p99)
+    assert errs.pop("colors") <= FWD_TOL
+    for k, v in errs.items():
+        assert v <= BWD_TOL, (k, v)
     assert (col[d["vis"] == 0] == 0).all()
     torch.cuda.empty_cache()
 
@@ -244,6 +247,33 @@ def test_all_culled_and_all_visible_masks(B, W, oracle):
     assert torch.equal(c1, c2) and all(torch.equal(g1[k], g2[k]) for k in g2)
 
 
+@pytest.mark.parametrize("C", [1, 2, 3, 4, 6])
+def test_g_colors_of_culled_pairs_are_never_read_as_values(B, W, oracle, C):
+    """include/nasg.h: g_colors[c,n,:] of a culled pair is ignored — it may be NaN, Inf or uninitialised memory
+    (a caller that fills only visible entries of a torch.empty buffer). Gradients must equal the oracle's on the
+    clean input; every kernel family (scalar, packed, generic; plain and g_campos variants; SH)."""
+    cfg = dataclasses.replace(W.CONFIGS[2], seed=900 + C, C=C)
+    inp = W.make_nasg(cfg, N=5_003)
+    rg = oracle.nasg_bwd(inp, 1)
+    bad = inp["g_colors"].copy()
+    culled = inp["vis"] == 0
+    bad[culled] = np.array([np.nan, np.inf, -np.inf], np.float32)
+    d = to_dev(dict(inp, g_colors=bad), NASG_KEYS)
+    for want_campos in (False, True):
+        _, g = run_nasg(B, d, 1, want_campos)
+        for k in ("g_means", "g_quat", "g_shape", "g_amp", "g_dc") + (("g_campos",) if want_campos else ()):
+            assert rel_err(g[k], rg[k]) <= BWD_TOL, (k, want_campos)
+    scfg = dataclasses.replace(W.CONFIGS[3], seed=900 + C, C=C)
+    sinp = W.make_sh(scfg, N=5_003)
+    srg = oracle.sh_bwd(sinp)
+    sbad = sinp["g_colors"].copy()
+    sbad[sinp["vis"] == 0] = np.nan
+    sd = to_dev(dict(sinp, g_colors=sbad), SH_KEYS)
+    _, sg = run_sh(B, sd, want_campos=True)
+    for k in ("g_means", "g_coeffs", "g_campos"):
+        assert rel_err(sg[k], srg[k]) <= BWD_TOL, k
+
+
 def test_optional_gradient_pointers_and_determinism(B, W):
     inp = W.make(2, 20_011)
     d = to_dev(inp, NASG_KEYS)
@@ -254,8 +284,7 @@ def test_optional_gradient_pointers_and_determinism(B, W):
     only = {"g_shape": torch.full_like(g_all["g_shape"], 7.0)}
     B.nasg_eval_bwd(d["means"], d["quat"], d["shape"], d["amp"], d["dc"], d["campos"], d["g_colors"], d["vis"], 1, out=only)
     torch.cuda.synchronize()
-    # (g_all came from the generic kernels, which g_campos selects; `only` from the fast path: same numbers up
-    # to summation order over the cameras, and the fast path is itself bit-reproducible)
+    # (g_all came from the g_campos variant of the fast-path kernel, `only` from the plain one: same arithmetic)
     assert (only["g_shape"] - g_all["g_shape"]).abs().max() <= 1e-5 * g_all["g_shape"].abs().max()
     again = {"g_shape": torch.full_like(g_all["g_shape"], 7.0)}
     B.nasg_eval_bwd(d["means"], d["quat"], d["shape"], d["amp"], d["dc"], d["campos"], d["g_colors"], d["vis"], 1, out=again)
