@@ -141,6 +141,13 @@ const char *nasg_version(void);
 /* Number of kernels the library has launched since load (all entry points; for bench accounting). */
 int64_t nasg_launch_count(void);
 
+/* Test hook: which kernel family the device entry points dispatch to. 0 (default) = automatic: the tile kernels
+ * (even K, C <= 4, N % 4 == 0 — N % 16 == 0 with a mask —, 16-byte aligned arrays, no g_campos), else the
+ * cp.async ring kernels (C <= 4), else the generic kernels; 1 = generic kernels only; 2 = never the tile kernels.
+ * Process-wide; exists so that the parity tests can compare every family with the oracle on the same inputs.
+ * The library never reads the environment. */
+void nasg_debug_set_path(int path);
+
 #ifdef __cplusplus
 }
 #endif

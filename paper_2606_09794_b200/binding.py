@@ -21,7 +21,7 @@ NORM_APPROX, NORM_EXACT, NORM_NASG = 0, 1, 2
 MAX_CAMERAS = 64
 SYMBOLS = ("nasg_eval_fwd", "nasg_eval_bwd", "sh_eval_fwd", "sh_eval_bwd", "nasg_workspace_bytes",
            "nasg_host_scratch_bytes", "nasg_eval_fwd_bwd_host", "sh_host_scratch_bytes",
-           "sh_eval_fwd_bwd_host", "nasg_strerror", "nasg_version", "nasg_launch_count")
+           "sh_eval_fwd_bwd_host", "nasg_strerror", "nasg_version", "nasg_launch_count", "nasg_debug_set_path")
 
 
 class NasgError(RuntimeError):
@@ -70,6 +70,8 @@ def _load():
     lib.nasg_strerror.restype = C.c_char_p
     lib.nasg_version.restype = C.c_char_p
     lib.nasg_launch_count.restype = i64
+    lib.nasg_debug_set_path.argtypes = [C.c_int]
+    lib.nasg_debug_set_path.restype = None
     for name in ("nasg_eval_fwd", "nasg_eval_bwd", "sh_eval_fwd", "sh_eval_bwd", "nasg_eval_fwd_bwd_host",
                  "sh_eval_fwd_bwd_host"):
         getattr(lib, name).restype = C.c_int
@@ -90,6 +92,11 @@ def nasg_version() -> str:
 
 def nasg_launch_count() -> int:
     return int(_lib.nasg_launch_count())
+
+
+def nasg_debug_set_path(path: int) -> None:
+    """Test hook (include/nasg.h): 0 = automatic dispatch, 1 = generic kernels only, 2 = never the tile kernels."""
+    _lib.nasg_debug_set_path(int(path))
 
 
 def nasg_workspace_bytes(N: int, K: int, Cn: int) -> int:

@@ -5,7 +5,6 @@
 #include "nasg_internal.h"
 
 #include <atomic>
-#include <cstdlib>
 
 namespace {
 
@@ -15,13 +14,12 @@ thread_local cudaError_t t_last_cuda = cudaSuccess;
 inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 inline bool supported_K(int K) { return K == 1 || K == 2 || K == 3 || K == 4 || K == 5 || K == 8; }
 
-// C <= 4 runs the persistent cp.async-pipelined kernels; NASG_FORCE_GENERIC=1 (debug/AB testing) or a
-// larger camera batch runs the generic ones.
-bool use_pipe(int C)
-{
-    static const bool force_generic = [] { const char *e = getenv("NASG_FORCE_GENERIC"); return e && e[0] == '1'; }();
-    return C <= 4 && !force_generic;
-}
+// Kernel family: 0 = automatic (tile kernels when their conditions hold, else the cp.async ring kernels for C <= 4,
+// else the generic kernels); 1 = generic only; 2 = no tile kernels. Set by nasg_debug_set_path() (a test hook, so
+// that every family can be compared with the oracle on the same inputs); never read from the environment.
+std::atomic<int> g_path{0};
+bool use_pipe(int C) { return C <= 4 && g_path.load(std::memory_order_relaxed) != 1; }
+bool use_tile() { return g_path.load(std::memory_order_relaxed) == 0; }
 
 int cuda_fail(cudaError_t e) { t_last_cuda = e; return NASG_ERR_CUDA; }
 
@@ -54,8 +52,12 @@ int nasg_eval_fwd(const nasg_inputs *in, float *colors, int norm_mode, void *cud
     if (!colors) return NASG_ERR_NULL;
     if (!aligned16(in->quat) || !aligned16(in->shape)) return NASG_ERR_ALIGN;
     nasg::FwdParams p{in->N, in->C, in->means, in->quat, in->shape, in->amp, in->dc, in->campos, in->vis, colors};
-    cudaError_t e = use_pipe(in->C) ? nasg::launch_nasg_fwd_pipe(p, in->K, norm_mode, (cudaStream_t)cuda_stream)
-                                    : nasg::launch_nasg_fwd(p, in->K, norm_mode, (cudaStream_t)cuda_stream);
+    cudaError_t e;
+    if (use_tile() && nasg::tile_path_ok(in->N, in->K, in->C, in->means, in->amp, in->dc, nullptr, in->vis))
+        e = nasg::launch_nasg_fwd_tile(p, in->K, norm_mode, (cudaStream_t)cuda_stream);
+    else
+        e = use_pipe(in->C) ? nasg::launch_nasg_fwd_pipe(p, in->K, norm_mode, (cudaStream_t)cuda_stream)
+                            : nasg::launch_nasg_fwd(p, in->K, norm_mode, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return cuda_fail(e);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     return NASG_OK;
@@ -88,8 +90,11 @@ int nasg_eval_bwd(const nasg_inputs *in, const float *g_colors, const nasg_grads
                       out->g_means, out->g_quat, out->g_shape, out->g_amp, out->g_dc, partial};
     int pipe_blocks = 0;
     const bool pipe = use_pipe(in->C);
-    cudaError_t e = pipe ? nasg::launch_nasg_bwd_pipe(p, in->K, norm_mode, st, &pipe_blocks)
-                         : nasg::launch_nasg_bwd(p, in->K, norm_mode, st);
+    cudaError_t e;
+    if (!partial && use_tile() && nasg::tile_path_ok(in->N, in->K, in->C, in->means, in->amp, nullptr, g_colors, in->vis))
+        e = nasg::launch_nasg_bwd_tile(p, in->K, norm_mode, st);
+    else
+        e = pipe ? nasg::launch_nasg_bwd_pipe(p, in->K, norm_mode, st, &pipe_blocks) : nasg::launch_nasg_bwd(p, in->K, norm_mode, st);
     if (e != cudaSuccess) return cuda_fail(e);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     if (partial) {      // second stage of g_campos: fixed-order sum of the per-block partials
@@ -171,5 +176,7 @@ const char *nasg_strerror(int code)
 const char *nasg_version(void) { return "0.1.0 sm_100a"; }
 
 int64_t nasg_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+void nasg_debug_set_path(int path) { g_path.store(path < 0 || path > 2 ? 0 : path, std::memory_order_relaxed); }
 
 } // extern "C"

@@ -195,28 +195,38 @@ def test_sh_indices_beyond_32_bits(B, W, oracle):
     torch.cuda.empty_cache()
 
 
-def test_generic_kernels_for_small_camera_counts_in_a_subprocess():
-    """C <= 4 always takes the persistent fast path; NASG_FORCE_GENERIC=1 (read once per process) routes it through
-    the generic one-thread-per-Gaussian kernels, which otherwise only serve C > 4. Same tolerances."""
-    import os, subprocess, sys, textwrap
-    code = textwrap.dedent("""
-        import sys; sys.path.insert(0, "tests"); sys.path.insert(0, ".")
-        from oracle import ref
-        from paper_2606_09794_b200 import binding as B, workloads as W
-        from gpu_util import check_nasg, check_sh
+@pytest.mark.parametrize("path", [1, 2])
+def test_every_kernel_family_on_the_same_inputs(B, W, oracle, path):
+    """Automatic dispatch picks the tile kernels (even K, C <= 4, aligned N), else the cp.async ring kernels, else the
+    generic one-thread-per-Gaussian kernels. nasg_debug_set_path (a test hook of the C ABI) forces 1 = generic only,
+    2 = never the tile kernels, so that every family meets the same tolerances on inputs the tile path would take."""
+    B.nasg_debug_set_path(path)
+    try:
         for mode in (1, 0, 2):
-            inp = W.make(2, 6001)
+            inp = W.make(2, 6016)
             if mode == 2:
                 inp = dict(inp, shape=inp["shape"].copy()); inp["shape"][..., 2:] = 0
-            check_nasg(B, ref, inp, mode, want_campos=True, label=f"generic mode={mode}")
-        check_nasg(B, ref, W.make(1, 5003), 1, want_campos=True, label="generic C=1")
-        check_sh(B, ref, W.make(3, 6001), want_campos=True, label="generic sh")
-        print("GENERIC-OK")
-    """)
-    env = dict(os.environ, NASG_FORCE_GENERIC="1")
-    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-    out = subprocess.run([sys.executable, "-c", code], cwd=root, env=env, capture_output=True, text=True, timeout=600)
-    assert out.returncode == 0 and "GENERIC-OK" in out.stdout, out.stdout[-2000:] + out.stderr[-2000:]
+            check_nasg(B, oracle, inp, mode, want_campos=True, label=f"path={path} mode={mode}")
+        check_nasg(B, oracle, W.make(1, 5008), 1, want_campos=True, label=f"path={path} C=1")
+        check_nasg(B, oracle, W.make(4, 4000), 1, want_campos=True, label=f"path={path} K=8")
+        check_sh(B, oracle, W.make(3, 6016), want_campos=True, label=f"path={path} sh")
+    finally:
+        B.nasg_debug_set_path(0)
+
+
+@pytest.mark.parametrize("K", [2, 4, 8])
+@pytest.mark.parametrize("C", [1, 2, 3, 4])
+@pytest.mark.parametrize("mode", [1, 0, 2])
+def test_tile_kernels_all_instantiations(B, W, oracle, K, C, mode):
+    """Tile path (N % 16 == 0): every compiled (K, C, mode), several tiles per block and a partial last tile; with and
+    without a visibility mask."""
+    cfg = dataclasses.replace(W.CONFIGS[2], seed=400 + K * 10 + C, K=K, C=C)
+    N = 256 * 1300 + 48 if (K, C, mode) == (4, 4, 1) else 256 * 9 + 48
+    inp = W.make_nasg(cfg, N=N)
+    if mode == 2:
+        inp = dict(inp, shape=inp["shape"].copy()); inp["shape"][..., 2:] = 0
+    check_nasg(B, oracle, inp, mode, label=f"tile K={K} C={C} mode={mode}")
+    check_nasg(B, oracle, dict(inp, vis=None), mode, label=f"tile K={K} C={C} mode={mode} no mask")
 
 
 # ---- edge cases -------------------------------------------------------------------------------
@@ -237,7 +247,7 @@ def test_empty_input_is_a_noop(B):
 
 
 def test_all_culled_and_all_visible_masks(B, W, oracle):
-    inp = W.make(2, 1_500)
+    inp = W.make(2, 1_504)          # N % 16 == 0: the masked and the NULL-mask call take the same kernel family
     dead = dict(inp, vis=np.zeros_like(inp["vis"]))
     col, g, _ = check_nasg(B, oracle, dead, 1, want_campos=True, label="all culled")
     assert (col == 0).all() and all((g[k] == 0).all() for k in ("g_means", "g_quat", "g_shape", "g_amp", "g_dc", "g_campos"))
