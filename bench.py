@@ -49,25 +49,6 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
-def alu_floor_ms(workload: str, N: int, sms: int, sm_hz: float):
-    """Issue-side floor of the dominant kernel from the committed ncu counts (None if not recorded)."""
-    try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            cyc = json.load(f).get("alu_cycles_per_warp_gaussian_bwd", {}).get(workload)
-        return None if cyc is None else 1e3 * (N / 32.0) * cyc / (sms * 4 * sm_hz)
-    except Exception:
-        return None
-
-
-def recorded_traffic(workload: str):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture."""
-    try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            return json.load(f).get(workload)
-    except Exception:
-        return None
-
-
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -190,8 +171,88 @@ def run_reference(args, W, cfg):
 
 
 # ---- the CUDA arm ---------------------------------------------------------------------------------
+class Resident:
+    """One config resident in HBM (this rank's shard) with its fwd() / bwd() launches through the C-ABI binding."""
+
+    def __init__(self, B, W, S, cfg, rank, layout, norm_mode):
+        import numpy as np
+        import torch
+        self.B, self.cfg, self.norm_mode, self.torch = B, cfg, norm_mode, torch
+        rcfg = S.weak_scaling_config(cfg, rank)
+        inp = W.make_sh(rcfg) if cfg.kind == "sh" else W.make_nasg(rcfg)
+        self.N, self.C, self.K = inp["N"], inp["C"], inp.get("K", 0)
+        # tile-record parameter layout (include/nasg.h: nasg_rec_*) where it applies, else the row arrays
+        self.rec = cfg.kind == "nasg" and layout == "rec" and self.K in (2, 4, 8) and self.C <= 4
+        self.keys = ("means", "coeffs", "campos", "vis", "g_colors") if cfg.kind == "sh" else \
+                    ("means", "quat", "shape", "amp", "dc", "campos", "vis", "g_colors")
+        d = {k: (None if inp.get(k) is None else torch.from_numpy(np.ascontiguousarray(inp[k])).cuda()) for k in self.keys}
+        self.d = d
+        self.colors = torch.empty((self.C, self.N, 3), dtype=torch.float32, device="cuda")
+        self.stream = torch.cuda.current_stream()
+        if self.rec:    # the parameters LIVE in HBM as records (packed once, outside any timed region: it is the storage layout)
+            self.params = B.nasg_rec_pack(d["means"], d["quat"], d["shape"], d["amp"], d["dc"])
+            self.g_params = torch.zeros_like(self.params)
+            for k in ("means", "quat", "shape", "amp", "dc"):
+                d[k] = None
+        else:
+            self.grads = B.sh_alloc_grads(self.N, self.C, "cuda") if cfg.kind == "sh" else B.nasg_alloc_grads(self.K, self.N, self.C, "cuda")
+        self.has_vis = d["vis"] is not None
+
+    def fwd(self):
+        B, d, st = self.B, self.d, self.stream
+        if self.rec:
+            B.nasg_rec_eval_fwd(self.params, self.N, self.K, d["campos"], d["vis"], self.norm_mode, out=self.colors, stream=st)
+        elif self.cfg.kind == "sh":
+            B.sh_eval_fwd(d["means"], d["coeffs"], d["campos"], d["vis"], out=self.colors, stream=st)
+        else:
+            B.nasg_eval_fwd(d["means"], d["quat"], d["shape"], d["amp"], d["dc"], d["campos"], d["vis"], self.norm_mode,
+                            out=self.colors, stream=st)
+
+    def bwd(self):
+        B, d, st = self.B, self.d, self.stream
+        if self.rec:
+            B.nasg_rec_eval_bwd(self.params, self.N, self.K, d["campos"], d["g_colors"], d["vis"], self.norm_mode,
+                                out=self.g_params, stream=st)
+        elif self.cfg.kind == "sh":
+            B.sh_eval_bwd(d["means"], d["coeffs"], d["campos"], d["g_colors"], d["vis"], out=self.grads, stream=st)
+        else:
+            B.nasg_eval_bwd(d["means"], d["quat"], d["shape"], d["amp"], d["dc"], d["campos"], d["g_colors"],
+                            d["vis"], self.norm_mode, out=self.grads, stream=st)
+
+    def kernel_name(self):
+        if self.rec:
+            return "nasg_rec_bwd_kernel"
+        pipe = self.C <= 4
+        if self.cfg.kind == "sh":
+            return "sh_bwd_pipe_kernel" if pipe else "sh_bwd_kernel"
+        tile = self.K % 2 == 0 and pipe and self.N % (16 if self.has_vis else 4) == 0
+        return "nasg_bwd_tile_kernel" if tile else ("nasg_bwd_pipe2_kernel" if self.C >= 2 else "nasg_bwd_pipe_kernel") if pipe else "nasg_bwd_kernel"
+
+    def timed(self, steps, warmup, barrier):
+        """`warmup` untimed steps, then `steps` timed ones (CUDA events on the launching stream, barrier + synchronize on
+        both sides). Returns mean fwd ms, mean bwd ms, total ms of the timed region."""
+        torch = self.torch
+        for _ in range(warmup):
+            self.fwd(); self.bwd()
+        barrier()
+        ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
+        for s in range(steps):
+            ev[s][0].record(self.stream); self.fwd(); ev[s][1].record(self.stream); self.bwd(); ev[s][2].record(self.stream)
+        barrier()
+        return (sum(e[0].elapsed_time(e[1]) for e in ev) / steps, sum(e[1].elapsed_time(e[2]) for e in ev) / steps,
+                ev[0][0].elapsed_time(ev[-1][2]))
+
+
+def recorded(workload: str, key: str):
+    """A figure of the committed ncu captures (profiles/traffic.json: which capture and commit is stated there)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            return json.load(f).get(key, {}).get(workload)
+    except Exception:
+        return None
+
+
 def run_ours(args, W, cfg):
-    import numpy as np
     import torch
     import torch.distributed as dist
     from paper_2606_09794_b200 import binding as B        # fails loudly if the CUDA library is missing
@@ -206,63 +267,42 @@ def run_ours(args, W, cfg):
     # each rank owns a shard of independent Gaussians (weak scaling: the per-GPU shard is the config's N;
     # rank r draws its shard from seed + 1000 r). No data-path collective: the path is per-Gaussian.
     from paper_2606_09794_b200 import sharding as S
-    rcfg = S.weak_scaling_config(cfg, rank)
-    inp = W.make_sh(rcfg) if cfg.kind == "sh" else W.make_nasg(rcfg)
-    N, C, K = inp["N"], inp["C"], inp.get("K", 0)
-    keys = ("means", "coeffs", "campos", "vis", "g_colors") if cfg.kind == "sh" else \
-           ("means", "quat", "shape", "amp", "dc", "campos", "vis", "g_colors")
-    d = {k: (None if inp.get(k) is None else torch.from_numpy(np.ascontiguousarray(inp[k])).cuda()) for k in keys}
-    colors = torch.empty((C, N, 3), dtype=torch.float32, device="cuda")
-    grads = B.sh_alloc_grads(N, C, "cuda") if cfg.kind == "sh" else B.nasg_alloc_grads(K, N, C, "cuda")
-    stream = torch.cuda.current_stream()
-
-    def fwd():
-        if cfg.kind == "sh":
-            B.sh_eval_fwd(d["means"], d["coeffs"], d["campos"], d["vis"], out=colors, stream=stream)
-        else:
-            B.nasg_eval_fwd(d["means"], d["quat"], d["shape"], d["amp"], d["dc"], d["campos"], d["vis"], args.norm_mode,
-                            out=colors, stream=stream)
-
-    def bwd():
-        if cfg.kind == "sh":
-            B.sh_eval_bwd(d["means"], d["coeffs"], d["campos"], d["g_colors"], d["vis"], out=grads, stream=stream)
-        else:
-            B.nasg_eval_bwd(d["means"], d["quat"], d["shape"], d["amp"], d["dc"], d["campos"], d["g_colors"],
-                            d["vis"], args.norm_mode, out=grads, stream=stream)
+    R = Resident(B, W, S, cfg, rank, args.layout, args.norm_mode)
+    N, C, K, rec, d, stream = R.N, R.C, R.K, R.rec, R.d, R.stream
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
-        fwd(); bwd()
-    barrier()
-    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
-    launches0 = B.nasg_launch_count()
+    warm = max(args.warmup, 3)
+    launches0 = None
     with ClockSampler(local) as clocks:
+        for _ in range(warm):
+            R.fwd(); R.bwd()
         barrier()
+        launches0 = B.nasg_launch_count()
         t_wall = time.perf_counter()
-        for s in range(args.steps):
-            ev[s][0].record(stream); fwd(); ev[s][1].record(stream); bwd(); ev[s][2].record(stream)
-        barrier()
+        fwd_ms, bwd_ms, total_ms = R.timed(args.steps, 0, barrier)
         timed_wall = time.perf_counter() - t_wall
         launches = B.nasg_launch_count() - launches0          # kernels launched inside the timed region
-        # the timed region is short (ms): keep the identical load running, untimed, until nvidia-smi
-        # (50 ms period) has had ~1 s to sample clocks and throttle reasons under this load
+        # the timed region is short: keep the identical load running, untimed, until nvidia-smi (50 ms period) has had
+        # ~1 s to sample clocks and throttle reasons under this load
         while time.perf_counter() - t_wall < 1.0:
             for _ in range(20):
-                fwd(); bwd()
+                R.fwd(); R.bwd()
             torch.cuda.synchronize()
-    total_ms = ev[0][0].elapsed_time(ev[-1][2])
-    fwd_ms = sum(e[0].elapsed_time(e[1]) for e in ev) / args.steps
-    bwd_ms = sum(e[1].elapsed_time(e[2]) for e in ev) / args.steps
     total_ms = S.max_over_ranks(total_ms, "cuda")
     value = world * N * args.steps / (total_ms * 1e-3)
 
     # ---- end to end through the host-buffer C-ABI entry point (pinned host memory) -----------------
-    host = {k: (None if d[k] is None else d[k].cpu().pin_memory()) for k in keys}
-    if cfg.kind == "sh":
+    host = {k: (None if d[k] is None else d[k].cpu().pin_memory()) for k in R.keys}
+    if rec:
+        host["params"] = R.params.cpu().pin_memory()
+        hout = dict(colors=torch.empty((C, N, 3)).pin_memory(), g_params=torch.empty(R.params.numel()).pin_memory())
+        scratch = torch.empty(B.nasg_rec_host_scratch_bytes(N, K, C), dtype=torch.uint8, device="cuda")
+        e2e_call = lambda: B.nasg_rec_eval_fwd_bwd_host(host, hout, N, K, scratch, args.norm_mode, stream=stream)
+    elif cfg.kind == "sh":
         hout = dict(colors=torch.empty((C, N, 3)).pin_memory(), g_means=torch.empty((N, 3)).pin_memory(),
                     g_coeffs=torch.empty((16, 3, N)).pin_memory())
         scratch = torch.empty(B.sh_host_scratch_bytes(N, C), dtype=torch.uint8, device="cuda")
@@ -283,39 +323,79 @@ def run_ours(args, W, cfg):
         e2e_call()
     e1.record(stream)
     barrier()
-    e2e_value = world * N * e2e_steps / (S.max_over_ranks(e0.elapsed_time(e1), "cuda") * 1e-3)
+    e2e_ms = S.max_over_ranks(e0.elapsed_time(e1), "cuda") / e2e_steps
+    e2e_value = world * N / (e2e_ms * 1e-3)
+    del host, hout, scratch
+
+    peak, peak_src = measured_peak()
+
+    def summary(r, f_ms, b_ms):
+        fb, bb = algorithmic_bytes(r.cfg.kind, r.K, r.C, r.has_vis)
+        return {"layout": "records" if r.rec else "rows", "kernel": r.kernel_name(), "fwd_ms": f_ms, "bwd_ms": b_ms,
+                "value": r.N / ((f_ms + b_ms) * 1e-3), "fwd_gbs": fb * r.N / (f_ms * 1e-3) / 1e9, "bwd_gbs": bb * r.N / (b_ms * 1e-3) / 1e9,
+                "bwd_frac": bb * r.N / (b_ms * 1e-3) / 1e9 / peak, "fwd+bwd_frac": (fb + bb) * r.N / ((f_ms + b_ms) * 1e-3) / 1e9 / peak}
+
+    # ---- the sustained figure, and the other configs in the same run (rank 0, one GPU) -----------------
+    extra = {}
+    if world == 1 and not args.no_others:
+        f2, b2, t2 = R.timed(1000, 0, barrier)                 # ~0.5 s of back-to-back steps: the board's power cap bites
+        extra["sustained"] = {"steps": 1000, "value": N * 1000 / (t2 * 1e-3), "fwd_ms": f2, "bwd_ms": b2}
+        others = {}
+        main_summary = summary(R, fwd_ms, bwd_ms)
+        specs = [(i, "rec") for i in (1, 2, 3, 4) if i != cfg.index]
+        if rec:
+            specs.append((cfg.index, "rows"))                  # the same workload through the row-array entry points
+        R_keep, R = R, None
+        if cfg.N > 2_000_000:
+            R_keep.d = None; R_keep.params = None; R_keep.g_params = None; R_keep.colors = None
+            torch.cuda.empty_cache()
+        for i, layout in specs:
+            r = Resident(B, W, S, W.CONFIGS[i], 0, layout, args.norm_mode)
+            f_ms, b_ms, _ = r.timed(20, 5, barrier)
+            others[("cfg%d" % i) + ("" if layout == "rec" else " rows")] = dict(summary(r, f_ms, b_ms), workload=W.CONFIGS[i].name, steps=20)
+            del r
+            torch.cuda.empty_cache()
+        extra["other_configs"] = others
+        R = R_keep
 
     if rank == 0:
-        fb, bb = algorithmic_bytes(cfg.kind, K, C, d["vis"] is not None)
-        peak, peak_src = measured_peak()
+        fb, bb = algorithmic_bytes(cfg.kind, K, C, R.has_vis)
         achieved = bb * N / (bwd_ms * 1e-3) / 1e9
-        pipe = C <= 4
-        kname = ("sh_bwd_pipe_kernel" if pipe else "sh_bwd_kernel") if cfg.kind == "sh" else \
-                (("nasg_bwd_pipe2_kernel" if C >= 2 else "nasg_bwd_pipe_kernel") if pipe else "nasg_bwd_kernel")
+        clk = clocks.summary()
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "warmup": warm, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": cfg.name, "N_per_gpu": N, "K": K, "C": C, "norm_mode": {1: "exact (eq.10)", 0: "approximate (NASG normaliser, PAPER.md:223)", 2: "pure NASG, no carrier (PAPER.md:423)"}[args.norm_mode],
-                       "l2": "inputs (%.2f GB/step) larger than the 126 MB L2; no flush" % ((fb + bb) * N / 1e9),
+            "config": {"workload": cfg.name, "N_per_gpu": N, "K": K, "C": C,
+                       "layout": "tile records (nasg_rec_*: parameters and gradients as [N/32][6+11K][32] records)" if rec else "row arrays",
+                       "norm_mode": {1: "exact (eq.10)", 0: "approximate (NASG normaliser, PAPER.md:223)", 2: "pure NASG, no carrier (PAPER.md:423)"}[args.norm_mode],
+                       "l2": ("inputs + outputs (%.2f GB/step) larger than the 126 MB L2; no flush" if (fb + bb) * N > 2.5e8 else
+                              "inputs + outputs (%.4f GB/step) FIT in the 126 MB L2 and are NOT flushed: L2-warm number") % ((fb + bb) * N / 1e9),
                        "parallelism": f"{world} x independent N-shards, no collective"},
             "fwd_ms": fwd_ms, "bwd_ms": bwd_ms,
             "algorithmic_gbs": {"fwd": fb * N / (fwd_ms * 1e-3) / 1e9, "bwd": achieved,
                                 "fwd+bwd": (fb + bb) * N / ((fwd_ms + bwd_ms) * 1e-3) / 1e9,
                                 "bytes_per_gaussian": {"fwd": fb, "bwd": bb}},
-            "roofline": {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": recorded_traffic(cfg.name), "peak_source": peak_src,
-                         "frac_of_nominal_8TBs": achieved / 8000.0},
-            "clocks": dict(clocks.summary(), window="timed region (%.0f ms) + identical untimed load up to 1 s" % (timed_wall * 1e3)),
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "api": "sh_eval_fwd_bwd_host" if cfg.kind == "sh" else "nasg_eval_fwd_bwd_host"},
+            "roofline": {"bound": "hbm", "kernel": R.kernel_name(), "achieved": achieved, "peak": peak, "unit": "GB/s",
+                         "frac": achieved / peak, "traffic": recorded(cfg.name, "dram_bytes_bwd_" + ("records" if rec else "rows")),
+                         "traffic_source": "recorded ncu --set full capture, not this run: profiles/traffic.json names capture and commit",
+                         "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0},
+            "clocks": dict(clk, window="timed region (%.0f ms) + identical untimed load up to 1 s" % (timed_wall * 1e3)),
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms,
+                    "gbs_each_way": [h2d / (e2e_ms * 1e-3) / 1e9, d2h / (e2e_ms * 1e-3) / 1e9],
+                    "api": "nasg_rec_eval_fwd_bwd_host" if rec else "sh_eval_fwd_bwd_host" if cfg.kind == "sh" else "nasg_eval_fwd_bwd_host"},
             "gpu_launches": int(launches),
         }
-        props = torch.cuda.get_device_properties(local)
-        alu_ms = alu_floor_ms(cfg.name, N, props.multi_processor_count, 1.965e9)
-        if alu_ms is not None:      # C = 4: the kernel is FP32-pipe/issue-bound, not HBM-bound
-            line["roofline"]["alu"] = {"floor_ms": alu_ms, "frac": alu_ms / bwd_ms,
-                                       "note": "warp-instruction issue floor at 1965 MHz from the committed ncu counts"}
+        line.update(extra)
+        # issue-slot utilisation of the dominant kernel AS WRITTEN (a diagnostic, not a roofline): its executed
+        # warp-instructions (committed ncu count) against the issue slots of the run at the SAMPLED SM clock
+        inst = recorded(cfg.name, "warp_instructions_per_32_gaussians_bwd_" + ("records" if rec else "rows"))
+        if inst is not None and clk.get("sm_mhz"):
+            props = torch.cuda.get_device_properties(local)
+            slots = props.multi_processor_count * 4 * clk["sm_mhz"] * 1e6 * bwd_ms * 1e-3
+            line["issue_utilisation"] = {"kernel": R.kernel_name(), "warp_instructions_per_32_gaussians": inst,
+                                         "frac_of_issue_slots": inst * (N / 32.0) / slots, "sm_mhz": clk["sm_mhz"],
+                                         "note": "diagnostic: executed instructions of the kernel as written (recorded ncu count) / issue slots at the sampled clock; packed f32x2 and MUFU instructions hold the issue port ~2 cycles (DESIGN.md section 7)"}
         if not args.no_cpu and world == 1:
             line["cpu_baseline"] = cpu_baseline(W, cfg)
         print(json.dumps(line), flush=True)
@@ -333,6 +413,10 @@ def main():
     ap.add_argument("--norm-mode", type=int, default=1, choices=[0, 1, 2],
                     help="1 = exact normaliser eq.(10) (default, the metric's configuration); 0 = the NASG normaliser the paper trained with; 2 = pure NASG lobe (no carrier)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
+    ap.add_argument("--no-others", action="store_true", help="skip the sustained run and the other configs (short profiling runs)")
+    ap.add_argument("--layout", default="rec", choices=["rec", "rows"],
+                    help="rec = tile-record parameter layout (nasg_rec_*, the fast path; NASGabor with even K, C <= 4); "
+                         "rows = the row-array entry points (nasg_eval_fwd/bwd)")
     args = ap.parse_args()
     global NORM_MODE
     NORM_MODE = 0 if args.norm_mode == 2 else args.norm_mode    # (the oracle has no carrier-free mode: same cost)

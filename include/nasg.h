@@ -106,6 +106,59 @@ int sh_eval_bwd(int64_t N, int32_t C, const float *means, const float *coeffs, c
                 const uint8_t *vis, const float *g_colors, float *g_means, float *g_coeffs,
                 float *g_campos, void *workspace, size_t workspace_bytes, void *cuda_stream);
 
+/* ---- tile-record parameter layout ("layout v2"): the fast path ---------------------------------------
+ * The per-Gaussian evaluation is issue-bound on B200 once C > 1, and with the row arrays above a
+ * warp's 32 Gaussians are 24-29 separate row segments whose addressing alone is 17-20 % of the executed instructions.
+ * The record layout stores everything a warp tile needs as ONE contiguous 16-byte aligned block, lobes interleaved in
+ * pairs so that they load as packed f32x2 operands:
+ *
+ *   params: float [T][6 + 11 K][32],  T = ceil(N / 32);  record of tile t (Gaussians n = 32 t + lane), floats:
+ *     [  0 ..  95]   means, planar:  x[32] y[32] z[32]
+ *     [ 96 .. 191]   dc (c0), planar: r[32] g[32] b[32]
+ *     [192 + 704 j + 64 c + 2 lane + h]   component c of lobe 2 j + h   (lobe pair j < K/2, h = 0,1)
+ *                    c = 0..3 quaternion (w,x,y,z) | 4..7 (log Lambda, log lambda, k, phi) | 8..10 amplitude (r,g,b)
+ *
+ * The same 6 + 11 K floats per Gaussian as the row arrays (the algorithmic bytes do not change); lanes past N in the
+ * last record are padding (written by nasg_rec_pack as a unit quaternion and zeros; never read back as results).
+ * Gradient records have the same layout (g_means, g_dc, then per pair the gradients of the 11 components); padding
+ * lanes of the last gradient record are not written. colors / g_colors [C,N,3] and vis [C,N] keep their shapes: they
+ * belong to the neighbouring stages (rasteriser). Restrictions of these entry points: K in {2, 4, 8}, C <= 4 (more
+ * cameras: call per batch of 4 and add the gradient records, or use the row-array entry points), no g_campos.
+ * g_colors / vis rows are moved with bulk copies when N % 4 == 0 (N % 16 == 0 with a mask) and the pointers are
+ * 16-byte aligned; otherwise they are loaded per lane (correct, slower). Everything else is as above: device
+ * pointers, caller-owned, asynchronous on cuda_stream, outputs overwritten, CUDA-graph capturable. */
+#define NASG_REC_MAX_CAMERAS 4
+#define NASG_REC_MAX_N ((int64_t)1 << 35)
+
+typedef struct {
+    int64_t N;
+    int32_t K;              /* 2, 4 or 8                                                            */
+    int32_t C;              /* 1..4                                                                 */
+    const float   *params;  /* nasg_rec_floats(N, K) floats, 16-byte aligned                        */
+    const float   *campos;  /* [C,3]                                                                */
+    const uint8_t *vis;     /* [C,N] or NULL                                                        */
+} nasg_rec_inputs;
+
+/* Floats in a parameter (or gradient) record array for N Gaussians of K lobes; 0 if K is unsupported. */
+size_t nasg_rec_floats(int64_t N, int32_t K);
+/* Row arrays -> records (reads means, quat, shape, amp, dc of `in`; campos, vis, C are ignored). */
+int nasg_rec_pack(const nasg_inputs *in, float *params, void *cuda_stream);
+/* Records -> row arrays (parameters or gradients alike); any output pointer may be NULL = skip. */
+int nasg_rec_unpack(int64_t N, int32_t K, const float *rec, float *means, float *quat, float *shape,
+                    float *amp, float *dc, void *cuda_stream);
+/* nasg_eval_fwd / nasg_eval_bwd on records: same function, same gradient (eq.(6), (9), (10)). */
+int nasg_rec_eval_fwd(const nasg_rec_inputs *in, float *colors, int norm_mode, void *cuda_stream);
+int nasg_rec_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float *g_params, int norm_mode,
+                      void *cuda_stream);
+
+/* End-to-end with HOST buffers, as nasg_eval_fwd_bwd_host below: params / g_params are HOST record arrays, campos, vis,
+ * g_colors, colors HOST arrays. A chunk of Gaussians is a contiguous block of records, so each chunk moves with one
+ * copy per direction for the parameters / gradients plus one strided copy each for vis, g_colors and colors. Padding
+ * lanes of the last gradient record are copied back as whatever the device buffer held (never results). */
+size_t nasg_rec_host_scratch_bytes(int64_t N, int32_t K, int32_t C);
+int nasg_rec_eval_fwd_bwd_host(const nasg_rec_inputs *in, const float *g_colors, float *colors, float *g_params,
+                               int norm_mode, void *dev_scratch, size_t dev_scratch_bytes, void *cuda_stream);
+
 /* Bytes of device scratch nasg_eval_bwd / sh_eval_bwd need when g_campos != NULL (pass K = 0 for SH). */
 size_t nasg_workspace_bytes(int64_t N, int32_t K, int32_t C);
 

@@ -21,7 +21,9 @@ NORM_APPROX, NORM_EXACT, NORM_NASG = 0, 1, 2
 MAX_CAMERAS = 64
 SYMBOLS = ("nasg_eval_fwd", "nasg_eval_bwd", "sh_eval_fwd", "sh_eval_bwd", "nasg_workspace_bytes",
            "nasg_host_scratch_bytes", "nasg_eval_fwd_bwd_host", "sh_host_scratch_bytes",
-           "sh_eval_fwd_bwd_host", "nasg_strerror", "nasg_version", "nasg_launch_count", "nasg_debug_set_path")
+           "sh_eval_fwd_bwd_host", "nasg_strerror", "nasg_version", "nasg_launch_count", "nasg_debug_set_path",
+           "nasg_rec_floats", "nasg_rec_pack", "nasg_rec_unpack", "nasg_rec_eval_fwd", "nasg_rec_eval_bwd",
+           "nasg_rec_host_scratch_bytes", "nasg_rec_eval_fwd_bwd_host")
 
 
 class NasgError(RuntimeError):
@@ -33,6 +35,11 @@ class NasgError(RuntimeError):
 class _Inputs(C.Structure):
     _fields_ = [("N", C.c_int64), ("K", C.c_int32), ("C", C.c_int32), ("means", C.c_void_p),
                 ("quat", C.c_void_p), ("shape", C.c_void_p), ("amp", C.c_void_p), ("dc", C.c_void_p),
+                ("campos", C.c_void_p), ("vis", C.c_void_p)]
+
+
+class _RecInputs(C.Structure):
+    _fields_ = [("N", C.c_int64), ("K", C.c_int32), ("C", C.c_int32), ("params", C.c_void_p),
                 ("campos", C.c_void_p), ("vis", C.c_void_p)]
 
 
@@ -52,6 +59,9 @@ def _load():
                 raise ImportError(
                     f"libnasg_b200.so is missing and could not be built ({exc}); run "
                     f"`python -m paper_2606_09794_b200.build`. There is no CPU fallback.") from exc
+            import warnings       # an older library exists: say that it does not match the sources
+            warnings.warn(f"libnasg_b200.so is older than its sources and the rebuild failed ({exc}); "
+                          f"loading the stale library", RuntimeWarning)
     lib = C.CDLL(path)
     vp, i64, i32, sz = C.c_void_p, C.c_int64, C.c_int32, C.c_size_t
     lib.nasg_eval_fwd.argtypes = [C.POINTER(_Inputs), vp, C.c_int, vp]
@@ -72,8 +82,18 @@ def _load():
     lib.nasg_launch_count.restype = i64
     lib.nasg_debug_set_path.argtypes = [C.c_int]
     lib.nasg_debug_set_path.restype = None
+    lib.nasg_rec_floats.argtypes = [i64, i32]
+    lib.nasg_rec_floats.restype = sz
+    lib.nasg_rec_pack.argtypes = [C.POINTER(_Inputs), vp, vp]
+    lib.nasg_rec_unpack.argtypes = [i64, i32, vp, vp, vp, vp, vp, vp, vp]
+    lib.nasg_rec_eval_fwd.argtypes = [C.POINTER(_RecInputs), vp, C.c_int, vp]
+    lib.nasg_rec_eval_bwd.argtypes = [C.POINTER(_RecInputs), vp, vp, C.c_int, vp]
+    lib.nasg_rec_host_scratch_bytes.argtypes = [i64, i32, i32]
+    lib.nasg_rec_host_scratch_bytes.restype = sz
+    lib.nasg_rec_eval_fwd_bwd_host.argtypes = [C.POINTER(_RecInputs), vp, vp, vp, C.c_int, vp, sz, vp]
     for name in ("nasg_eval_fwd", "nasg_eval_bwd", "sh_eval_fwd", "sh_eval_bwd", "nasg_eval_fwd_bwd_host",
-                 "sh_eval_fwd_bwd_host"):
+                 "sh_eval_fwd_bwd_host", "nasg_rec_pack", "nasg_rec_unpack", "nasg_rec_eval_fwd", "nasg_rec_eval_bwd",
+                 "nasg_rec_eval_fwd_bwd_host"):
         getattr(lib, name).restype = C.c_int
     return lib
 
@@ -177,6 +197,8 @@ def nasg_eval_bwd(means, quat, shape, amp, dc, campos, g_colors, vis=None, norm_
     _chk(g_colors, "g_colors", (inp.C, inp.N, 3), torch.float32, "cuda")
     if out is None:
         out = nasg_alloc_grads(inp.K, inp.N, inp.C, means.device, want_campos)
+    elif want_campos and (out.get("g_campos") is None or out.get("workspace") is None):
+        raise ValueError("want_campos=True but the supplied `out` lacks g_campos / workspace (nasg_alloc_grads(..., want_campos=True))")
     gs = _grads_struct(out)
     rc = _lib.nasg_eval_bwd(C.byref(inp), _ptr(g_colors), C.byref(gs), int(norm_mode), _stream(stream))
     if rc != 0:
@@ -245,6 +267,12 @@ def nasg_eval_fwd_bwd_host(host: dict, host_out: dict, dev_scratch: torch.Tensor
 
 def sh_eval_fwd_bwd_host(host: dict, host_out: dict, dev_scratch: torch.Tensor, stream=None) -> None:
     N, Cn = int(host["means"].shape[0]), int(host["campos"].shape[0])
+    f32 = torch.float32
+    _chk(host["means"], "means", (N, 3), f32, "cpu"); _chk(host["coeffs"], "coeffs", (16, 3, N), f32, "cpu")
+    _chk(host["campos"], "campos", (Cn, 3), f32, "cpu"); _chk(host.get("vis"), "vis", (Cn, N), torch.uint8, "cpu")
+    _chk(host["g_colors"], "g_colors", (Cn, N, 3), f32, "cpu"); _chk(host_out["colors"], "colors", (Cn, N, 3), f32, "cpu")
+    _chk(host_out.get("g_means"), "g_means", (N, 3), f32, "cpu"); _chk(host_out.get("g_coeffs"), "g_coeffs", (16, 3, N), f32, "cpu")
+    _chk(host_out.get("g_campos"), "g_campos", (Cn, 3), f32, "cpu")
     rc = _lib.sh_eval_fwd_bwd_host(N, Cn, _ptr(host["means"]), _ptr(host["coeffs"]), _ptr(host["campos"]),
                                    _ptr(host.get("vis")), _ptr(host["g_colors"]), _ptr(host_out["colors"]),
                                    _ptr(host_out.get("g_means")), _ptr(host_out.get("g_coeffs")),
@@ -252,3 +280,95 @@ def sh_eval_fwd_bwd_host(host: dict, host_out: dict, dev_scratch: torch.Tensor, 
                                    dev_scratch.numel() * dev_scratch.element_size(), _stream(stream))
     if rc != 0:
         raise NasgError(rc, "sh_eval_fwd_bwd_host")
+
+
+# ---- tile-record layout (include/nasg.h: nasg_rec_*) ----------------------------------------------
+def nasg_rec_floats(N: int, K: int) -> int:
+    return int(_lib.nasg_rec_floats(N, K))
+
+
+def nasg_rec_pack(means, quat, shape, amp, dc, out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    """Row arrays (layout v1) -> tile records: float tensor of nasg_rec_floats(N, K) elements."""
+    K, N = int(quat.shape[0]), int(quat.shape[1])
+    f32 = torch.float32
+    _chk(means, "means", (N, 3), f32, "cuda"); _chk(quat, "quat", (K, N, 4), f32, "cuda")
+    _chk(shape, "shape", (K, N, 4), f32, "cuda"); _chk(amp, "amp", (K, 3, N), f32, "cuda"); _chk(dc, "dc", (3, N), f32, "cuda")
+    inp = _Inputs(N, K, 1, _ptr(means), _ptr(quat), _ptr(shape), _ptr(amp), _ptr(dc), None, None)
+    if out is None:
+        out = torch.empty(nasg_rec_floats(N, K), dtype=f32, device=means.device)
+    _chk(out, "params", (nasg_rec_floats(N, K),), f32, "cuda")
+    rc = _lib.nasg_rec_pack(C.byref(inp), _ptr(out), _stream(stream))
+    if rc != 0:
+        raise NasgError(rc, "nasg_rec_pack")
+    return out
+
+
+def nasg_rec_unpack(rec: torch.Tensor, N: int, K: int, stream=None) -> dict:
+    """Tile records (parameters or gradients) -> dict of row arrays means, quat, shape, amp, dc."""
+    f32 = torch.float32
+    _chk(rec, "rec", (nasg_rec_floats(N, K),), f32, "cuda")
+    dev = rec.device
+    out = dict(means=torch.empty((N, 3), dtype=f32, device=dev), quat=torch.empty((K, N, 4), dtype=f32, device=dev),
+               shape=torch.empty((K, N, 4), dtype=f32, device=dev), amp=torch.empty((K, 3, N), dtype=f32, device=dev),
+               dc=torch.empty((3, N), dtype=f32, device=dev))
+    rc = _lib.nasg_rec_unpack(N, K, _ptr(rec), _ptr(out["means"]), _ptr(out["quat"]), _ptr(out["shape"]), _ptr(out["amp"]),
+                              _ptr(out["dc"]), _stream(stream))
+    if rc != 0:
+        raise NasgError(rc, "nasg_rec_unpack")
+    return out
+
+
+def _rec_inputs(params, N, K, campos, vis) -> _RecInputs:
+    Cn = int(campos.shape[0])
+    _chk(params, "params", (nasg_rec_floats(N, K),), torch.float32, "cuda")
+    _chk(campos, "campos", (Cn, 3), torch.float32, "cuda"); _chk(vis, "vis", (Cn, N), torch.uint8, "cuda")
+    return _RecInputs(N, K, Cn, _ptr(params), _ptr(campos), _ptr(vis))
+
+
+def nasg_rec_eval_fwd(params, N: int, K: int, campos, vis=None, norm_mode: int = NORM_EXACT,
+                      out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    """colors [C,N,3] from tile-record parameters (same function as nasg_eval_fwd)."""
+    inp = _rec_inputs(params, N, K, campos, vis)
+    if out is None:
+        out = torch.empty((inp.C, N, 3), dtype=torch.float32, device=params.device)
+    _chk(out, "colors", (inp.C, N, 3), torch.float32, "cuda")
+    rc = _lib.nasg_rec_eval_fwd(C.byref(inp), _ptr(out), int(norm_mode), _stream(stream))
+    if rc != 0:
+        raise NasgError(rc, "nasg_rec_eval_fwd")
+    return out
+
+
+def nasg_rec_eval_bwd(params, N: int, K: int, campos, g_colors, vis=None, norm_mode: int = NORM_EXACT,
+                      out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    """Gradient record array (layout of `params`) of sum(g_colors * colors)."""
+    inp = _rec_inputs(params, N, K, campos, vis)
+    _chk(g_colors, "g_colors", (inp.C, N, 3), torch.float32, "cuda")
+    if out is None:
+        out = torch.zeros(nasg_rec_floats(N, K), dtype=torch.float32, device=params.device)   # (padding lanes stay 0)
+    _chk(out, "g_params", (nasg_rec_floats(N, K),), torch.float32, "cuda")
+    rc = _lib.nasg_rec_eval_bwd(C.byref(inp), _ptr(g_colors), _ptr(out), int(norm_mode), _stream(stream))
+    if rc != 0:
+        raise NasgError(rc, "nasg_rec_eval_bwd")
+    return out
+
+
+def nasg_rec_host_scratch_bytes(N: int, K: int, Cn: int) -> int:
+    return int(_lib.nasg_rec_host_scratch_bytes(N, K, Cn))
+
+
+def nasg_rec_eval_fwd_bwd_host(host: dict, host_out: dict, N: int, K: int, dev_scratch: torch.Tensor,
+                               norm_mode: int = NORM_EXACT, stream=None) -> None:
+    """End-to-end call with HOST tensors on the tile-record layout: ``host`` holds params (records), campos, vis (or
+    None), g_colors; ``host_out`` holds colors and g_params (records)."""
+    f32 = torch.float32
+    Cn = int(host["campos"].shape[0])
+    nf = nasg_rec_floats(N, K)
+    _chk(host["params"], "params", (nf,), f32, "cpu"); _chk(host["campos"], "campos", (Cn, 3), f32, "cpu")
+    _chk(host.get("vis"), "vis", (Cn, N), torch.uint8, "cpu"); _chk(host["g_colors"], "g_colors", (Cn, N, 3), f32, "cpu")
+    _chk(host_out["colors"], "colors", (Cn, N, 3), f32, "cpu"); _chk(host_out["g_params"], "g_params", (nf,), f32, "cpu")
+    inp = _RecInputs(N, K, Cn, _ptr(host["params"]), _ptr(host["campos"]), _ptr(host.get("vis")))
+    rc = _lib.nasg_rec_eval_fwd_bwd_host(C.byref(inp), _ptr(host["g_colors"]), _ptr(host_out["colors"]), _ptr(host_out["g_params"]),
+                                         int(norm_mode), _ptr(dev_scratch), dev_scratch.numel() * dev_scratch.element_size(),
+                                         _stream(stream))
+    if rc != 0:
+        raise NasgError(rc, "nasg_rec_eval_fwd_bwd_host")

@@ -151,6 +151,85 @@ int sh_eval_bwd(int64_t N, int32_t C, const float *means, const float *coeffs, c
     return NASG_OK;
 }
 
+// ---- tile-record layout (include/nasg.h: nasg_rec_*) ---------------------------------------------
+static bool rec_K_ok(int K) { return K == 2 || K == 4 || K == 8; }
+static int norm_ok(int m) { return m == NASG_NORM_APPROX || m == NASG_NORM_EXACT || m == NASG_NORM_NASG; }
+
+size_t nasg_rec_floats(int64_t N, int32_t K)
+{
+    if (N <= 0 || !rec_K_ok(K)) return 0;
+    return (size_t)nasg::rec_total_floats(N, K);
+}
+
+int nasg_rec_pack(const nasg_inputs *in, float *params, void *cuda_stream)
+{
+    if (!in) return NASG_ERR_NULL;
+    if (in->N < 0 || in->N > NASG_REC_MAX_N) return NASG_ERR_SHAPE;
+    if (!rec_K_ok(in->K)) return NASG_ERR_UNSUPPORTED_K;
+    if (in->N == 0) return NASG_OK;
+    if (!in->means || !in->quat || !in->shape || !in->amp || !in->dc || !params) return NASG_ERR_NULL;
+    if (!aligned16(in->quat) || !aligned16(in->shape) || !aligned16(params)) return NASG_ERR_ALIGN;
+    cudaError_t e = nasg::launch_rec_pack(in->N, in->K, in->means, in->quat, in->shape, in->amp, in->dc, params, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(e);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return NASG_OK;
+}
+
+int nasg_rec_unpack(int64_t N, int32_t K, const float *rec, float *means, float *quat, float *shape, float *amp, float *dc,
+                    void *cuda_stream)
+{
+    if (N < 0 || N > NASG_REC_MAX_N) return NASG_ERR_SHAPE;
+    if (!rec_K_ok(K)) return NASG_ERR_UNSUPPORTED_K;
+    if (N == 0) return NASG_OK;
+    if (!rec) return NASG_ERR_NULL;
+    if (!aligned16(quat) || !aligned16(shape) || !aligned16(rec)) return NASG_ERR_ALIGN;
+    cudaError_t e = nasg::launch_rec_unpack(N, K, rec, means, quat, shape, amp, dc, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(e);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return NASG_OK;
+}
+
+static int check_rec_inputs(const nasg_rec_inputs *in, int norm_mode)
+{
+    if (!in) return NASG_ERR_NULL;
+    if (in->N < 0 || in->N > NASG_REC_MAX_N || in->C < 1 || in->C > NASG_REC_MAX_CAMERAS) return NASG_ERR_SHAPE;
+    if (!rec_K_ok(in->K)) return NASG_ERR_UNSUPPORTED_K;
+    if (!norm_ok(norm_mode)) return NASG_ERR_NORM_MODE;
+    if (in->N == 0) return NASG_OK;
+    if (!in->params || !in->campos) return NASG_ERR_NULL;
+    if (!aligned16(in->params)) return NASG_ERR_ALIGN;
+    return NASG_OK;
+}
+
+int nasg_rec_eval_fwd(const nasg_rec_inputs *in, float *colors, int norm_mode, void *cuda_stream)
+{
+    int rc = check_rec_inputs(in, norm_mode);
+    if (rc != NASG_OK) return rc;
+    if (in->N == 0) return NASG_OK;
+    if (!colors) return NASG_ERR_NULL;
+    const int bulk_rows = !in->vis || ((in->N & 15) == 0 && aligned16(in->vis));
+    nasg::RecFwdParams p{in->N, in->C, bulk_rows, in->params, in->campos, in->vis, colors};
+    cudaError_t e = nasg::launch_nasg_rec_fwd(p, in->K, norm_mode, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(e);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return NASG_OK;
+}
+
+int nasg_rec_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float *g_params, int norm_mode, void *cuda_stream)
+{
+    int rc = check_rec_inputs(in, norm_mode);
+    if (rc != NASG_OK) return rc;
+    if (in->N == 0) return NASG_OK;
+    if (!g_colors || !g_params) return NASG_ERR_NULL;
+    if (!aligned16(g_params)) return NASG_ERR_ALIGN;
+    const int bulk_rows = (in->N & 3) == 0 && aligned16(g_colors) && (!in->vis || ((in->N & 15) == 0 && aligned16(in->vis)));
+    nasg::RecBwdParams p{in->N, in->C, bulk_rows, in->params, in->campos, in->vis, g_colors, g_params};
+    cudaError_t e = nasg::launch_nasg_rec_bwd(p, in->K, norm_mode, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(e);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return NASG_OK;
+}
+
 size_t nasg_workspace_bytes(int64_t N, int32_t K, int32_t C)
 {
     (void)K;

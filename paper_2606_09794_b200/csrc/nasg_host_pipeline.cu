@@ -89,19 +89,9 @@ cudaError_t copy_rows(void *dst, size_t dst_cols, const void *src, size_t src_co
 // Runs `chunks` chunks through the three-stage pipeline. copy_in/compute/copy_out enqueue the work of
 // chunk i (Gaussians [n0, n0+nc)) that uses device buffer b on the given stream.
 template <typename CopyIn, typename Compute, typename CopyOut>
-int run_pipeline(int64_t N, int64_t chunk, cudaStream_t user, CopyIn copy_in, Compute compute, CopyOut copy_out)
+int enqueue_chunks(HostPipe &hp, int64_t N, int64_t chunk, cudaStream_t user, CopyIn copy_in, Compute compute, CopyOut copy_out)
 {
-    int dev = 0;
-    NASG_TRY_CUDA(cudaGetDevice(&dev));
-    if (dev < 0 || dev >= 64) return NASG_ERR_SHAPE;
-    HostPipe &hp = g_pipes[dev];
-    std::lock_guard<std::mutex> lock(hp.mu);
-    NASG_TRY_CUDA(hp.init());
     const int64_t chunks = (N + chunk - 1) / chunk;
-    NASG_TRY_CUDA(cudaEventRecord(hp.start, user));
-    NASG_TRY_CUDA(cudaStreamWaitEvent(hp.in, hp.start, 0));
-    NASG_TRY_CUDA(cudaStreamWaitEvent(hp.comp, hp.start, 0));
-    NASG_TRY_CUDA(cudaStreamWaitEvent(hp.out, hp.start, 0));
     for (int64_t i = 0; i < chunks; ++i) {
         const int b = (int)(i & 1);
         const int64_t n0 = i * chunk, nc = (n0 + chunk <= N) ? chunk : N - n0;
@@ -120,6 +110,30 @@ int run_pipeline(int64_t N, int64_t chunk, cudaStream_t user, CopyIn copy_in, Co
     NASG_TRY_CUDA(cudaStreamWaitEvent(user, hp.out_done[(chunks - 1) & 1], 0));
     if (chunks >= 2) NASG_TRY_CUDA(cudaStreamWaitEvent(user, hp.out_done[(chunks - 2) & 1], 0));
     return NASG_OK;
+}
+template <typename CopyIn, typename Compute, typename CopyOut>
+int run_pipeline(int64_t N, int64_t chunk, cudaStream_t user, CopyIn copy_in, Compute compute, CopyOut copy_out)
+{
+    int dev = 0;
+    NASG_TRY_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return NASG_ERR_SHAPE;
+    HostPipe &hp = g_pipes[dev];
+    std::lock_guard<std::mutex> lock(hp.mu);
+    NASG_TRY_CUDA(hp.init());
+    NASG_TRY_CUDA(cudaEventRecord(hp.start, user));
+    NASG_TRY_CUDA(cudaStreamWaitEvent(hp.in, hp.start, 0));
+    NASG_TRY_CUDA(cudaStreamWaitEvent(hp.comp, hp.start, 0));
+    NASG_TRY_CUDA(cudaStreamWaitEvent(hp.out, hp.start, 0));
+    const int rc = enqueue_chunks(hp, N, chunk, user, copy_in, compute, copy_out);
+    if (rc != NASG_OK) {
+        // an enqueue failed half-way: whatever is already queued on the internal streams may still touch the caller's
+        // buffers, so the caller's stream is joined to all three before the error is returned (best effort)
+        cudaStream_t ss[3] = {hp.in, hp.comp, hp.out};
+        cudaEvent_t es[3] = {hp.in_done[0], hp.comp_done[0], hp.out_done[0]};
+        for (int i = 0; i < 3; ++i)
+            if (cudaEventRecord(es[i], ss[i]) == cudaSuccess) cudaStreamWaitEvent(user, es[i], 0);
+    }
+    return rc;
 }
 
 } // namespace
@@ -309,6 +323,89 @@ int sh_eval_fwd_bwd_host(int64_t N, int32_t C, const float *means, const float *
         if (g_means) NASG_TRY_CUDA(copy_rows(g_means, Nn, d.gm, w, o, 0, w, 1, 12, D2H, st));
         if (g_coeffs) NASG_TRY_CUDA(copy_rows(g_coeffs, Nn, d.gco, w, o, 0, w, 48, 4, D2H, st));
         if (g_campos) NASG_TRY_CUDA(cudaMemcpyAsync(g_campos, d_gcam, c * 12, D2H, st));
+        return NASG_OK;
+    };
+    return run_pipeline(N, chunk, user, copy_in, compute, copy_out);
+}
+
+} // extern "C"
+
+// ---- NASGabor, tile-record layout: a chunk of Gaussians is a contiguous range of records ---------------
+namespace {
+struct RecDev { float *params, *gparams, *gcol, *col; uint8_t *vis; };
+size_t rec_footprint(size_t n, int K, size_t c)
+{
+    return 2 * align_up((size_t)nasg::rec_total_floats((int64_t)n, K) * 4) + align_up(c * n) + 2 * align_up(c * n * 12);
+}
+bool carve_rec(Carver &cv, RecDev &d, size_t n, int K, size_t c)
+{
+    const size_t rf = (size_t)nasg::rec_total_floats((int64_t)n, K);
+    d.params = cv.take<float>(rf); d.gparams = cv.take<float>(rf); d.vis = cv.take<uint8_t>(c * n);
+    d.gcol = cv.take<float>(c * n * 3); d.col = cv.take<float>(c * n * 3);
+    return cv.off <= cv.cap;
+}
+} // namespace
+
+extern "C" {
+
+size_t nasg_rec_host_scratch_bytes(int64_t N, int32_t K, int32_t C)
+{
+    if (N <= 0 || !(K == 2 || K == 4 || K == 8) || C < 1) return 0;
+    const size_t c = (size_t)C;
+    const size_t single = rec_footprint((size_t)N, K, c), chunked = 2 * rec_footprint((size_t)chunk_size(N, false), K, c);
+    return (single > chunked ? single : chunked) + align_up(c * 12) + SCRATCH_SLOP;
+}
+
+int nasg_rec_eval_fwd_bwd_host(const nasg_rec_inputs *in, const float *g_colors, float *colors, float *g_params,
+                               int norm_mode, void *dev_scratch, size_t dev_scratch_bytes, void *cuda_stream)
+{
+    if (!in) return NASG_ERR_NULL;
+    if (in->N < 0 || in->N > NASG_REC_MAX_N || in->C < 1 || in->C > NASG_REC_MAX_CAMERAS) return NASG_ERR_SHAPE;
+    if (!(in->K == 2 || in->K == 4 || in->K == 8)) return NASG_ERR_UNSUPPORTED_K;
+    if (norm_mode != NASG_NORM_APPROX && norm_mode != NASG_NORM_EXACT && norm_mode != NASG_NORM_NASG) return NASG_ERR_NORM_MODE;
+    if (in->N == 0) return NASG_OK;
+    if (!in->params || !in->campos || !g_colors || !colors || !g_params || !dev_scratch) return NASG_ERR_NULL;
+    if (dev_scratch_bytes < nasg_rec_host_scratch_bytes(in->N, in->K, in->C) || !aligned16(dev_scratch)) return NASG_ERR_WORKSPACE;
+    const int64_t N = in->N;
+    const int K = in->K;
+    const size_t c = (size_t)in->C, Nn = (size_t)N;
+    const int64_t chunk = chunk_size(N, false);              // a multiple of 256 Gaussians = 8 records (or all of N)
+    const bool two = chunk < N;
+
+    Carver cv{static_cast<char *>(dev_scratch), 0, dev_scratch_bytes};
+    float *d_campos = cv.take<float>(c * 3);
+    RecDev dev[2];
+    if (!carve_rec(cv, dev[0], (size_t)chunk, K, c)) return NASG_ERR_WORKSPACE;
+    if (two && !carve_rec(cv, dev[1], (size_t)chunk, K, c)) return NASG_ERR_WORKSPACE;
+    if (!d_campos) return NASG_ERR_WORKSPACE;
+
+    const cudaMemcpyKind H2D = cudaMemcpyHostToDevice, D2H = cudaMemcpyDeviceToHost;
+    cudaStream_t user = (cudaStream_t)cuda_stream;
+    NASG_TRY_CUDA(cudaMemcpyAsync(d_campos, in->campos, c * 12, H2D, user));     // replicated; before the pipeline's start event
+    const nasg_rec_inputs host = *in;
+    const size_t rec_f = (size_t)nasg::rec_total_floats(32, K);                  // floats per record
+
+    auto copy_in = [&](int b, int64_t n0, int64_t nc, cudaStream_t st) -> int {
+        const RecDev &d = dev[b];
+        const size_t o = (size_t)n0, w = (size_t)nc;
+        // the chunk's records are one contiguous block: a single copy
+        NASG_TRY_CUDA(cudaMemcpyAsync(d.params, host.params + (o / 32) * rec_f, (size_t)nasg::rec_total_floats(nc, K) * 4, H2D, st));
+        if (host.vis) NASG_TRY_CUDA(copy_rows(d.vis, w, host.vis, Nn, 0, o, w, c, 1, H2D, st));
+        NASG_TRY_CUDA(copy_rows(d.gcol, w, g_colors, Nn, 0, o, w, c, 12, H2D, st));
+        return NASG_OK;
+    };
+    auto compute = [&](int b, int64_t nc, cudaStream_t st) -> int {
+        const RecDev &d = dev[b];
+        nasg_rec_inputs din = host;
+        din.N = nc; din.params = d.params; din.campos = d_campos; din.vis = host.vis ? d.vis : nullptr;
+        NASG_TRY(nasg_rec_eval_fwd(&din, d.col, norm_mode, st));
+        return nasg_rec_eval_bwd(&din, d.gcol, d.gparams, norm_mode, st);
+    };
+    auto copy_out = [&](int b, int64_t n0, int64_t nc, cudaStream_t st) -> int {
+        const RecDev &d = dev[b];
+        const size_t o = (size_t)n0, w = (size_t)nc;
+        NASG_TRY_CUDA(copy_rows(colors, Nn, d.col, w, o, 0, w, c, 12, D2H, st));
+        NASG_TRY_CUDA(cudaMemcpyAsync(g_params + (o / 32) * rec_f, d.gparams, (size_t)nasg::rec_total_floats(nc, K) * 4, D2H, st));
         return NASG_OK;
     };
     return run_pipeline(N, chunk, user, copy_in, compute, copy_out);

@@ -36,6 +36,25 @@ struct ShParams {
     float *cam_partial;
 };
 
+// tile-record layout (nasg_rec_kernels.cu; include/nasg.h: nasg_rec_*)
+struct RecFwdParams {
+    int64_t N;
+    int C;
+    int bulk_rows;               // vis rows can be moved with bulk copies (N % 16 == 0, 16-byte aligned); else per-lane loads
+    const float *params, *campos;
+    const uint8_t *vis;
+    float *colors;
+};
+struct RecBwdParams {
+    int64_t N;
+    int C;
+    int bulk_rows;               // g_colors (N % 4 == 0) and vis rows (N % 16 == 0) can be moved with bulk copies
+    const float *params, *campos;
+    const uint8_t *vis;
+    const float *g_colors;
+    float *g_params;
+};
+
 int64_t grid_blocks(int64_t N);
 int api_cuda_fail(cudaError_t e);     // remembers e for nasg_strerror(), returns NASG_ERR_CUDA (nasg_api.cu)
 cudaError_t launch_nasg_fwd(const FwdParams &p, int K, int mode, cudaStream_t st);
@@ -47,6 +66,14 @@ cudaError_t launch_nasg_bwd_pipe(const BwdParams &p, int K, int mode, cudaStream
 bool tile_path_ok(int64_t N, int K, int C, const void *means, const void *amp, const void *planar, const void *rows, const void *vis);
 cudaError_t launch_nasg_fwd_tile(const FwdParams &p, int K, int mode, cudaStream_t st);
 cudaError_t launch_nasg_bwd_tile(const BwdParams &p, int K, int mode, cudaStream_t st);
+// headline path (nasg_rec_kernels.cu): tile-record parameter layout, even K, C <= 4
+int64_t rec_total_floats(int64_t N, int K);
+cudaError_t launch_nasg_rec_fwd(const RecFwdParams &p, int K, int mode, cudaStream_t st);
+cudaError_t launch_nasg_rec_bwd(const RecBwdParams &p, int K, int mode, cudaStream_t st);
+cudaError_t launch_rec_pack(int64_t N, int K, const float *means, const float *quat, const float *shape, const float *amp, const float *dc,
+                            float *rec_out, cudaStream_t st);
+cudaError_t launch_rec_unpack(int64_t N, int K, const float *rec_in, float *means, float *quat, float *shape, float *amp, float *dc,
+                              cudaStream_t st);
 cudaError_t launch_campos_reduce(const float *partial, int64_t nblocks, int C, float *out, cudaStream_t st);
 cudaError_t launch_sh_fwd(const ShParams &p, cudaStream_t st);
 cudaError_t launch_sh_bwd(const ShParams &p, cudaStream_t st);

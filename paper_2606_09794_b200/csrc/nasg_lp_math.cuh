@@ -319,12 +319,42 @@ NASG_HD void acc_zero(AccPair &A)
 // Backward of one (lobe pair, camera): adds to the pair's accumulators and returns the pair's contribution to
 // dL/dd of this camera (gdx, gdy, gdz: halves summed by the caller when it wants to).
 // gc = dL/dcolour of this camera (0 for a culled camera), w = amplitudes of the pair.
-template <bool CARRIER>
+// FIRST: this is the first camera of the lobe pair: the accumulators are initialised instead of added to (no zeroing pass).
+template <bool CARRIER, bool FIRST = false>
 NASG_HD void lobe_pair_bwd(const LobePair &L, const EvalPair &T, f2 G, float gc0, float gc1, float gc2, f2 w0, f2 w1, f2 w2,
                            AccPair &A, f2 &gdx, f2 &gdy, f2 &gdz)
 {
     const f2 c0 = splat(gc0), c1 = splat(gc1), c2 = splat(gc2);
     const f2 gG = fma2(w0, c0, fma2(w1, c1, mul2(w2, c2)));                 // dL/dG, eq.(6)
+    if (FIRST) {
+        A.gw0 = mul2(G, c0); A.gw1 = mul2(G, c1); A.gw2 = mul2(G, c2);
+        const f2 gGG = mul2(gG, G);
+        const f2 P = mul2(scl2(L.lam2e, LN2), T.kp);
+        const f2 Q = add2(P, splat(1.0f));
+        const f2 A_tau2 = mul2(scl2(T.L2, 2.0f * LN2), Q);
+        const f2 A_kap = mul2(fma2(T.tau, Q, P), T.inv_1pv);
+        const f2 B1 = mul2(mul2(gGG, A_tau2), T.inv_s2);
+        f2 gu = mul2(mul2(B1, L.a), T.u);
+        if (CARRIER) {
+            const f2 hs = mul2(mul2(gG, T.Gh), T.sn);
+            gu = fma2(neg2(hs), L.k, gu);
+            A.Sk = mul2(hs, T.u);
+            A.Sp = hs;
+        } else {
+            A.Sk = splat(0.f); A.Sp = splat(0.f);
+        }
+        const f2 gv = fma2(mul2(B1, T.tau), T.v, mul2(gGG, A_kap));
+        A.S0 = gGG;
+        A.S1 = mul2(gGG, T.em1);
+        A.S2 = mul2(B1, T.uu);
+        A.th0 = mul2(gv, T.om);
+        A.th1 = fma2(gv, T.u, mul2(neg2(gu), T.v));
+        A.th2 = mul2(gu, T.om);
+        gdx = fma2(gu, L.Xx, fma2(gv, L.Zx, gdx));
+        gdy = fma2(gu, L.Xy, fma2(gv, L.Zy, gdy));
+        gdz = fma2(gu, L.Xz, fma2(gv, L.Zz, gdz));
+        return;
+    }
     A.gw0 = fma2(G, c0, A.gw0); A.gw1 = fma2(G, c1, A.gw1); A.gw2 = fma2(G, c2, A.gw2);
     const f2 gGG = mul2(gG, G);
     const f2 P = mul2(scl2(L.lam2e, LN2), T.kp);                            // 2 lambda kappa^(1+tau)
@@ -376,6 +406,22 @@ NASG_HD void lobe_pair_finish(const LobePair &L, const LobePairGrad &Gd, const A
                 lo(A.th0), lo(A.th1), lo(A.th2), lo(qsw), lo(qsx), lo(qsy), lo(qsz), gs0, gq0);
     lobe_finish(hi(L.a), hi(L.lam2e), hi(Gd.nA), hi(Gd.nL), hi(Gd.nk), hi(A.S0), hi(A.S1), hi(A.S2), hi(A.Sk), hi(A.Sp),
                 hi(A.th0), hi(A.th1), hi(A.th2), hi(qsw), hi(qsx), hi(qsy), hi(qsz), gs1, gq1);
+}
+
+// The same for both lobes at once, results as pairs (lobe l, lobe l+1) per component: for the tile-record layout, whose
+// gradient records hold pairs (nasg_rec_kernels.cu), the packed form needs no re-assembly: 25 packed operations per pair.
+NASG_HD void lobe_pair_finish2(const LobePair &L, const LobePairGrad &Gd, const AccPair &A, f2 qw, f2 qx, f2 qy, f2 qz,
+                               f2 &gl1, f2 &gl2, f2 &gk, f2 &gphi, f2 &gqw, f2 &gqx, f2 &gqy, f2 &gqz)
+{
+    gl1 = fma2(scl2(A.S2, 0.5f), add2(L.a, splat(1.0f)), mul2(neg2(A.S0), Gd.nA));
+    gl2 = sub2(fma2(scl2(L.lam2e, LN2), A.S1, mul2(neg2(A.S0), Gd.nL)), gl1);
+    gk = fma2(neg2(A.S0), Gd.nk, neg2(A.Sk));
+    gphi = scl2(A.Sp, -1.0f);
+    // g_theta = (-th0, th1, th2);  (w, v) (x) (0, t) = ( -v.t ,  w t + v cross t )
+    gqw = fma2(qx, A.th0, neg2(fma2(qy, A.th1, mul2(qz, A.th2))));
+    gqx = fma2(neg2(qw), A.th0, fma2(qy, A.th2, mul2(neg2(qz), A.th1)));
+    gqy = fma2(qw, A.th1, fma2(neg2(qz), A.th0, mul2(neg2(qx), A.th2)));
+    gqz = fma2(qw, A.th2, fma2(qx, A.th1, mul2(qy, A.th0)));
 }
 
 } // namespace lp

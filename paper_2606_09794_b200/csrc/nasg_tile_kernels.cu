@@ -23,6 +23,7 @@
 // Warps never wait for each other: no __syncthreads, no atomics (a first version that shared 256-Gaussian tiles
 // between the 8 warps of a block, refilled by the last warp to release a slot, lost 25 % of its time to the drift
 // between warps: profiles/).
+#include "bulk_common.cuh"
 #include "nasg_internal.h"
 #include "nasg_lp_math.cuh"
 #include "pipe_common.cuh"
@@ -38,45 +39,7 @@ constexpr int NWARP = TB / 32;
 constexpr int WT = 32;                  // Gaussians per warp tile
 constexpr int STAGE_BYTES = WT * (2 * 16 + 2 * 16 + 6 * 4);        // quat[2], shape[2], amp[6] rows of a lobe pair: 2816 B
 
-// ---- mbarrier / bulk-copy primitives ------------------------------------------------------------
-__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-// wait for the phase with this parity (the suspend-time hint keeps a warp whose data is late asleep in hardware)
-__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
-{
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        "LAB_WAIT:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
-        "@p bra DONE;\n\t"
-        "bra LAB_WAIT;\n\t"
-        "DONE:\n\t"
-        "}" ::"r"(bar), "r"(parity), "r"(0x989680u) : "memory");
-}
-__device__ __forceinline__ bool elect_one()
-{
-    unsigned pred;
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        "elect.sync _|p, 0xffffffff;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t"
-        "}" : "=r"(pred));
-    return pred != 0;
-}
-__device__ __forceinline__ void bulk_g2s(unsigned dst, const void *src, unsigned bytes, unsigned bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
-}
+using namespace bulk;          // mbarrier / bulk-copy primitives, shared-memory accessors (bulk_common.cuh)
 
 // ---- shared-memory layout: one private region per warp ---------------------------------------------
 // [ stage 0 | ... | stage S-1 ][ header 0 | ... ][ scratch (backward) ][ mbarriers ]
@@ -169,29 +132,9 @@ __device__ __forceinline__ void warp_init(WarpCtx &c, unsigned char *smem, int r
     c.N = N;
     if ((threadIdx.x & 31) == 0) {
         for (int s = 0; s < 4; ++s) { mbar_init(bar_full(c, s), 1); mbar_init(bar_hfull(c, s), 1); }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        mbar_init_fence();
     }
     __syncwarp();
-}
-
-// shared-memory accesses by 32-bit shared-window address. Plain loads (not asm): they cannot move across the mbarrier
-// wait or the __syncwarp + re-issue, which are asm volatile with a memory clobber / a barrier.
-__device__ __forceinline__ float4 lds128(unsigned addr) { return *reinterpret_cast<const float4 *>(__cvta_shared_to_generic(addr)); }
-__device__ __forceinline__ float lds32(unsigned addr) { return *reinterpret_cast<const float *>(__cvta_shared_to_generic(addr)); }
-__device__ __forceinline__ unsigned lds8(unsigned addr) { return *reinterpret_cast<const unsigned char *>(__cvta_shared_to_generic(addr)); }
-// two pairs as one 16-byte access (pairs stay pairs: no re-assembly)
-__device__ __forceinline__ void sts64x2(unsigned addr, f2 a, f2 b)
-{
-    asm volatile("st.shared.v2.b64 [%0], {%1,%2};" ::"r"(addr), "l"(a), "l"(b) : "memory");
-}
-__device__ __forceinline__ void lds64x2(unsigned addr, f2 &a, f2 &b)
-{
-    asm volatile("ld.shared.v2.b64 {%0,%1}, [%2];" : "=l"(a), "=l"(b) : "r"(addr));
-}
-__device__ __forceinline__ void sts128(unsigned addr, float4 v)
-{
-    asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
 }
 
 // the 22 values of a lobe pair for this lane, as 11 pairs (lobe l, lobe l+1). Every value is read with its own

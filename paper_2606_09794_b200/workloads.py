@@ -127,3 +127,46 @@ def take(inp: dict, idx: np.ndarray) -> dict:
     if "dc" in inp:
         out["dc"] = np.ascontiguousarray(inp["dc"][:, idx])
     return out
+
+
+# ---- tile-record layout (include/nasg.h "layout v2"): pure re-ordering, no arithmetic ----------------
+REC_TILE = 32
+
+
+def rec_floats(N: int, K: int) -> int:
+    return ((N + REC_TILE - 1) // REC_TILE) * REC_TILE * (6 + 11 * K)
+
+
+def pack_records(means, quat, shape, amp, dc) -> np.ndarray:
+    """Row arrays -> float32 [T, 6 + 11 K, 32] records flattened (K even). Padding lanes: unit quaternion, zeros."""
+    K, N = quat.shape[0], quat.shape[1]
+    assert K % 2 == 0
+    T = (N + REC_TILE - 1) // REC_TILE
+    Np = T * REC_TILE
+
+    def padded(a, axis, fill=0.0):
+        pad = [(0, 0)] * a.ndim
+        pad[axis] = (0, Np - N)
+        return np.pad(a, pad, constant_values=fill)
+
+    rec = np.empty((T, 6 + 11 * K, REC_TILE), dtype=np.float32)
+    rec[:, 0:3, :] = padded(means, 0).reshape(T, REC_TILE, 3).transpose(0, 2, 1)
+    rec[:, 3:6, :] = padded(dc, 1).reshape(3, T, REC_TILE).transpose(1, 0, 2)
+    q = padded(quat, 1)
+    q[:, N:, 0] = 1.0
+    comp = np.concatenate([q, padded(shape, 1), padded(amp, 2).transpose(0, 2, 1)], axis=2)      # [K, Np, 11]
+    # [K/2, 2, T, 32, 11] -> [T, K/2, 11, 32, 2]
+    comp = comp.reshape(K // 2, 2, T, REC_TILE, 11).transpose(2, 0, 4, 3, 1)
+    rec[:, 6:, :] = comp.reshape(T, (K // 2) * 11 * 2, REC_TILE)
+    return rec.reshape(-1)
+
+
+def unpack_records(rec: np.ndarray, N: int, K: int) -> dict:
+    """Inverse of pack_records (also for gradient records): dict means, quat, shape, amp, dc."""
+    T = (N + REC_TILE - 1) // REC_TILE
+    rec = np.asarray(rec).reshape(T, 6 + 11 * K, REC_TILE)
+    means = rec[:, 0:3, :].transpose(0, 2, 1).reshape(T * REC_TILE, 3)[:N]
+    dc = rec[:, 3:6, :].transpose(1, 0, 2).reshape(3, T * REC_TILE)[:, :N]
+    comp = rec[:, 6:, :].reshape(T, K // 2, 11, REC_TILE, 2).transpose(1, 4, 0, 3, 2).reshape(K, T * REC_TILE, 11)[:, :N]
+    return dict(means=np.ascontiguousarray(means), dc=np.ascontiguousarray(dc), quat=np.ascontiguousarray(comp[..., 0:4]),
+                shape=np.ascontiguousarray(comp[..., 4:8]), amp=np.ascontiguousarray(comp[..., 8:11].transpose(0, 2, 1)))

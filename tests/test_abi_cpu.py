@@ -105,3 +105,49 @@ def test_product_never_imports_the_oracle():
     for f in ("nasg_ref.c", "sh_ref.c", "ref.py"):
         src = open(os.path.join(ROOT, "oracle", f)).read()
         assert "binding" not in src and "csrc" not in src and "nasg.h" not in src, f
+
+
+def test_rec_error_codes_without_gpu(B):
+    import ctypes as C
+    lib = B._lib
+    inp = B._RecInputs(64, 3, 1, 16, 16, None)
+    assert lib.nasg_rec_eval_fwd(C.byref(inp), 16, 1, None) == -3          # K = 3
+    inp = B._RecInputs(64, 4, 5, 16, 16, None)
+    assert lib.nasg_rec_eval_fwd(C.byref(inp), 16, 1, None) == -2          # C = 5
+    inp = B._RecInputs(64, 4, 1, None, 16, None)
+    assert lib.nasg_rec_eval_fwd(C.byref(inp), 16, 1, None) == -1
+    inp = B._RecInputs(64, 4, 1, 20, 16, None)
+    assert lib.nasg_rec_eval_fwd(C.byref(inp), 16, 1, None) == -4          # params misaligned
+    inp = B._RecInputs(64, 4, 1, 16, 16, None)
+    assert lib.nasg_rec_eval_fwd(C.byref(inp), 16, 7, None) == -7
+    assert lib.nasg_rec_eval_bwd(C.byref(inp), 16, None, 1, None) == -1
+    inp = B._RecInputs(0, 4, 1, None, None, None)
+    assert lib.nasg_rec_eval_fwd(C.byref(inp), None, 1, None) == 0         # N = 0: no-op
+
+
+def test_record_layout_reordering_round_trips():
+    """workloads.pack_records / unpack_records (no arithmetic: the input generator's re-ordering into the tile-record
+    layout of include/nasg.h) against the documented index formula."""
+    import numpy as np
+    from paper_2606_09794_b200 import workloads as W
+    for cfg, N in ((2, 77), (4, 32), (0, 1)):
+        inp = W.make(cfg, N)
+        K = inp["K"]
+        rec = W.pack_records(inp["means"], inp["quat"], inp["shape"], inp["amp"], inp["dc"])
+        assert rec.size == W.rec_floats(N, K)
+        back = W.unpack_records(rec, N, K)
+        for k in ("means", "quat", "shape", "amp", "dc"):
+            assert np.array_equal(back[k], inp[k]), k
+        R = (6 + 11 * K) * 32
+        for n in {0, N // 2, N - 1}:
+            t, lane = divmod(n, 32)
+            flat = rec[t * R:(t + 1) * R]
+            assert flat[lane] == inp["means"][n, 0] and flat[64 + lane] == inp["means"][n, 2]
+            assert flat[96 + 32 + lane] == inp["dc"][1, n]
+            for l in range(K):
+                j, h = divmod(l, 2)
+                for c in range(4):
+                    assert flat[192 + 704 * j + 64 * c + 2 * lane + h] == inp["quat"][l, n, c]
+                    assert flat[192 + 704 * j + 64 * (4 + c) + 2 * lane + h] == inp["shape"][l, n, c]
+                for c in range(3):
+                    assert flat[192 + 704 * j + 64 * (8 + c) + 2 * lane + h] == inp["amp"][l, c, n]

@@ -384,9 +384,22 @@ def test_host_entry_point_matches_device_path(B, W):
 
 
 def test_host_entry_point_chunked_pipeline(B, W):
-    """Large enough to be cut into several chunks (ragged last chunk): bit-identical to the device path."""
+    """Large enough to be cut into several chunks (ragged last chunk): bit-identical to the device path when both run
+    the same kernel family (the tile kernels would take the 16-aligned chunks but not the ragged whole, and the two
+    families round differently: the family is pinned to the ring kernels here; the automatic dispatch is then checked
+    against the same result within the forward / backward tolerances)."""
     inp = W.make(2, 3 * 131072 + 4099)
     d = to_dev(inp, NASG_KEYS)
+    B.nasg_debug_set_path(2)
+    try:
+        _host_chunked_nasg(B, inp, d, exact=True)
+    finally:
+        B.nasg_debug_set_path(0)
+    _host_chunked_nasg(B, inp, d, exact=False)
+    _host_chunked_sh(B, W)
+
+
+def _host_chunked_nasg(B, inp, d, exact):
     col, g = run_nasg(B, d, 1)
     host = {k: torch.from_numpy(np.ascontiguousarray(inp[k])).pin_memory() for k in NASG_KEYS}
     N, K, C = inp["N"], inp["K"], inp["C"]
@@ -401,9 +414,17 @@ def test_host_entry_point_chunked_pipeline(B, W):
         with torch.cuda.stream(side):
             B.nasg_eval_fwd_bwd_host(host, out, scratch, 1, stream=side)
         side.synchronize()                               # the caller's stream alone orders the call
-        assert torch.equal(out["colors"], col.cpu())
-        for k in ("g_means", "g_quat", "g_shape", "g_amp", "g_dc"):
-            assert torch.equal(out[k], g[k].cpu()), k
+        if exact:
+            assert torch.equal(out["colors"], col.cpu())
+            for k in ("g_means", "g_quat", "g_shape", "g_amp", "g_dc"):
+                assert torch.equal(out[k], g[k].cpu()), k
+        else:
+            assert rel_err(out["colors"], col.cpu().numpy().astype(np.float64)) <= FWD_TOL
+            for k in ("g_means", "g_quat", "g_shape", "g_amp", "g_dc"):
+                assert rel_err(out[k], g[k].cpu().numpy().astype(np.float64)) <= BWD_TOL, k
+
+
+def _host_chunked_sh(B, W):
     inp = W.make(3, 2 * 131072 + 777)
     d = to_dev(inp, SH_KEYS)
     col, g = run_sh(B, d)

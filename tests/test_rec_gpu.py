@@ -1,0 +1,230 @@
+"""GPU parity of the tile-record entry points (include/nasg.h: nasg_rec_*) against the fp64 oracle, element by element.
+
+The oracle knows nothing of records: it evaluates the plain row arrays; the records are produced from the same seeded
+arrays by the library's own nasg_rec_pack (checked bit for bit against the numpy re-ordering of workloads.py, which holds
+no arithmetic), and gradient records are taken apart again with nasg_rec_unpack before the comparison."""
+import dataclasses
+
+import numpy as np
+import pytest
+import torch
+
+from gpu_util import BWD_TOL, FWD_TOL, NASG_KEYS, p99_rel, rel_err, to_dev
+
+pytestmark = pytest.mark.gpu
+GRADS = (("g_means", "means"), ("g_quat", "quat"), ("g_shape", "shape"), ("g_amp", "amp"), ("g_dc", "dc"))
+
+
+@pytest.fixture(scope="module")
+def B():
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    from paper_2606_09794_b200 import binding
+    return binding
+
+
+@pytest.fixture(scope="module")
+def W():
+    from paper_2606_09794_b200 import workloads
+    return workloads
+
+
+def run_rec(B, d, N, K, mode=1):
+    params = B.nasg_rec_pack(d["means"], d["quat"], d["shape"], d["amp"], d["dc"])
+    col = B.nasg_rec_eval_fwd(params, N, K, d["campos"], d["vis"], mode)
+    grec = B.nasg_rec_eval_bwd(params, N, K, d["campos"], d["g_colors"], d["vis"], mode)
+    g = B.nasg_rec_unpack(grec, N, K)
+    torch.cuda.synchronize()
+    return col, g, params, grec
+
+
+def check_rec(B, oracle, inp, mode=1, label=""):
+    d = to_dev(inp, NASG_KEYS)
+    col, g, _, _ = run_rec(B, d, inp["N"], inp["K"], mode)
+    rc, rg = oracle.nasg_fwd(inp, mode), oracle.nasg_bwd(inp, mode)
+    errs = {"colors": rel_err(col, rc)}
+    for gk, pk in GRADS:
+        errs[gk] = rel_err(g[pk], rg[gk])
+    print(label, " ".join(f"{k}={v:.2e}" for k, v in errs.items()))
+    assert errs["colors"] <= FWD_TOL, (label, errs)
+    for k, v in errs.items():
+        if k != "colors":
+            assert v <= BWD_TOL, (label, k, errs)
+    return col, g
+
+
+def test_pack_matches_the_documented_layout_and_round_trips(B, W):
+    for cfg, N in ((2, 4099), (0, 10_000), (4, 31), (1, 1), (2, 32), (2, 64)):
+        inp = W.make(cfg, N)
+        d = to_dev(inp, NASG_KEYS)
+        K = inp["K"]
+        rec = B.nasg_rec_pack(d["means"], d["quat"], d["shape"], d["amp"], d["dc"])
+        want = W.pack_records(inp["means"], inp["quat"], inp["shape"], inp["amp"], inp["dc"])
+        assert rec.numel() == B.nasg_rec_floats(N, K) == W.rec_floats(N, K) == want.size
+        assert np.array_equal(rec.cpu().numpy(), want)
+        back = B.nasg_rec_unpack(rec, N, K)
+        for k in ("means", "quat", "shape", "amp", "dc"):
+            assert np.array_equal(back[k].cpu().numpy(), inp[k]), k
+
+
+@pytest.mark.parametrize("cfg,N", [(0, None), (1, 70_001), (2, 50_003), (2, 50_016), (4, 40_007), (4, 40_000)])
+@pytest.mark.parametrize("mode", [1, 0])
+def test_rec_configs_small(B, W, oracle, cfg, N, mode):
+    """Several tiles per warp and a ragged last record; N % 16 == 0 (bulk-copied g_colors / vis rows) and odd N
+    (per-lane row loads)."""
+    inp = W.make(cfg, N)
+    check_rec(B, oracle, inp, mode, label=f"rec cfg{cfg} N={inp['N']} mode={mode}")
+
+
+@pytest.mark.parametrize("K", [2, 4, 8])
+@pytest.mark.parametrize("C", [1, 2, 3, 4])
+@pytest.mark.parametrize("N", [2_064, 2_101])
+def test_rec_all_lobe_counts_and_cameras(B, W, oracle, K, C, N):
+    cfg = dataclasses.replace(W.CONFIGS[2], seed=90 + K * 10 + C, K=K, C=C)
+    inp = W.make_nasg(cfg, N=N + 32 * K)
+    check_rec(B, oracle, inp, 1, label=f"rec K={K} C={C} N={inp['N']}")
+
+
+@pytest.mark.parametrize("N", [1, 31, 32, 33, 255, 256, 257, 8 * 32 * 148 * 2 + 16])
+def test_rec_tiny_and_ragged_sizes(B, W, oracle, N):
+    inp = W.make(2, N)
+    check_rec(B, oracle, inp, 1, label=f"rec N={N}")
+
+
+def test_rec_pure_nasg_mode(B, W, oracle):
+    inp = W.make(2, 20_016)
+    zero = dict(inp, shape=inp["shape"].copy())
+    zero["shape"][..., 2:] = 0.0
+    rc, rg = oracle.nasg_fwd(zero, 0), oracle.nasg_bwd(zero, 0)
+    d = to_dev(inp, NASG_KEYS)
+    col, g, _, _ = run_rec(B, d, inp["N"], inp["K"], 2)
+    assert rel_err(col, rc) <= FWD_TOL
+    for gk, pk in (("g_means", "means"), ("g_quat", "quat"), ("g_amp", "amp"), ("g_dc", "dc")):
+        assert rel_err(g[pk], rg[gk]) <= BWD_TOL, gk
+    assert rel_err(g["shape"][..., :2], rg["g_shape"][..., :2]) <= BWD_TOL
+    assert (g["shape"][..., 2:] == 0).all()
+
+
+def test_rec_masks_culled_pairs_and_nan_g_colors(B, W, oracle):
+    """Culled pairs: colour exactly 0, no gradient; g_colors of a culled pair is never read as a value (NaN there must
+    not leak); a Gaussian culled in every camera has zero gradients; all-culled and all-visible masks."""
+    inp = W.make(2, 6_016)
+    vis = inp["vis"].copy()
+    vis[:, 100:164] = 0                                   # two whole tiles dead
+    gc = inp["g_colors"].copy()
+    gc[vis == 0] = np.nan
+    bad = dict(inp, vis=vis, g_colors=gc)
+    clean = dict(inp, vis=vis)
+    d = to_dev(bad, NASG_KEYS)
+    col, g, _, _ = run_rec(B, d, inp["N"], inp["K"], 1)
+    rc, rg = oracle.nasg_fwd(clean, 1), oracle.nasg_bwd(clean, 1)
+    assert rel_err(col, rc) <= FWD_TOL and (col.cpu().numpy()[vis == 0] == 0).all()
+    for gk, pk in GRADS:
+        assert rel_err(g[pk], rg[gk]) <= BWD_TOL, gk
+    dead = ~(vis != 0).any(0)
+    assert dead.sum() >= 64
+    gm, gq, ga = g["means"].cpu().numpy(), g["quat"].cpu().numpy(), g["amp"].cpu().numpy()
+    assert (gm[dead] == 0).all() and (gq[:, dead] == 0).all() and (ga[:, :, dead] == 0).all()
+    # g_dc = masked sum of g_colors
+    want = (np.where(vis[..., None] != 0, inp["g_colors"], 0.0).astype(np.float64)).sum(0).T
+    assert np.abs(g["dc"].cpu().numpy() - want).max() <= 1e-6 * np.abs(want).max()
+    for fill in (0, 1):
+        v = np.full_like(vis, fill)
+        check_rec(B, oracle, dict(inp, vis=v), 1, label=f"rec mask all {fill}")
+    check_rec(B, oracle, dict(inp, vis=None), 1, label="rec mask NULL")
+
+
+def test_rec_matches_the_row_array_entry_points(B, W):
+    """The record kernels and the row-array kernels compute the same function: they agree far inside the tolerances
+    (different instruction order, so not bit for bit)."""
+    from gpu_util import run_nasg
+    inp = W.make(2, 30_000)
+    d = to_dev(inp, NASG_KEYS)
+    col1, g1 = run_nasg(B, d, 1)
+    col2, g2, _, _ = run_rec(B, d, inp["N"], inp["K"], 1)
+    assert rel_err(col2, col1.cpu().numpy().astype(np.float64)) <= FWD_TOL
+    for gk, pk in GRADS:
+        assert rel_err(g2[pk], g1[gk].cpu().numpy().astype(np.float64)) <= BWD_TOL, gk
+
+
+def test_rec_bit_reproducible_and_graph_capturable(B, W):
+    inp = W.make(2, 40_000)
+    d = to_dev(inp, NASG_KEYS)
+    N, K = inp["N"], inp["K"]
+    col, g, params, grec = run_rec(B, d, N, K, 1)
+    col2, g2, _, grec2 = run_rec(B, d, N, K, 1)
+    assert torch.equal(col, col2) and torch.equal(grec, grec2)
+    s = torch.cuda.Stream()
+    out, gout = torch.empty_like(col), torch.zeros_like(grec)
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        B.nasg_rec_eval_fwd(params, N, K, d["campos"], d["vis"], 1, out=out, stream=s)      # warm
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=s):
+            B.nasg_rec_eval_fwd(params, N, K, d["campos"], d["vis"], 1, out=out, stream=s)
+            B.nasg_rec_eval_bwd(params, N, K, d["campos"], d["g_colors"], d["vis"], 1, out=gout, stream=s)
+    out.zero_()
+    graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(out, col) and torch.equal(gout, grec)
+
+
+def test_rec_padding_lanes_of_the_gradient_record_are_not_written(B, W):
+    inp = W.make(2, 70)
+    d = to_dev(inp, NASG_KEYS)
+    N, K = inp["N"], inp["K"]
+    params = B.nasg_rec_pack(d["means"], d["quat"], d["shape"], d["amp"], d["dc"])
+    grec = torch.full((B.nasg_rec_floats(N, K),), 123.0, device="cuda")
+    B.nasg_rec_eval_bwd(params, N, K, d["campos"], d["g_colors"], d["vis"], 1, out=grec)
+    torch.cuda.synchronize()
+    r = grec.cpu().numpy().reshape(3, 6 + 11 * K, 32)
+    assert (r[2, :6, 6:] == 123.0).all() and (r[2, :6, :6] != 123.0).all()
+    pairs = r[2, 6:].reshape(K // 2, 11, 32, 2)
+    assert (pairs[:, :, 6:] == 123.0).all() and (pairs[:, :, :6] != 123.0).all()
+    assert (r[:2] != 123.0).all()
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 4])
+def test_rec_full_size_every_element(B, W, oracle, cfg):
+    """BASELINE sizes in bench.py's launch configuration: every element of every output array against the oracle."""
+    inp = W.make(cfg)
+    d = to_dev(inp, NASG_KEYS)
+    N, K = inp["N"], inp["K"]
+    col, g, _, _ = run_rec(B, d, N, K, 1)
+    rc = oracle.nasg_fwd(inp, 1)
+    errs, p99 = {"colors": rel_err(col, rc)}, {"colors": p99_rel(col, rc)}
+    if d["vis"] is not None:
+        assert (col[d["vis"] == 0] == 0).all()
+    del rc, col
+    rg = oracle.nasg_bwd(inp, 1)
+    for gk, pk in GRADS:
+        errs[gk], p99[gk] = rel_err(g[pk], rg[gk]), p99_rel(g[pk], rg[gk])
+    print(f"rec cfg{cfg} full N={N} all elements:", " ".join(f"{k}={errs[k]:.2e}(p99 {p99[k]:.1e})" for k in errs))
+    assert errs.pop("colors") <= FWD_TOL
+    for k, v in errs.items():
+        assert v <= BWD_TOL, (k, v)
+
+
+@pytest.mark.parametrize("N", [10_007, 3 * 131072 + 4099])
+def test_rec_host_entry_point(B, W, N):
+    """nasg_rec_eval_fwd_bwd_host (single chunk and chunked pipeline with a ragged last chunk): bit-identical to the
+    device entry points on the same records (the chunks are multiples of 256 Gaussians, so every chunk runs the same
+    kernels on the same tiles)."""
+    inp = W.make(2, N)
+    d = to_dev(inp, NASG_KEYS)
+    K = inp["K"]
+    col, _, params, grec = run_rec(B, d, N, K, 1)
+    host = dict(params=params.cpu().pin_memory(), campos=d["campos"].cpu(), vis=d["vis"].cpu().pin_memory(),
+                g_colors=d["g_colors"].cpu().pin_memory())
+    out = dict(colors=torch.empty((inp["C"], N, 3)).pin_memory(), g_params=torch.zeros(B.nasg_rec_floats(N, K)).pin_memory())
+    scratch = torch.empty(B.nasg_rec_host_scratch_bytes(N, K, inp["C"]), dtype=torch.uint8, device="cuda")
+    side = torch.cuda.Stream()
+    for _ in range(2):
+        out["colors"].fill_(7.0)
+        with torch.cuda.stream(side):
+            B.nasg_rec_eval_fwd_bwd_host(host, out, N, K, scratch, 1, stream=side)
+        side.synchronize()
+        assert torch.equal(out["colors"], col.cpu())
+        got = B.nasg_rec_unpack(out["g_params"].cuda(), N, K)
+        want = B.nasg_rec_unpack(grec, N, K)
+        for k in ("means", "quat", "shape", "amp", "dc"):
+            assert torch.equal(got[k], want[k]), k
