@@ -349,3 +349,155 @@ int nasg_ref_bwd(int64_t N, int K, int C, const double *means, const double *qua
     }
     return 0;
 }
+
+/* ============================================================================================
+ * Paper-native parameter record: 3 + 9K floats per primitive
+ * (Table 5), no phase, Table 8 activations:
+ *
+ *   (c_theta, c_phi, c_tau) = tanh(raw)                 cosines of the frame angles
+ *   lambda = exp(raw), a = exp(raw), k = 20 (tanh(raw) + 1), w = tanh(raw)
+ *   s = +sqrt(1 - c^2);  z = (c_theta s_phi, s_theta s_phi, c_phi),
+ *   x = (c_theta c_phi c_tau - s_theta s_tau, s_theta c_phi c_tau + c_theta s_tau, -s_phi c_tau)
+ *                                                      Supplementary C
+ *   backward through the frame: eqs.(37)-(44) PAPER.md:687-720, with eq.(39) read as
+ *   dz/dc_theta = (s_phi, -(c_theta/s_theta) s_phi, 0) (R6(iii): the printed eq.(39) is garbled),
+ *   and ds/dc = -c/s (eq.36).
+ * The DC colour c0 has no activation (the paper lists none). The lobe itself is lobe_partials()
+ * above with phi = 0. Layouts: euler [K,N,3] (theta, phi, tau raw), shp [K,N,3] (lambda, a, k raw),
+ * ampraw [K,3,N], dc [3,N]; gradients are with respect to the RAW (pre-activation) values.
+ * ============================================================================================ */
+typedef struct {
+    double c[3], s[3];      /* cos / sin of theta, phi, tau */
+    double X[3], Z[3];
+    double lambda, a, k, w[3];
+    double tk;              /* tanh(k_raw) */
+} paper_lobe;
+
+static void paper_decode(const double *eu, const double *sp, const double w_raw[3], paper_lobe *L)
+{
+    for (int i = 0; i < 3; ++i) { L->c[i] = tanh(eu[i]); L->s[i] = sqrt(1.0 - L->c[i] * L->c[i]); }
+    const double ct = L->c[0], cp = L->c[1], cu = L->c[2], st = L->s[0], sp_ = L->s[1], su = L->s[2];
+    L->Z[0] = ct * sp_; L->Z[1] = st * sp_; L->Z[2] = cp;
+    L->X[0] = ct * cp * cu - st * su; L->X[1] = st * cp * cu + ct * su; L->X[2] = -sp_ * cu;
+    L->lambda = exp(sp[0]); L->a = exp(sp[1]);
+    L->tk = tanh(sp[2]); L->k = 20.0 * (L->tk + 1.0);
+    for (int ch = 0; ch < 3; ++ch) L->w[ch] = tanh(w_raw[ch]);
+}
+
+/* exported for the pins: frame (X, Z) and its derivatives with respect to the three cosines, eqs.(38)-(44) */
+void nasg_ref_paper_frame(const double eu_raw[3], double X[3], double Z[3], double dX[3][3], double dZ[3][3])
+{
+    paper_lobe L; double sp[3] = { 0, 0, 0 }, w[3] = { 0, 0, 0 };
+    paper_decode(eu_raw, sp, w, &L);
+    for (int i = 0; i < 3; ++i) { X[i] = L.X[i]; Z[i] = L.Z[i]; }
+    const double ct = L.c[0], cp = L.c[1], cu = L.c[2], st = L.s[0], sp_ = L.s[1], su = L.s[2];
+    /* d/dc_theta: eq.(38), eq.(39) as corrected */
+    dX[0][0] = cp * cu + (ct / st) * su; dX[0][1] = -(ct / st) * cp * cu + su; dX[0][2] = 0.0;
+    dZ[0][0] = sp_; dZ[0][1] = -(ct / st) * sp_; dZ[0][2] = 0.0;
+    /* d/dc_phi: eqs.(41), (42) */
+    dX[1][0] = ct * cu; dX[1][1] = st * cu; dX[1][2] = (cp / sp_) * cu;
+    dZ[1][0] = -ct * cp / sp_; dZ[1][1] = -st * cp / sp_; dZ[1][2] = 1.0;
+    /* d/dc_tau: eq.(44); z does not depend on tau */
+    dX[2][0] = ct * cp + st * cu / su; dX[2][1] = st * cp - ct * cu / su; dX[2][2] = -sp_;
+    dZ[2][0] = dZ[2][1] = dZ[2][2] = 0.0;
+}
+
+int nasg_ref_paper_fwd(int64_t N, int K, int C, const double *means, const double *euler, const double *shp,
+                       const double *ampraw, const double *dc, const double *campos, const uint8_t *vis,
+                       int norm_mode, double *colors)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t n = 0; n < N; ++n) {
+        for (int c = 0; c < C; ++c) {
+            double *col = colors + ((size_t)c * N + n) * 3;
+            if (vis && !vis[(size_t)c * N + n]) { col[0] = col[1] = col[2] = 0.0; continue; }
+            double dx = means[3 * n] - campos[3 * c], dy = means[3 * n + 1] - campos[3 * c + 1],
+                   dz = means[3 * n + 2] - campos[3 * c + 2];
+            double dist = sqrt(dx * dx + dy * dy + dz * dz);
+            double d[3] = { dx / dist, dy / dist, dz / dist };
+            double rgb[3] = { dc[n], dc[N + n], dc[2 * N + n] };
+            for (int l = 0; l < K; ++l) {
+                double wr[3] = { ampraw[((size_t)l * 3 + 0) * N + n], ampraw[((size_t)l * 3 + 1) * N + n],
+                                 ampraw[((size_t)l * 3 + 2) * N + n] };
+                paper_lobe L; double o[7];
+                paper_decode(euler + ((size_t)l * N + n) * 3, shp + ((size_t)l * N + n) * 3, wr, &L);
+                double u = d[0] * L.X[0] + d[1] * L.X[1] + d[2] * L.X[2];
+                double v = d[0] * L.Z[0] + d[1] * L.Z[1] + d[2] * L.Z[2];
+                lobe_partials(u, v, L.lambda, L.a, L.k, 0.0, norm_mode, o);
+                for (int ch = 0; ch < 3; ++ch) rgb[ch] += L.w[ch] * o[0];
+            }
+            col[0] = rgb[0]; col[1] = rgb[1]; col[2] = rgb[2];
+        }
+    }
+    return 0;
+}
+
+int nasg_ref_paper_bwd(int64_t N, int K, int C, const double *means, const double *euler, const double *shp,
+                       const double *ampraw, const double *dc, const double *campos, const uint8_t *vis,
+                       const double *g_colors, int norm_mode, double *g_means, double *g_euler, double *g_shp,
+                       double *g_ampraw, double *g_dc)
+{
+    (void)dc;
+#pragma omp parallel for schedule(static)
+    for (int64_t n = 0; n < N; ++n) {
+        double gm[3] = { 0, 0, 0 }, gdc[3] = { 0, 0, 0 };
+        for (int c = 0; c < C; ++c) {
+            if (vis && !vis[(size_t)c * N + n]) continue;
+            const double *gcol = g_colors + ((size_t)c * N + n) * 3;
+            for (int ch = 0; ch < 3; ++ch) gdc[ch] += gcol[ch];
+        }
+        for (int l = 0; l < K; ++l) {
+            const double *eu = euler + ((size_t)l * N + n) * 3;
+            double wr[3] = { ampraw[((size_t)l * 3 + 0) * N + n], ampraw[((size_t)l * 3 + 1) * N + n],
+                             ampraw[((size_t)l * 3 + 2) * N + n] };
+            paper_lobe L;
+            paper_decode(eu, shp + ((size_t)l * N + n) * 3, wr, &L);
+            double gX[3] = { 0, 0, 0 }, gZ[3] = { 0, 0, 0 }, gw[3] = { 0, 0, 0 }, g_lambda = 0, g_a = 0, g_k = 0;
+            for (int c = 0; c < C; ++c) {
+                if (vis && !vis[(size_t)c * N + n]) continue;
+                const double *gcol = g_colors + ((size_t)c * N + n) * 3;
+                double dx = means[3 * n] - campos[3 * c], dy = means[3 * n + 1] - campos[3 * c + 1],
+                       dz = means[3 * n + 2] - campos[3 * c + 2];
+                double dist = sqrt(dx * dx + dy * dy + dz * dz);
+                double d[3] = { dx / dist, dy / dist, dz / dist };
+                double u = d[0] * L.X[0] + d[1] * L.X[1] + d[2] * L.X[2];
+                double v = d[0] * L.Z[0] + d[1] * L.Z[1] + d[2] * L.Z[2];
+                double o[7];
+                lobe_partials(u, v, L.lambda, L.a, L.k, 0.0, norm_mode, o);
+                double gG = gcol[0] * L.w[0] + gcol[1] * L.w[1] + gcol[2] * L.w[2];
+                for (int ch = 0; ch < 3; ++ch) gw[ch] += gcol[ch] * o[0];
+                g_lambda += gG * o[3]; g_a += gG * o[4]; g_k += gG * o[5];
+                double gd[3];
+                for (int i = 0; i < 3; ++i) {
+                    gX[i] += gG * o[1] * d[i];
+                    gZ[i] += gG * o[2] * d[i];
+                    gd[i] = gG * (o[1] * L.X[i] + o[2] * L.Z[i]);
+                }
+                double dg = d[0] * gd[0] + d[1] * gd[1] + d[2] * gd[2];
+                for (int i = 0; i < 3; ++i) gm[i] += (gd[i] - d[i] * dg) / dist;
+            }
+            /* chain rule through the cosines, eqs.(37), (40), (43), then through tanh: dc/draw = 1 - c^2 */
+            double X[3], Z[3], dX[3][3], dZ[3][3];
+            nasg_ref_paper_frame(eu, X, Z, dX, dZ);
+            if (g_euler) {
+                double *ge = g_euler + ((size_t)l * N + n) * 3;
+                for (int i = 0; i < 3; ++i) {
+                    double gc = 0.0;
+                    for (int j = 0; j < 3; ++j) gc += gX[j] * dX[i][j] + gZ[j] * dZ[i][j];
+                    ge[i] = gc * (1.0 - L.c[i] * L.c[i]);
+                }
+            }
+            if (g_shp) {
+                double *gs = g_shp + ((size_t)l * N + n) * 3;
+                gs[0] = g_lambda * L.lambda;                       /* lambda = exp(raw) */
+                gs[1] = g_a * L.a;                                 /* a = exp(raw)      */
+                gs[2] = g_k * 20.0 * (1.0 - L.tk * L.tk);          /* k = 20 (tanh(raw) + 1) */
+            }
+            if (g_ampraw)
+                for (int ch = 0; ch < 3; ++ch) g_ampraw[((size_t)l * 3 + ch) * N + n] = gw[ch] * (1.0 - L.w[ch] * L.w[ch]);
+        }
+        if (g_means) { g_means[3 * n] = gm[0]; g_means[3 * n + 1] = gm[1]; g_means[3 * n + 2] = gm[2]; }
+        if (g_dc) { g_dc[n] = gdc[0]; g_dc[N + n] = gdc[1]; g_dc[2 * N + n] = gdc[2]; }
+    }
+    return 0;
+}

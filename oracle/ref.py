@@ -48,6 +48,11 @@ def lib():
         L.nasg_ref_dlnI.argtypes = [dbl, dbl, dbl, i32, dp]
         L.nasg_ref_partials.argtypes = [dbl, dbl, dbl, dbl, dbl, dbl, i32, dp]
         L.nasg_ref_frame.argtypes = [dp, dp, dp]
+        L.nasg_ref_paper_frame.argtypes = [dp, dp, dp, dp, dp]
+        L.nasg_ref_paper_fwd.argtypes = [i64, i32, i32, dp, dp, dp, dp, dp, dp, u8p, i32, dp]
+        L.nasg_ref_paper_bwd.argtypes = [i64, i32, i32, dp, dp, dp, dp, dp, dp, u8p, dp, i32, dp, dp, dp, dp, dp]
+        L.nasg_ref_paper_fwd.restype = i32
+        L.nasg_ref_paper_bwd.restype = i32
         L.sh_ref_basis.argtypes = [dp, dp, dp]
         L.nasg_ref_num_threads.restype = i32
         L.nasg_ref_set_num_threads.argtypes = [i32]
@@ -161,3 +166,37 @@ def sh_basis(d) -> tuple:
     Y, dY = np.empty(16), np.empty((16, 3))
     lib().sh_ref_basis(_p(d), _p(Y), _p(dY))
     return Y, dY
+
+
+# ---- paper-native parameter record (Table 8 activations, Supplementary C frame) -----------------
+def paper_frame(euler_raw) -> tuple:
+    """X, Z and their derivatives dX[i], dZ[i] with respect to the cosines (c_theta, c_phi, c_tau), eqs.(38)-(44)."""
+    e = _d(euler_raw)
+    X, Z, dX, dZ = np.empty(3), np.empty(3), np.empty((3, 3)), np.empty((3, 3))
+    lib().nasg_ref_paper_frame(_p(e), _p(X), _p(Z), _p(dX), _p(dZ))
+    return X, Z, dX, dZ
+
+
+def paper_fwd(inp: dict, norm_mode: int = 1) -> np.ndarray:
+    """colors [C,N,3] fp64 from the paper-native record: inp holds means, euler [K,N,3], shp [K,N,3], ampraw [K,3,N], dc."""
+    N, K, Cn = int(inp["N"]), int(inp["K"]), int(inp["C"])
+    means, eu, sp, aw, dc, campos = (_d(inp[k]) for k in ("means", "euler", "shp", "ampraw", "dc", "campos"))
+    vis = None if inp.get("vis") is None else np.ascontiguousarray(inp["vis"], dtype=np.uint8)
+    colors = np.empty((Cn, N, 3), dtype=np.float64)
+    rc = lib().nasg_ref_paper_fwd(N, K, Cn, _p(means), _p(eu), _p(sp), _p(aw), _p(dc), _p(campos), _p(vis), norm_mode, _p(colors))
+    assert rc == 0
+    return colors
+
+
+def paper_bwd(inp: dict, norm_mode: int = 1, g_colors: Optional[np.ndarray] = None) -> dict:
+    """fp64 gradients with respect to the RAW values: g_means, g_euler, g_shp, g_ampraw, g_dc."""
+    N, K, Cn = int(inp["N"]), int(inp["K"]), int(inp["C"])
+    means, eu, sp, aw, dc, campos = (_d(inp[k]) for k in ("means", "euler", "shp", "ampraw", "dc", "campos"))
+    gcol = _d(inp["g_colors"] if g_colors is None else g_colors)
+    vis = None if inp.get("vis") is None else np.ascontiguousarray(inp["vis"], dtype=np.uint8)
+    out = dict(g_means=np.empty((N, 3)), g_euler=np.empty((K, N, 3)), g_shp=np.empty((K, N, 3)),
+               g_ampraw=np.empty((K, 3, N)), g_dc=np.empty((3, N)))
+    rc = lib().nasg_ref_paper_bwd(N, K, Cn, _p(means), _p(eu), _p(sp), _p(aw), _p(dc), _p(campos), _p(vis), _p(gcol), norm_mode,
+                                  _p(out["g_means"]), _p(out["g_euler"]), _p(out["g_shp"]), _p(out["g_ampraw"]), _p(out["g_dc"]))
+    assert rc == 0
+    return out

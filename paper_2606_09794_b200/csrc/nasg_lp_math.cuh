@@ -38,7 +38,7 @@ namespace lp {
 // tile kernels were IMAD.MOV pair assembly. Halves are taken out (lo/hi) only for the scalar-only operations
 // (MUFU, compare + select, min/max, |x|) and put back with pack().
 // ---------------------------------------------------------------------------------------------
-#ifdef __CUDA_ARCH__
+#if defined(__CUDA_ARCH__) && !defined(NASG_LP_SCALAR)
 typedef unsigned long long f2;
 __device__ __forceinline__ f2 pack(float lo, float hi) { f2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
 __device__ __forceinline__ float lo(f2 v) { float a; asm("{ .reg .b32 t; mov.b64 {%0, t}, %1; }" : "=f"(a) : "l"(v)); return a; }

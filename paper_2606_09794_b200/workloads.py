@@ -19,7 +19,7 @@ import numpy as np
 
 # sub-stream tags (one independent stream per array)
 TAG_MEANS, TAG_CAMPOS, TAG_VIS, TAG_QUAT, TAG_BW, TAG_FREQ, TAG_PHASE = 0, 1, 2, 3, 4, 5, 6
-TAG_AMP, TAG_DC, TAG_GCOL, TAG_SH = 7, 8, 9, 10
+TAG_AMP, TAG_DC, TAG_GCOL, TAG_SH, TAG_EULER = 7, 8, 9, 10, 11
 
 
 @dataclass(frozen=True)
@@ -92,6 +92,29 @@ def make_nasg(cfg: Config, N: Optional[int] = None) -> dict:
     return out
 
 
+def make_paper(cfg: Config, N: Optional[int] = None) -> dict:
+    """The same config with the paper-native parameter record (include/nasg.h: nasg_paper_*; Table 8): RAW
+    (pre-activation) values, drawn directly so that this module applies no activation: euler [K,N,3] ~ U[-1.8,1.8]
+    (cosines tanh(raw) in +-0.947), shp [K,N,3] = (lambda_raw = the smaller of the two log-bandwidth draws, a_raw = their
+    difference - 0.5, k_raw ~ U[-2.5,-0.7], i.e. k in [0.3,7.9]; the high-frequency config U[-1.1,-0.2], k in [4,16]),
+    ampraw ~ N(0,0.3), dc ~ N(0,0.3); geometry, masks and g_colors as make_nasg."""
+    assert cfg.kind == "nasg"
+    out = make_geometry(cfg, N)
+    N, K = out["N"], cfg.K
+    euler = _rng(cfg.seed, TAG_EULER).uniform(-1.8, 1.8, size=(K, N, 3))
+    b = _rng(cfg.seed, TAG_BW).uniform(cfg.bw_range[0], cfg.bw_range[1], size=(K, N, 2))
+    kr = (-2.5, -0.7) if cfg.k_range[1] <= 8.0 else (-1.1, -0.2)
+    shp = np.empty((K, N, 3), dtype=np.float64)
+    shp[..., 0] = b.min(axis=2)
+    shp[..., 1] = b.max(axis=2) - b.min(axis=2) - 0.5
+    shp[..., 2] = _rng(cfg.seed, TAG_FREQ).uniform(kr[0], kr[1], size=(K, N))
+    ampraw = _rng(cfg.seed, TAG_AMP).normal(0.0, 0.3, size=(K, 3, N))
+    dc = _rng(cfg.seed, TAG_DC).normal(0.0, 0.3, size=(3, N))
+    out.update(K=K, euler=euler.astype(np.float32), shp=shp.astype(np.float32), ampraw=ampraw.astype(np.float32),
+               dc=dc.astype(np.float32))
+    return out
+
+
 def make_sh(cfg: Config, N: Optional[int] = None) -> dict:
     """Inputs of sh_eval_fwd/bwd (config 3): geometry of config 2 plus degree-3 coefficients."""
     assert cfg.kind == "sh"
@@ -137,36 +160,60 @@ def rec_floats(N: int, K: int) -> int:
     return ((N + REC_TILE - 1) // REC_TILE) * REC_TILE * (6 + 11 * K)
 
 
-def pack_records(means, quat, shape, amp, dc) -> np.ndarray:
-    """Row arrays -> float32 [T, 6 + 11 K, 32] records flattened (K even). Padding lanes: unit quaternion, zeros."""
-    K, N = quat.shape[0], quat.shape[1]
+def _pack(means, dc, comp) -> np.ndarray:
+    """means [N,3], dc [3,N], comp [K,N,M] (the M per-lobe components) -> float32 [T, 6 + M K, 32] flattened."""
+    K, N, M = comp.shape
     assert K % 2 == 0
     T = (N + REC_TILE - 1) // REC_TILE
     Np = T * REC_TILE
-
-    def padded(a, axis, fill=0.0):
-        pad = [(0, 0)] * a.ndim
-        pad[axis] = (0, Np - N)
-        return np.pad(a, pad, constant_values=fill)
-
-    rec = np.empty((T, 6 + 11 * K, REC_TILE), dtype=np.float32)
-    rec[:, 0:3, :] = padded(means, 0).reshape(T, REC_TILE, 3).transpose(0, 2, 1)
-    rec[:, 3:6, :] = padded(dc, 1).reshape(3, T, REC_TILE).transpose(1, 0, 2)
-    q = padded(quat, 1)
-    q[:, N:, 0] = 1.0
-    comp = np.concatenate([q, padded(shape, 1), padded(amp, 2).transpose(0, 2, 1)], axis=2)      # [K, Np, 11]
-    # [K/2, 2, T, 32, 11] -> [T, K/2, 11, 32, 2]
-    comp = comp.reshape(K // 2, 2, T, REC_TILE, 11).transpose(2, 0, 4, 3, 1)
-    rec[:, 6:, :] = comp.reshape(T, (K // 2) * 11 * 2, REC_TILE)
+    rec = np.empty((T, 6 + M * K, REC_TILE), dtype=np.float32)
+    rec[:, 0:3, :] = np.pad(means, ((0, Np - N), (0, 0))).reshape(T, REC_TILE, 3).transpose(0, 2, 1)
+    rec[:, 3:6, :] = np.pad(dc, ((0, 0), (0, Np - N))).reshape(3, T, REC_TILE).transpose(1, 0, 2)
+    comp = np.pad(comp, ((0, 0), (0, Np - N), (0, 0)))
+    # [K/2, 2, T, 32, M] -> [T, K/2, M, 32, 2]
+    comp = comp.reshape(K // 2, 2, T, REC_TILE, M).transpose(2, 0, 4, 3, 1)
+    rec[:, 6:, :] = comp.reshape(T, (K // 2) * M * 2, REC_TILE)
     return rec.reshape(-1)
+
+
+def _unpack(rec, N: int, K: int, M: int):
+    T = (N + REC_TILE - 1) // REC_TILE
+    rec = np.asarray(rec).reshape(T, 6 + M * K, REC_TILE)
+    means = rec[:, 0:3, :].transpose(0, 2, 1).reshape(T * REC_TILE, 3)[:N]
+    dc = rec[:, 3:6, :].transpose(1, 0, 2).reshape(3, T * REC_TILE)[:, :N]
+    comp = rec[:, 6:, :].reshape(T, K // 2, M, REC_TILE, 2).transpose(1, 4, 0, 3, 2).reshape(K, T * REC_TILE, M)[:, :N]
+    return np.ascontiguousarray(means), np.ascontiguousarray(dc), comp
+
+
+def pack_records(means, quat, shape, amp, dc) -> np.ndarray:
+    """Row arrays -> float32 [T, 6 + 11 K, 32] records flattened (K even). Padding lanes: unit quaternion, zeros."""
+    N = quat.shape[1]
+    rec = _pack(means, dc, np.concatenate([quat, shape, amp.transpose(0, 2, 1)], axis=2))
+    if N % REC_TILE:
+        K = quat.shape[0]
+        r = rec.reshape(-1, 6 + 11 * K, REC_TILE)
+        r[-1, 6:].reshape(K // 2, 11, REC_TILE, 2)[:, 0, N % REC_TILE:, :] = 1.0       # quaternion w of the padding lanes
+    return rec
 
 
 def unpack_records(rec: np.ndarray, N: int, K: int) -> dict:
     """Inverse of pack_records (also for gradient records): dict means, quat, shape, amp, dc."""
-    T = (N + REC_TILE - 1) // REC_TILE
-    rec = np.asarray(rec).reshape(T, 6 + 11 * K, REC_TILE)
-    means = rec[:, 0:3, :].transpose(0, 2, 1).reshape(T * REC_TILE, 3)[:N]
-    dc = rec[:, 3:6, :].transpose(1, 0, 2).reshape(3, T * REC_TILE)[:, :N]
-    comp = rec[:, 6:, :].reshape(T, K // 2, 11, REC_TILE, 2).transpose(1, 4, 0, 3, 2).reshape(K, T * REC_TILE, 11)[:, :N]
-    return dict(means=np.ascontiguousarray(means), dc=np.ascontiguousarray(dc), quat=np.ascontiguousarray(comp[..., 0:4]),
-                shape=np.ascontiguousarray(comp[..., 4:8]), amp=np.ascontiguousarray(comp[..., 8:11].transpose(0, 2, 1)))
+    means, dc, comp = _unpack(rec, N, K, 11)
+    return dict(means=means, dc=dc, quat=np.ascontiguousarray(comp[..., 0:4]), shape=np.ascontiguousarray(comp[..., 4:8]),
+                amp=np.ascontiguousarray(comp[..., 8:11].transpose(0, 2, 1)))
+
+
+def paper_rec_floats(N: int, K: int) -> int:
+    return ((N + REC_TILE - 1) // REC_TILE) * REC_TILE * (6 + 9 * K)
+
+
+def pack_paper_records(means, euler, shp, ampraw, dc) -> np.ndarray:
+    """Paper-native record (3 + 9 K appearance floats per Gaussian) as tile records
+    float32 [T, 6 + 9 K, 32]: per lobe the components (theta, phi, tau, lambda, a, k, w_r, w_g, w_b), all RAW."""
+    return _pack(means, dc, np.concatenate([euler, shp, ampraw.transpose(0, 2, 1)], axis=2))
+
+
+def unpack_paper_records(rec: np.ndarray, N: int, K: int) -> dict:
+    means, dc, comp = _unpack(rec, N, K, 9)
+    return dict(means=means, dc=dc, euler=np.ascontiguousarray(comp[..., 0:3]), shp=np.ascontiguousarray(comp[..., 3:6]),
+                ampraw=np.ascontiguousarray(comp[..., 6:9].transpose(0, 2, 1)))
