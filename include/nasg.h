@@ -151,6 +151,22 @@ int nasg_rec_eval_fwd(const nasg_rec_inputs *in, float *colors, int norm_mode, v
 int nasg_rec_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float *g_params, int norm_mode,
                       void *cuda_stream);
 
+/* ---- the paper's own parameter record --------------------------------------
+ * 3 + 9 K appearance floats per primitive (Table 5) instead of 3 + 11 K: per lobe
+ * the RAW (pre-activation) values of Table 8, activations applied inside the kernels:
+ *     (c_theta, c_phi, c_tau) = tanh(raw), sines = +sqrt(1 - c^2)       frame of Supplementary C:
+ *     z = (c_theta s_phi, s_theta s_phi, c_phi),  x = (c_theta c_phi c_tau - s_theta s_tau, s_theta c_phi c_tau + c_theta s_tau, -s_phi c_tau)
+ *     lambda = exp(raw), a = exp(raw), k = 20 (tanh(raw) + 1), w = tanh(raw); no phase; c0 (dc) has no activation.
+ * Stored as tile records like the layout above with 9 components per lobe:
+ *     [192 + 576 j + 64 c + 2 lane + h],  c = 0..2 (theta, phi, tau) | 3..5 (lambda, a, k) | 6..8 amplitude (r,g,b)
+ * nasg_paper_floats(N, K) floats. The lobe function and the normaliser are those of nasg_eval_fwd (eq.(9), eq.(10)
+ * / norm_mode); the gradient record holds dL/d(raw) (the chain rule of eqs.(37)-(44), and of the
+ * activations, is applied inside the backward kernel). Same restrictions as nasg_rec_eval_*. */
+size_t nasg_paper_floats(int64_t N, int32_t K);
+int nasg_paper_eval_fwd(const nasg_rec_inputs *in, float *colors, int norm_mode, void *cuda_stream);
+int nasg_paper_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float *g_params, int norm_mode,
+                        void *cuda_stream);
+
 /* End-to-end with HOST buffers, as nasg_eval_fwd_bwd_host below: params / g_params are HOST record arrays, campos, vis,
  * g_colors, colors HOST arrays. A chunk of Gaussians is a contiguous block of records, so each chunk moves with one
  * copy per direction for the parameters / gradients plus one strided copy each for vis, g_colors and colors. Padding

@@ -201,7 +201,7 @@ static int check_rec_inputs(const nasg_rec_inputs *in, int norm_mode)
     return NASG_OK;
 }
 
-int nasg_rec_eval_fwd(const nasg_rec_inputs *in, float *colors, int norm_mode, void *cuda_stream)
+static int rec_eval_fwd(const nasg_rec_inputs *in, float *colors, int norm_mode, int pk, void *cuda_stream)
 {
     int rc = check_rec_inputs(in, norm_mode);
     if (rc != NASG_OK) return rc;
@@ -209,13 +209,13 @@ int nasg_rec_eval_fwd(const nasg_rec_inputs *in, float *colors, int norm_mode, v
     if (!colors) return NASG_ERR_NULL;
     const int bulk_rows = !in->vis || ((in->N & 15) == 0 && aligned16(in->vis));
     nasg::RecFwdParams p{in->N, in->C, bulk_rows, in->params, in->campos, in->vis, colors};
-    cudaError_t e = nasg::launch_nasg_rec_fwd(p, in->K, norm_mode, (cudaStream_t)cuda_stream);
+    cudaError_t e = nasg::launch_nasg_rec_fwd(p, in->K, norm_mode, pk, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return cuda_fail(e);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     return NASG_OK;
 }
 
-int nasg_rec_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float *g_params, int norm_mode, void *cuda_stream)
+static int rec_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float *g_params, int norm_mode, int pk, void *cuda_stream)
 {
     int rc = check_rec_inputs(in, norm_mode);
     if (rc != NASG_OK) return rc;
@@ -224,10 +224,34 @@ int nasg_rec_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float *g
     if (!aligned16(g_params)) return NASG_ERR_ALIGN;
     const int bulk_rows = (in->N & 3) == 0 && aligned16(g_colors) && (!in->vis || ((in->N & 15) == 0 && aligned16(in->vis)));
     nasg::RecBwdParams p{in->N, in->C, bulk_rows, in->params, in->campos, in->vis, g_colors, g_params};
-    cudaError_t e = nasg::launch_nasg_rec_bwd(p, in->K, norm_mode, (cudaStream_t)cuda_stream);
+    cudaError_t e = nasg::launch_nasg_rec_bwd(p, in->K, norm_mode, pk, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return cuda_fail(e);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     return NASG_OK;
+}
+
+int nasg_rec_eval_fwd(const nasg_rec_inputs *in, float *colors, int norm_mode, void *cuda_stream)
+{
+    return rec_eval_fwd(in, colors, norm_mode, 0, cuda_stream);
+}
+int nasg_rec_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float *g_params, int norm_mode, void *cuda_stream)
+{
+    return rec_eval_bwd(in, g_colors, g_params, norm_mode, 0, cuda_stream);
+}
+
+// ---- paper-native record (Table 8 activations, Supplementary C frame, no phase): 9 floats per lobe
+size_t nasg_paper_floats(int64_t N, int32_t K)
+{
+    if (N <= 0 || !rec_K_ok(K)) return 0;
+    return (size_t)nasg::rec_total_floats(N, K, 1);
+}
+int nasg_paper_eval_fwd(const nasg_rec_inputs *in, float *colors, int norm_mode, void *cuda_stream)
+{
+    return rec_eval_fwd(in, colors, norm_mode, 1, cuda_stream);
+}
+int nasg_paper_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float *g_params, int norm_mode, void *cuda_stream)
+{
+    return rec_eval_bwd(in, g_colors, g_params, norm_mode, 1, cuda_stream);
 }
 
 size_t nasg_workspace_bytes(int64_t N, int32_t K, int32_t C)

@@ -106,8 +106,9 @@ NASG_HD f2 g_fun2(f2 x2, f2 ix, f2 t)
 //   else:                            Psi = Lambda/(1-e^{-2 Lambda}) e^{-Lambda}   2 S(s)
 // E1 = ex2 of (r-Lambda) or of (-Lambda); e^{-2 Lambda} = E1^2 (e^{-2r} or 1). The trigonometric side
 // is skipped when no active lane of the warp holds a lobe with s <= 0.05 (always in cfg4).
+// lg_root = log2(lambda sqrt(1+a)).
 template <bool EXACT, bool GRAD>
-NASG_HD void normaliser2(f2 l1, f2 l2, f2 Lam, f2 lam, f2 k, f2 &lgI, LobePairGrad &G)
+NASG_HD void normaliser2(f2 lg_root, f2 Lam, f2 lam, f2 k, f2 &lgI, LobePairGrad &G)
 {
     const f2 x = add2(lam, lam);
     const f2 em = ex2_2(scl2(x, -LOG2E));                                   // e^{-2 lambda}
@@ -118,8 +119,7 @@ NASG_HD void normaliser2(f2 l1, f2 l2, f2 Lam, f2 lam, f2 k, f2 &lgI, LobePairGr
     ps = fma2(x, ps, splat(-0.5f));
     ps = fma2(x, ps, splat(1.0f));
     const f2 one_m = sel2(lo(lam) > 0.125f, hi(lam) > 0.125f, sub2(splat(1.0f), em), mul2(x, ps));
-    // 1/(2I) = lambda sqrt(1+a) / (2 pi (1-e^{-2 lambda}) (1+Psi));  lambda sqrt(1+a) = e^{(l1+l2)/2}
-    const f2 lg_root = scl2(add2(l1, l2), 0.5f * LOG2E);
+    // 1/(2I) = lambda sqrt(1+a) / (2 pi (1-e^{-2 lambda}) (1+Psi))
     if (!EXACT) {
         lgI = sub2(lg_root, lg2_2(scl2(one_m, 2.0f * TWO_PI)));             // NASG: I = 2 pi (1-e^{-2 lambda})/(lambda sqrt(1+a))
         if (GRAD) {
@@ -229,7 +229,59 @@ NASG_HD void lobe_pair_setup(f2 w, f2 x, f2 y, f2 z, const f2 l1, const f2 l2, c
     L.lam2e = scl2(lam, 2.0f * LOG2E);
     L.k = MODE == 2 ? splat(0.f) : k0;
     L.phi = MODE == 2 ? splat(0.f) : phi0;
-    normaliser2<MODE == 1, GRAD>(l1, l2, Lam, lam, k0, L.lgI, G);
+    normaliser2<MODE == 1, GRAD>(scl2(add2(l1, l2), 0.5f * LOG2E), Lam, lam, k0, L.lgI, G);   // lambda sqrt(1+a) = e^{(l1+l2)/2}
+}
+
+// ---------------------------------------------------------------------------------------------
+// Paper-native parameter record (Table 8, Supplementary C; include/nasg.h: nasg_paper_*): the lobe pair is
+// given by RAW values: frame angles (theta, phi, tau) with cos = tanh(raw), sin = +sqrt(1 - cos^2) = sech(raw);
+// lambda = exp(raw), a = exp(raw), k = 20 (tanh(raw) + 1), w = tanh(raw); no phase. [x y z] = Rz(theta) Ry(phi) Rz(tau).
+// tanh and sech come from h = e^{-|raw|} directly, cos = sign (1-h^2)/(1+h^2), sin = 2h/(1+h^2): the pair (cos, sin) is a
+// unit vector to fp32 rounding even when sin is tiny (sqrt(1 - cos^2) would lose it), so the frame stays orthonormal.
+// ---------------------------------------------------------------------------------------------
+#if defined(__CUDA_ARCH__) && !defined(NASG_LP_SCALAR)
+__device__ __forceinline__ f2 copysign2(f2 mag, f2 sgn) { return (mag & 0x7fffffff7fffffffull) | (sgn & 0x8000000080000000ull); }
+#else
+NASG_HD f2 copysign2(f2 mag, f2 sgn) { return pack(copysignf(lo(mag), lo(sgn)), copysignf(hi(mag), hi(sgn))); }
+#endif
+// tanh(x) from t = e^{-2|x|}: sign(x) (1-t)/(1+t)
+NASG_HD f2 tanh2(f2 x)
+{
+    const f2 t = ex2_2(scl2(abs2(x), -2.0f * LOG2E));
+    return copysign2(mul2(sub2(splat(1.0f), t), rcp2(add2(t, splat(1.0f)))), x);
+}
+struct PaperTrig { f2 st, cp, sp, cu, su; };      // sin theta | cos, sin phi | cos, sin tau  (what the backward chain needs)
+
+template <int MODE, bool GRAD>
+NASG_HD void lobe_pair_setup_paper(f2 th, f2 ph, f2 ta, f2 lr, f2 ar, f2 kr, LobePair &L, LobePairGrad &G, PaperTrig &tr)
+{
+    f2 c[3], s[3];
+    const f2 raw[3] = {th, ph, ta};
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        const f2 h = ex2_2(scl2(abs2(raw[i]), -LOG2E));                     // e^{-|x|}
+        const f2 t = mul2(h, h);
+        const f2 r = rcp2(add2(t, splat(1.0f)));
+        c[i] = copysign2(mul2(sub2(splat(1.0f), t), r), raw[i]);           // tanh(x)
+        s[i] = mul2(add2(h, h), r);                                         // sech(x) = sqrt(1 - tanh^2)
+    }
+    const f2 ct = c[0], st = s[0], cp = c[1], sp = s[1], cu = c[2], su = s[2];
+    const f2 cpcu = mul2(cp, cu), cpsu = mul2(cp, su);
+    L.Xx = fma2(ct, cpcu, neg2(mul2(st, su))); L.Xy = fma2(st, cpcu, mul2(ct, su)); L.Xz = neg2(mul2(sp, cu));
+    L.Yx = neg2(fma2(ct, cpsu, mul2(st, cu))); L.Yy = fma2(ct, cu, neg2(mul2(st, cpsu))); L.Yz = mul2(sp, su);
+    L.Zx = mul2(ct, sp); L.Zy = mul2(st, sp); L.Zz = cp;
+    if (GRAD) { tr.st = st; tr.cp = cp; tr.sp = sp; tr.cu = cu; tr.su = su; }
+    const f2 lam = ex2_2(scl2(lr, LOG2E));
+    const f2 a = ex2_2(scl2(ar, LOG2E));
+    const f2 one_pa = add2(a, splat(1.0f));
+    L.a = a;
+    L.lam2e = scl2(lam, 2.0f * LOG2E);
+    f2 k = splat(0.f);
+    if (MODE != 2) k = fma2(tanh2(kr), splat(20.0f), splat(20.0f));        // 20 (tanh + 1)
+    L.k = k;
+    L.phi = splat(0.f);
+    // log2(lambda sqrt(1+a)) = raw_lambda log2(e) + log2(1+a)/2
+    normaliser2<MODE == 1, GRAD>(fma2(lr, splat(LOG2E), scl2(lg2_2(one_pa), 0.5f)), mul2(lam, one_pa), lam, k, L.lgI, G);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -422,6 +474,36 @@ NASG_HD void lobe_pair_finish2(const LobePair &L, const LobePairGrad &Gd, const 
     gqx = fma2(neg2(qw), A.th0, fma2(qy, A.th2, mul2(neg2(qz), A.th1)));
     gqy = fma2(qw, A.th1, fma2(neg2(qz), A.th0, mul2(neg2(qx), A.th2)));
     gqz = fma2(qw, A.th2, fma2(qx, A.th1, mul2(qy, A.th0)));
+}
+
+// gradients with respect to the 9 raw values of both lobes from the accumulators (eqs.(37)-(44) in rotation-vector
+// form: for R = Rz(theta) Ry(phi) Rz(tau) the body-frame rotation vectors of the three angles are e3 (tau),
+// (sin tau, cos tau, 0) (phi) and (-sin phi cos tau, sin phi sin tau, cos phi) (theta); d angle / d raw = -sin(angle),
+// so the 1/sin of eq.(36) cancels against tanh' = sin^2), w = activated amplitudes.
+template <int MODE>
+NASG_HD void lobe_pair_finish_paper(const LobePair &L, const LobePairGrad &Gd, const AccPair &A, const PaperTrig &tr, f2 w0, f2 w1, f2 w2,
+                                    f2 &gth, f2 &gph, f2 &gta, f2 &glr, f2 &gar, f2 &gkr, f2 &gw0, f2 &gw1, f2 &gw2)
+{
+    const f2 one_pa = add2(L.a, splat(1.0f));
+    const f2 gl1 = fma2(scl2(A.S2, 0.5f), one_pa, mul2(neg2(A.S0), Gd.nA));            // (1+a) dL/da
+    glr = fma2(scl2(L.lam2e, LN2), A.S1, mul2(neg2(A.S0), Gd.nL));                       // lambda dL/dlambda
+    gar = mul2(gl1, mul2(L.a, rcp2(one_pa)));                                            // a dL/da
+    if (MODE != 2) {
+        const f2 gk = fma2(neg2(A.S0), Gd.nk, neg2(A.Sk));
+        gkr = mul2(gk, mul2(L.k, fma2(L.k, splat(-0.05f), splat(2.0f))));                // dk/draw = 20 (1 - tanh^2) = k (2 - k/20)
+    } else {
+        gkr = splat(0.f);
+    }
+    gw0 = mul2(A.gw0, fma2(neg2(w0), w0, splat(1.0f)));
+    gw1 = mul2(A.gw1, fma2(neg2(w1), w1, splat(1.0f)));
+    gw2 = mul2(A.gw2, fma2(neg2(w2), w2, splat(1.0f)));
+    // g_theta (rotation vector in the lobe frame) = (-th0, th1, th2)
+    const f2 g_tau = A.th2;
+    const f2 g_phi = fma2(tr.cu, A.th1, mul2(neg2(tr.su), A.th0));
+    const f2 g_the = fma2(tr.sp, fma2(tr.su, A.th1, mul2(tr.cu, A.th0)), mul2(tr.cp, A.th2));
+    gta = mul2(neg2(tr.su), g_tau);
+    gph = mul2(neg2(tr.sp), g_phi);
+    gth = mul2(neg2(tr.st), g_the);
 }
 
 } // namespace lp

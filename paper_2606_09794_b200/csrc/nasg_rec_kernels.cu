@@ -49,10 +49,16 @@ using namespace bulk;
 constexpr int FWD_TB = NASG_REC_FWD_TB, BWD_TB = NASG_REC_BWD_TB;     // threads per block (warps are independent: any multiple of 32)
 constexpr int WT = 32;                  // Gaussians per tile record
 constexpr int HDR_FLOATS = 6 * WT;      // means + dc
-constexpr int PAIR_FLOATS = 11 * 2 * WT;
 constexpr int HDR_BYTES = HDR_FLOATS * 4;       // 768
-constexpr int PAIR_BYTES = PAIR_FLOATS * 4;     // 2816
-__host__ __device__ constexpr int rec_floats(int K) { return HDR_FLOATS + (K / 2) * PAIR_FLOATS; }
+// PK = parameter kind of the record: 0 = quaternion + (log Lambda, log lambda, k, phi) + amplitude: 11 components per lobe;
+//      1 = the paper's own record (Table 8, Supplementary C): 3 frame angles + (lambda, a, k) + amplitude, all raw
+//          (pre-activation), no phase: 9 components per lobe (3 + 9 K appearance floats)
+template <int PK> struct Rec {
+    static constexpr int NCOMP = PK ? 9 : 11;
+    static constexpr int PAIR_FLOATS = NCOMP * 2 * WT;
+    static constexpr int PAIR_BYTES = PAIR_FLOATS * 4;        // 2816 | 2304
+    __host__ __device__ static constexpr int rec_floats(int K) { return HDR_FLOATS + (K / 2) * PAIR_FLOATS; }
+};
 
 #ifndef NASG_REC_FWD_STAGES
 #define NASG_REC_FWD_STAGES 3
@@ -69,11 +75,12 @@ __host__ __device__ constexpr int rec_floats(int K) { return HDR_FLOATS + (K / 2
 // header slot: record header (means, dc: 768 B) | backward: g_colors float [CT][32][3] | vis uint8 [CT][32]
 // scratch (backward, per-lane columns): cam float4 [CT][32] = (dx,dy,dz,1/|Delta|) | gcm float4 [CT][32] = masked
 //          g_colors | qs 2 x (f2,f2) [32] = qhat 2/|q| of the current pair
-template <int CT, bool BWD> struct Layout {
+template <int CT, bool BWD, int PK> struct Layout {
+    static constexpr int PAIR_BYTES = Rec<PK>::PAIR_BYTES;
     static constexpr int H_GC = HDR_BYTES;
     static constexpr int H_VIS = H_GC + (BWD ? CT * WT * 12 : 0);
     static constexpr int H_BYTES = H_VIS + ((CT * WT + 127) / 128) * 128;
-    static constexpr int SCRATCH = BWD ? (2 * CT + 2) * WT * 16 : 0;
+    static constexpr int SCRATCH = BWD ? (2 * CT + (PK ? 3 : 2)) * WT * 16 : 0;       // cam, gcm, parked frame terms (qs | trig)
     __host__ __device__ static constexpr int region(int stages, int hslots) { return stages * PAIR_BYTES + hslots * H_BYTES + SCRATCH + 64; }
 };
 
@@ -87,13 +94,14 @@ struct Warp {                            // warp-uniform state
 struct StageCursor { const char *src; int tile, j; };
 struct HdrCursor { const char *src; const char *gc; const uint8_t *vis; int tile; };
 
-template <int NPAIR>
+template <int NPAIR, int PAIR_BYTES>
 __device__ __forceinline__ void stage_advance(StageCursor &s, int tstride, int64_t rec_jump)
 {
     s.src += PAIR_BYTES;
     if (++s.j == NPAIR) { s.j = 0; s.tile += tstride; s.src += rec_jump; }
 }
 // (elected lane) lobe pair under the cursor -> stage slot `dst`, completing on `bar`
+template <int PAIR_BYTES>
 __device__ __forceinline__ void stage_issue(const StageCursor &s, int T, unsigned dst, unsigned bar)
 {
     if (s.tile < T) {
@@ -105,7 +113,7 @@ __device__ __forceinline__ void stage_issue(const StageCursor &s, int T, unsigne
 template <int CT, bool BWD>
 __device__ __forceinline__ void hdr_issue(const HdrCursor &h, const Warp &w, unsigned dst, unsigned bar, bool bulk_rows, int64_t N)
 {
-    using L = Layout<CT, BWD>;
+    using L = Layout<CT, BWD, 0>;           // (the header slot does not depend on the parameter kind)
     if (h.tile < w.T) {
         const unsigned cnt = h.tile == w.T - 1 ? w.last_cnt : (unsigned)WT;
         unsigned bytes = HDR_BYTES;
@@ -127,23 +135,23 @@ __device__ __forceinline__ void hdr_issue(const HdrCursor &h, const Warp &w, uns
     }
 }
 template <bool BWD>
-__device__ __forceinline__ void hdr_advance(HdrCursor &h, int tstride, int K)
+__device__ __forceinline__ void hdr_advance(HdrCursor &h, int tstride, int rec_bytes)
 {
     h.tile += tstride;
-    h.src += (int64_t)tstride * (rec_floats(K) * 4);
+    h.src += (int64_t)tstride * rec_bytes;
     if (BWD) h.gc += (int64_t)tstride * (WT * 12);
     if (h.vis) h.vis += (int64_t)tstride * WT;
 }
 
-template <int CT, bool BWD>
+template <int CT, bool BWD, int PK>
 __device__ __forceinline__ void warp_init(Warp &w, unsigned char *smem, int stages, int hslots, int64_t N)
 {
-    using L = Layout<CT, BWD>;
+    using L = Layout<CT, BWD, PK>;
     constexpr int NWARP = (BWD ? BWD_TB : FWD_TB) / 32;
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     const int region = L::region(stages, hslots);
     w.stage0 = smem_u32(smem) + (unsigned)warp * (unsigned)region;
-    w.hdr0 = w.stage0 + (unsigned)stages * PAIR_BYTES;
+    w.hdr0 = w.stage0 + (unsigned)stages * L::PAIR_BYTES;
     w.scr = w.hdr0 + (unsigned)hslots * (unsigned)L::H_BYTES;
     w.bars = w.stage0 + (unsigned)region - 64u;
     w.T = (int)((N + WT - 1) / WT);
@@ -159,14 +167,28 @@ __device__ __forceinline__ void warp_init(Warp &w, unsigned char *smem, int stag
 __device__ __forceinline__ unsigned bar_full(const Warp &w, int s) { return w.bars + 8u * s; }
 __device__ __forceinline__ unsigned bar_hfull(const Warp &w, int h) { return w.bars + 32u + 8u * h; }
 
-// the 11 operand pairs (lobe 2j, lobe 2j+1) of this lane: 64-bit loads, conflict-free, no re-assembly
-struct PairRegs { f2 qw, qx, qy, qz, l1, l2, k, phi, w0, w1, w2; };
-__device__ __forceinline__ void load_pair(unsigned stage, int lane, PairRegs &r)
+// the operand pairs (lobe 2j, lobe 2j+1) of this lane: 64-bit loads, conflict-free, no re-assembly
+template <int PK> struct PairRegs { f2 v[Rec<PK>::NCOMP]; };
+template <int PK>
+__device__ __forceinline__ void load_pair(unsigned stage, int lane, PairRegs<PK> &r)
 {
     const unsigned a = stage + lane * 8;
-    r.qw = lds64<f2>(a); r.qx = lds64<f2>(a + 256); r.qy = lds64<f2>(a + 512); r.qz = lds64<f2>(a + 768);
-    r.l1 = lds64<f2>(a + 1024); r.l2 = lds64<f2>(a + 1280); r.k = lds64<f2>(a + 1536); r.phi = lds64<f2>(a + 1792);
-    r.w0 = lds64<f2>(a + 2048); r.w1 = lds64<f2>(a + 2304); r.w2 = lds64<f2>(a + 2560);
+#pragma unroll
+    for (int c = 0; c < Rec<PK>::NCOMP; ++c) r.v[c] = lds64<f2>(a + 256 * c);
+}
+// set-up of the pair from its record components; w = the (activated) amplitudes
+template <int PK, int MODE, bool GRAD>
+__device__ __forceinline__ void setup_pair(const PairRegs<PK> &r, LobePair &Lp, LobePairGrad &Gd, f2 (&park)[6], f2 &w0, f2 &w1, f2 &w2)
+{
+    if (PK == 0) {
+        lobe_pair_setup<MODE, GRAD>(r.v[0], r.v[1], r.v[2], r.v[3], r.v[4], r.v[5], r.v[6], r.v[7], Lp, Gd, park[0], park[1], park[2], park[3]);
+        w0 = r.v[8]; w1 = r.v[9]; w2 = r.v[10];
+    } else {
+        PaperTrig tr;
+        lobe_pair_setup_paper<MODE, GRAD>(r.v[0], r.v[1], r.v[2], r.v[3], r.v[4], r.v[5], Lp, Gd, tr);
+        if (GRAD) { park[0] = tr.st; park[1] = tr.cp; park[2] = tr.sp; park[3] = tr.cu; park[4] = tr.su; park[5] = tr.su; }
+        w0 = tanh2(r.v[6]); w1 = tanh2(r.v[7]); w2 = tanh2(r.v[PK ? 8 : 0]);
+    }
 }
 
 __device__ __forceinline__ void direction(float mx, float my, float mz, const float *campos, int c, float &dx, float &dy, float &dz, float &inv)
@@ -187,18 +209,19 @@ __device__ __forceinline__ void st_cs2(float *p, f2 v)
 // ---------------------------------------------------------------------------------------------
 // forward
 // ---------------------------------------------------------------------------------------------
-template <int K, int CT, int MODE>
+template <int K, int CT, int MODE, int PK>
 __global__ void __launch_bounds__(FWD_TB, NASG_REC_FWD_MINB) nasg_rec_fwd_kernel(RecFwdParams p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int S = NASG_REC_FWD_STAGES, NPAIR = K / 2, HS = NASG_REC_FWD_HSLOTS;
-    using L = Layout<CT, false>;
-    constexpr int RECB = rec_floats(K) * 4;
+    using L = Layout<CT, false, PK>;
+    constexpr int PAIR_BYTES = Rec<PK>::PAIR_BYTES;
+    constexpr int RECB = Rec<PK>::rec_floats(K) * 4;
     const int lane = threadIdx.x & 31;
     const int64_t N = p.N;
     const bool bulk_rows = p.bulk_rows != 0;
     Warp w;
-    warp_init<CT, false>(w, smem_raw, S, HS, N);
+    warp_init<CT, false, PK>(w, smem_raw, S, HS, N);
     const int64_t rec_jump = (int64_t)w.tstride * RECB - (int64_t)NPAIR * PAIR_BYTES;
     const char *params = reinterpret_cast<const char *>(p.params);
     StageCursor sc{params + (int64_t)w.tile0 * RECB + HDR_BYTES, w.tile0, 0};
@@ -207,12 +230,12 @@ __global__ void __launch_bounds__(FWD_TB, NASG_REC_FWD_MINB) nasg_rec_fwd_kernel
 #pragma unroll
     for (int h = 0; h < HS; ++h) {
         if (elect_one()) hdr_issue<CT, false>(hc, w, w.hdr0 + h * L::H_BYTES, bar_hfull(w, h), bulk_rows, N);
-        hdr_advance<false>(hc, w.tstride, K);
+        hdr_advance<false>(hc, w.tstride, RECB);
     }
 #pragma unroll
     for (int m = 0; m < S; ++m) {
-        if (elect_one()) stage_issue(sc, w.T, w.stage0 + m * PAIR_BYTES, bar_full(w, m));
-        stage_advance<NPAIR>(sc, w.tstride, rec_jump);
+        if (elect_one()) stage_issue<PAIR_BYTES>(sc, w.T, w.stage0 + m * PAIR_BYTES, bar_full(w, m));
+        stage_advance<NPAIR, PAIR_BYTES>(sc, w.tstride, rec_jump);
     }
     int slot = 0, hslot = 0;
     unsigned par = 0, hpar = 0;
@@ -237,7 +260,7 @@ __global__ void __launch_bounds__(FWD_TB, NASG_REC_FWD_MINB) nasg_rec_fwd_kernel
         mask = valid ? mask : 0u;
         __syncwarp();
         if (elect_one()) hdr_issue<CT, false>(hc, w, hdr, bar_hfull(w, hslot), bulk_rows, N);
-        hdr_advance<false>(hc, w.tstride, K);
+        hdr_advance<false>(hc, w.tstride, RECB);
         if (++hslot == HS) { hslot = 0; hpar ^= 1u; }
         float dx[CT], dy[CT], dz[CT];
         f2 col[CT][3];
@@ -252,21 +275,21 @@ __global__ void __launch_bounds__(FWD_TB, NASG_REC_FWD_MINB) nasg_rec_fwd_kernel
         for (int j = 0; j < NPAIR; ++j) {
             const unsigned stage = w.stage0 + (unsigned)slot * PAIR_BYTES;
             mbar_wait(bar_full(w, slot), par);
-            PairRegs r;
-            load_pair(stage, lane, r);
+            PairRegs<PK> r;
+            load_pair<PK>(stage, lane, r);
             __syncwarp();
-            if (elect_one()) stage_issue(sc, w.T, stage, bar_full(w, slot));
-            stage_advance<NPAIR>(sc, w.tstride, rec_jump);
+            if (elect_one()) stage_issue<PAIR_BYTES>(sc, w.T, stage, bar_full(w, slot));
+            stage_advance<NPAIR, PAIR_BYTES>(sc, w.tstride, rec_jump);
             if (++slot == S) { slot = 0; par ^= 1u; }
-            LobePair Lp; LobePairGrad Gd; f2 u0, u1, u2, u3;
-            lobe_pair_setup<MODE, false>(r.qw, r.qx, r.qy, r.qz, r.l1, r.l2, r.k, r.phi, Lp, Gd, u0, u1, u2, u3);
+            LobePair Lp; LobePairGrad Gd; f2 park[6], w0, w1, w2;
+            setup_pair<PK, MODE, false>(r, Lp, Gd, park, w0, w1, w2);
 #pragma unroll
             for (int t = 0; t < CT; ++t) {     // every camera slot is evaluated (iid masks: some lane always needs it); culled slots are zeroed at the store
                 EvalPair T;
                 const f2 G = lobe_pair_eval<false, MODE != 2>(Lp, dx[t], dy[t], dz[t], T);
-                col[t][0] = fma2(r.w0, G, col[t][0]);
-                col[t][1] = fma2(r.w1, G, col[t][1]);
-                col[t][2] = fma2(r.w2, G, col[t][2]);
+                col[t][0] = fma2(w0, G, col[t][0]);
+                col[t][1] = fma2(w1, G, col[t][1]);
+                col[t][2] = fma2(w2, G, col[t][2]);
             }
         }
         if (valid) {
@@ -286,32 +309,33 @@ __global__ void __launch_bounds__(FWD_TB, NASG_REC_FWD_MINB) nasg_rec_fwd_kernel
 // ---------------------------------------------------------------------------------------------
 // backward
 // ---------------------------------------------------------------------------------------------
-template <int K, int CT, int MODE>
+template <int K, int CT, int MODE, int PK>
 __global__ void __launch_bounds__(BWD_TB, NASG_REC_BWD_MINB) nasg_rec_bwd_kernel(RecBwdParams p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int S = NASG_REC_BWD_STAGES, NPAIR = K / 2;
-    using L = Layout<CT, true>;
-    constexpr int RECF = rec_floats(K), RECB = RECF * 4;
+    using L = Layout<CT, true, PK>;
+    constexpr int PAIR_BYTES = Rec<PK>::PAIR_BYTES, PAIR_FLOATS = Rec<PK>::PAIR_FLOATS;
+    constexpr int RECF = Rec<PK>::rec_floats(K), RECB = RECF * 4;
     const int lane = threadIdx.x & 31;
     const int64_t N = p.N;
     const bool bulk_rows = p.bulk_rows != 0;
     Warp w;
-    warp_init<CT, true>(w, smem_raw, S, 1, N);
+    warp_init<CT, true, PK>(w, smem_raw, S, 1, N);
     const unsigned scr_cam = w.scr + lane * 16;                          // + t * WT * 16: (dx,dy,dz,1/|Delta|) of camera t
     const unsigned scr_gc = scr_cam + CT * WT * 16;                      // + t * WT * 16: masked g_colors of camera t
-    const unsigned scr_qs = scr_gc + CT * WT * 16;                       // + {0, WT * 16}
+    const unsigned scr_qs = scr_gc + CT * WT * 16;                       // + {0, WT * 16[, 2 WT * 16]}: parked frame terms
     const int64_t rec_jump = (int64_t)w.tstride * RECB - (int64_t)NPAIR * PAIR_BYTES;
     const char *params = reinterpret_cast<const char *>(p.params);
     StageCursor sc{params + (int64_t)w.tile0 * RECB + HDR_BYTES, w.tile0, 0};
     HdrCursor hc{params + (int64_t)w.tile0 * RECB, reinterpret_cast<const char *>(p.g_colors) + (int64_t)w.tile0 * (WT * 12),
                  p.vis ? p.vis + (int64_t)w.tile0 * WT : nullptr, w.tile0};
     if (elect_one()) hdr_issue<CT, true>(hc, w, w.hdr0, bar_hfull(w, 0), bulk_rows, N);
-    hdr_advance<true>(hc, w.tstride, K);
+    hdr_advance<true>(hc, w.tstride, RECB);
 #pragma unroll
     for (int m = 0; m < S; ++m) {
-        if (elect_one()) stage_issue(sc, w.T, w.stage0 + m * PAIR_BYTES, bar_full(w, m));
-        stage_advance<NPAIR>(sc, w.tstride, rec_jump);
+        if (elect_one()) stage_issue<PAIR_BYTES>(sc, w.T, w.stage0 + m * PAIR_BYTES, bar_full(w, m));
+        stage_advance<NPAIR, PAIR_BYTES>(sc, w.tstride, rec_jump);
     }
     int slot = 0;
     unsigned par = 0, hpar = 0;
@@ -348,7 +372,7 @@ __global__ void __launch_bounds__(BWD_TB, NASG_REC_BWD_MINB) nasg_rec_bwd_kernel
         }
         __syncwarp();
         if (elect_one()) hdr_issue<CT, true>(hc, w, w.hdr0, bar_hfull(w, 0), bulk_rows, N);
-        hdr_advance<true>(hc, w.tstride, K);
+        hdr_advance<true>(hc, w.tstride, RECB);
         float gd[CT][3];
 #pragma unroll
         for (int t = 0; t < CT; ++t) gd[t][0] = gd[t][1] = gd[t][2] = 0.f;
@@ -358,18 +382,20 @@ __global__ void __launch_bounds__(BWD_TB, NASG_REC_BWD_MINB) nasg_rec_bwd_kernel
         for (int j = 0; j < NPAIR; ++j) {
             const unsigned stage = w.stage0 + (unsigned)slot * PAIR_BYTES;
             mbar_wait(bar_full(w, slot), par);
-            PairRegs r;
-            load_pair(stage, lane, r);
+            PairRegs<PK> r;
+            load_pair<PK>(stage, lane, r);
             __syncwarp();
-            if (elect_one()) stage_issue(sc, w.T, stage, bar_full(w, slot));
-            stage_advance<NPAIR>(sc, w.tstride, rec_jump);
+            if (elect_one()) stage_issue<PAIR_BYTES>(sc, w.T, stage, bar_full(w, slot));
+            stage_advance<NPAIR, PAIR_BYTES>(sc, w.tstride, rec_jump);
             if (++slot == S) { slot = 0; par ^= 1u; }
             LobePair Lp; LobePairGrad Gd;
-            {
-                f2 qsw, qsx, qsy, qsz;
-                lobe_pair_setup<MODE, true>(r.qw, r.qx, r.qy, r.qz, r.l1, r.l2, r.k, r.phi, Lp, Gd, qsw, qsx, qsy, qsz);
-                sts64x2(scr_qs, qsw, qsx);
-                sts64x2(scr_qs + WT * 16, qsy, qsz);
+            f2 w0, w1, w2;
+            {       // frame terms the end of the pair needs (quaternion 2/|q| | sines and cosines of the angles) are parked in shared memory
+                f2 park[6];
+                setup_pair<PK, MODE, true>(r, Lp, Gd, park, w0, w1, w2);
+                sts64x2(scr_qs, park[0], park[1]);
+                sts64x2(scr_qs + WT * 16, park[2], park[3]);
+                if (PK) sts64x2(scr_qs + 2 * WT * 16, park[4], park[5]);
             }
             AccPair A;
 #pragma unroll
@@ -379,18 +405,24 @@ __global__ void __launch_bounds__(BWD_TB, NASG_REC_BWD_MINB) nasg_rec_bwd_kernel
                 EvalPair T;
                 const f2 G = lobe_pair_eval<true, MODE != 2>(Lp, cam.x, cam.y, cam.z, T);
                 f2 gx = splat(0.f), gy = splat(0.f), gz = splat(0.f);
-                if (t == 0) lobe_pair_bwd<MODE != 2, true>(Lp, T, G, gc.x, gc.y, gc.z, r.w0, r.w1, r.w2, A, gx, gy, gz);
-                else lobe_pair_bwd<MODE != 2, false>(Lp, T, G, gc.x, gc.y, gc.z, r.w0, r.w1, r.w2, A, gx, gy, gz);
+                if (t == 0) lobe_pair_bwd<MODE != 2, true>(Lp, T, G, gc.x, gc.y, gc.z, w0, w1, w2, A, gx, gy, gz);
+                else lobe_pair_bwd<MODE != 2, false>(Lp, T, G, gc.x, gc.y, gc.z, w0, w1, w2, A, gx, gy, gz);
                 gd[t][0] += lo(gx) + hi(gx); gd[t][1] += lo(gy) + hi(gy); gd[t][2] += lo(gz) + hi(gz);
             }
-            f2 qsw, qsx, qsy, qsz, gl1, gl2, gk, gphi, gqw, gqx, gqy, gqz;
-            lds64x2(scr_qs, qsw, qsx);
-            lds64x2(scr_qs + WT * 16, qsy, qsz);
-            lobe_pair_finish2(Lp, Gd, A, qsw, qsx, qsy, qsz, gl1, gl2, gk, gphi, gqw, gqx, gqy, gqz);
+            f2 park[6], g[Rec<PK>::NCOMP];
+            lds64x2(scr_qs, park[0], park[1]);
+            lds64x2(scr_qs + WT * 16, park[2], park[3]);
+            if (PK) {
+                lds64x2(scr_qs + 2 * WT * 16, park[4], park[5]);
+                const PaperTrig tr{park[0], park[1], park[2], park[3], park[4]};
+                lobe_pair_finish_paper<MODE>(Lp, Gd, A, tr, w0, w1, w2, g[0], g[1], g[2], g[3], g[4], g[5], g[6], g[7], g[PK ? 8 : 0]);
+            } else {
+                lobe_pair_finish2(Lp, Gd, A, park[0], park[1], park[2], park[3], g[4], g[5], g[6], g[7], g[0], g[1], g[2], g[3]);
+                g[8] = A.gw0; g[9] = A.gw1; g[PK ? 0 : 10] = A.gw2;
+            }
             if (valid) {
-                st_cs2(gpair, gqw); st_cs2(gpair + 64, gqx); st_cs2(gpair + 128, gqy); st_cs2(gpair + 192, gqz);
-                st_cs2(gpair + 256, gl1); st_cs2(gpair + 320, gl2); st_cs2(gpair + 384, gk); st_cs2(gpair + 448, gphi);
-                st_cs2(gpair + 512, A.gw0); st_cs2(gpair + 576, A.gw1); st_cs2(gpair + 640, A.gw2);
+#pragma unroll
+                for (int c = 0; c < Rec<PK>::NCOMP; ++c) st_cs2(gpair + 64 * c, g[c]);
             }
             gpair += PAIR_FLOATS;
         }
@@ -419,7 +451,7 @@ __global__ void __launch_bounds__(256) rec_pack_kernel(int64_t N, int K, const f
     const int64_t T = (N + WT - 1) / WT;
     if (n >= T * WT) return;
     const int lane = (int)(n & 31);
-    float *r = rec + (n >> 5) * rec_floats(K);
+    float *r = rec + (n >> 5) * Rec<0>::rec_floats(K);
     const bool valid = n < N;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
@@ -427,7 +459,7 @@ __global__ void __launch_bounds__(256) rec_pack_kernel(int64_t N, int K, const f
         r[(3 + c) * WT + lane] = valid ? dc[(int64_t)c * N + n] : 0.f;
     }
     for (int l = 0; l < K; ++l) {
-        float *o = r + HDR_FLOATS + (l >> 1) * PAIR_FLOATS + 2 * lane + (l & 1);
+        float *o = r + HDR_FLOATS + (l >> 1) * Rec<0>::PAIR_FLOATS + 2 * lane + (l & 1);
         float4 q = make_float4(1.f, 0.f, 0.f, 0.f), s = make_float4(0.f, 0.f, 0.f, 0.f);
         float a0 = 0.f, a1 = 0.f, a2 = 0.f;
         if (valid) {
@@ -446,14 +478,14 @@ __global__ void __launch_bounds__(256) rec_unpack_kernel(int64_t N, int K, const
     const int64_t n = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (n >= N) return;
     const int lane = (int)(n & 31);
-    const float *r = rec + (n >> 5) * rec_floats(K);
+    const float *r = rec + (n >> 5) * Rec<0>::rec_floats(K);
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         if (means) means[3 * n + c] = r[c * WT + lane];
         if (dc) dc[(int64_t)c * N + n] = r[(3 + c) * WT + lane];
     }
     for (int l = 0; l < K; ++l) {
-        const float *o = r + HDR_FLOATS + (l >> 1) * PAIR_FLOATS + 2 * lane + (l & 1);
+        const float *o = r + HDR_FLOATS + (l >> 1) * Rec<0>::PAIR_FLOATS + 2 * lane + (l & 1);
         if (quat) reinterpret_cast<float4 *>(quat)[(int64_t)l * N + n] = make_float4(o[0], o[64], o[128], o[192]);
         if (shape) reinterpret_cast<float4 *>(shape)[(int64_t)l * N + n] = make_float4(o[256], o[320], o[384], o[448]);
         if (amp) { amp[((int64_t)l * 3 + 0) * N + n] = o[512]; amp[((int64_t)l * 3 + 1) * N + n] = o[576]; amp[((int64_t)l * 3 + 2) * N + n] = o[640]; }
@@ -467,7 +499,10 @@ namespace rec = lp::rec;
 // ---------------------------------------------------------------------------------------------
 // launchers: persistent grid = resident blocks (occupancy API, cached per instantiation and device)
 // ---------------------------------------------------------------------------------------------
-int64_t rec_total_floats(int64_t N, int K) { return ((N + rec::WT - 1) / rec::WT) * (int64_t)rec::rec_floats(K); }
+int64_t rec_total_floats(int64_t N, int K, int pk)
+{
+    return ((N + rec::WT - 1) / rec::WT) * (int64_t)(pk ? rec::Rec<1>::rec_floats(K) : rec::Rec<0>::rec_floats(K));
+}
 
 template <typename Kernel>
 static int rec_grid(Kernel kernel, int TB, size_t smem, int64_t N, int *cached)
@@ -487,70 +522,80 @@ static int rec_grid(Kernel kernel, int TB, size_t smem, int64_t N, int *cached)
     return (int)(need < resident ? need : resident);
 }
 
-template <int K, int CT>
+template <int K, int CT, int PK>
 static cudaError_t launch_rec_fwd_kc(const RecFwdParams &p, int mode, cudaStream_t st)
 {
     constexpr int TB = rec::FWD_TB;
-    constexpr size_t smem = (size_t)(TB / 32) * rec::Layout<CT, false>::region(NASG_REC_FWD_STAGES, NASG_REC_FWD_HSLOTS);
+    constexpr size_t smem = (size_t)(TB / 32) * rec::Layout<CT, false, PK>::region(NASG_REC_FWD_STAGES, NASG_REC_FWD_HSLOTS);
     static int cache[3][64] = {{0}};
     using namespace rec;
-    if (mode == 1) nasg_rec_fwd_kernel<K, CT, 1><<<rec_grid(nasg_rec_fwd_kernel<K, CT, 1>, TB, smem, p.N, cache[1]), TB, smem, st>>>(p);
-    else if (mode == 0) nasg_rec_fwd_kernel<K, CT, 0><<<rec_grid(nasg_rec_fwd_kernel<K, CT, 0>, TB, smem, p.N, cache[0]), TB, smem, st>>>(p);
-    else nasg_rec_fwd_kernel<K, CT, 2><<<rec_grid(nasg_rec_fwd_kernel<K, CT, 2>, TB, smem, p.N, cache[2]), TB, smem, st>>>(p);
+    if (mode == 1) nasg_rec_fwd_kernel<K, CT, 1, PK><<<rec_grid(nasg_rec_fwd_kernel<K, CT, 1, PK>, TB, smem, p.N, cache[1]), TB, smem, st>>>(p);
+    else if (mode == 0) nasg_rec_fwd_kernel<K, CT, 0, PK><<<rec_grid(nasg_rec_fwd_kernel<K, CT, 0, PK>, TB, smem, p.N, cache[0]), TB, smem, st>>>(p);
+    else nasg_rec_fwd_kernel<K, CT, 2, PK><<<rec_grid(nasg_rec_fwd_kernel<K, CT, 2, PK>, TB, smem, p.N, cache[2]), TB, smem, st>>>(p);
     return cudaGetLastError();
 }
-template <int K>
+template <int K, int PK>
 static cudaError_t launch_rec_fwd_k(const RecFwdParams &p, int mode, cudaStream_t st)
 {
     switch (p.C) {
-    case 1: return launch_rec_fwd_kc<K, 1>(p, mode, st);
-    case 2: return launch_rec_fwd_kc<K, 2>(p, mode, st);
-    case 3: return launch_rec_fwd_kc<K, 3>(p, mode, st);
-    case 4: return launch_rec_fwd_kc<K, 4>(p, mode, st);
+    case 1: return launch_rec_fwd_kc<K, 1, PK>(p, mode, st);
+    case 2: return launch_rec_fwd_kc<K, 2, PK>(p, mode, st);
+    case 3: return launch_rec_fwd_kc<K, 3, PK>(p, mode, st);
+    case 4: return launch_rec_fwd_kc<K, 4, PK>(p, mode, st);
     default: return cudaErrorInvalidValue;
     }
 }
-cudaError_t launch_nasg_rec_fwd(const RecFwdParams &p, int K, int mode, cudaStream_t st)
+template <int PK>
+static cudaError_t launch_rec_fwd_pk(const RecFwdParams &p, int K, int mode, cudaStream_t st)
 {
     switch (K) {
-    case 2: return launch_rec_fwd_k<2>(p, mode, st);
-    case 4: return launch_rec_fwd_k<4>(p, mode, st);
-    case 8: return launch_rec_fwd_k<8>(p, mode, st);
+    case 2: return launch_rec_fwd_k<2, PK>(p, mode, st);
+    case 4: return launch_rec_fwd_k<4, PK>(p, mode, st);
+    case 8: return launch_rec_fwd_k<8, PK>(p, mode, st);
     default: return cudaErrorInvalidValue;
     }
 }
+cudaError_t launch_nasg_rec_fwd(const RecFwdParams &p, int K, int mode, int pk, cudaStream_t st)
+{
+    return pk ? launch_rec_fwd_pk<1>(p, K, mode, st) : launch_rec_fwd_pk<0>(p, K, mode, st);
+}
 
-template <int K, int CT>
+template <int K, int CT, int PK>
 static cudaError_t launch_rec_bwd_kc(const RecBwdParams &p, int mode, cudaStream_t st)
 {
     constexpr int TB = rec::BWD_TB;
-    constexpr size_t smem = (size_t)(TB / 32) * rec::Layout<CT, true>::region(NASG_REC_BWD_STAGES, 1);
+    constexpr size_t smem = (size_t)(TB / 32) * rec::Layout<CT, true, PK>::region(NASG_REC_BWD_STAGES, 1);
     static int cache[3][64] = {{0}};
     using namespace rec;
-    if (mode == 1) nasg_rec_bwd_kernel<K, CT, 1><<<rec_grid(nasg_rec_bwd_kernel<K, CT, 1>, TB, smem, p.N, cache[1]), TB, smem, st>>>(p);
-    else if (mode == 0) nasg_rec_bwd_kernel<K, CT, 0><<<rec_grid(nasg_rec_bwd_kernel<K, CT, 0>, TB, smem, p.N, cache[0]), TB, smem, st>>>(p);
-    else nasg_rec_bwd_kernel<K, CT, 2><<<rec_grid(nasg_rec_bwd_kernel<K, CT, 2>, TB, smem, p.N, cache[2]), TB, smem, st>>>(p);
+    if (mode == 1) nasg_rec_bwd_kernel<K, CT, 1, PK><<<rec_grid(nasg_rec_bwd_kernel<K, CT, 1, PK>, TB, smem, p.N, cache[1]), TB, smem, st>>>(p);
+    else if (mode == 0) nasg_rec_bwd_kernel<K, CT, 0, PK><<<rec_grid(nasg_rec_bwd_kernel<K, CT, 0, PK>, TB, smem, p.N, cache[0]), TB, smem, st>>>(p);
+    else nasg_rec_bwd_kernel<K, CT, 2, PK><<<rec_grid(nasg_rec_bwd_kernel<K, CT, 2, PK>, TB, smem, p.N, cache[2]), TB, smem, st>>>(p);
     return cudaGetLastError();
 }
-template <int K>
+template <int K, int PK>
 static cudaError_t launch_rec_bwd_k(const RecBwdParams &p, int mode, cudaStream_t st)
 {
     switch (p.C) {
-    case 1: return launch_rec_bwd_kc<K, 1>(p, mode, st);
-    case 2: return launch_rec_bwd_kc<K, 2>(p, mode, st);
-    case 3: return launch_rec_bwd_kc<K, 3>(p, mode, st);
-    case 4: return launch_rec_bwd_kc<K, 4>(p, mode, st);
+    case 1: return launch_rec_bwd_kc<K, 1, PK>(p, mode, st);
+    case 2: return launch_rec_bwd_kc<K, 2, PK>(p, mode, st);
+    case 3: return launch_rec_bwd_kc<K, 3, PK>(p, mode, st);
+    case 4: return launch_rec_bwd_kc<K, 4, PK>(p, mode, st);
     default: return cudaErrorInvalidValue;
     }
 }
-cudaError_t launch_nasg_rec_bwd(const RecBwdParams &p, int K, int mode, cudaStream_t st)
+template <int PK>
+static cudaError_t launch_rec_bwd_pk(const RecBwdParams &p, int K, int mode, cudaStream_t st)
 {
     switch (K) {
-    case 2: return launch_rec_bwd_k<2>(p, mode, st);
-    case 4: return launch_rec_bwd_k<4>(p, mode, st);
-    case 8: return launch_rec_bwd_k<8>(p, mode, st);
+    case 2: return launch_rec_bwd_k<2, PK>(p, mode, st);
+    case 4: return launch_rec_bwd_k<4, PK>(p, mode, st);
+    case 8: return launch_rec_bwd_k<8, PK>(p, mode, st);
     default: return cudaErrorInvalidValue;
     }
+}
+cudaError_t launch_nasg_rec_bwd(const RecBwdParams &p, int K, int mode, int pk, cudaStream_t st)
+{
+    return pk ? launch_rec_bwd_pk<1>(p, K, mode, st) : launch_rec_bwd_pk<0>(p, K, mode, st);
 }
 
 cudaError_t launch_rec_pack(int64_t N, int K, const float *means, const float *quat, const float *shape, const float *amp, const float *dc,

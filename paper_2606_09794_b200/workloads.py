@@ -97,9 +97,14 @@ def make_paper(cfg: Config, N: Optional[int] = None) -> dict:
     (pre-activation) values, drawn directly so that this module applies no activation: euler [K,N,3] ~ U[-1.8,1.8]
     (cosines tanh(raw) in +-0.947), shp [K,N,3] = (lambda_raw = the smaller of the two log-bandwidth draws, a_raw = their
     difference - 0.5, k_raw ~ U[-2.5,-0.7], i.e. k in [0.3,7.9]; the high-frequency config U[-1.1,-0.2], k in [4,16]),
-    ampraw ~ N(0,0.3), dc ~ N(0,0.3); geometry, masks and g_colors as make_nasg."""
+    ampraw ~ N(0,0.3), dc ~ N(0,0.3); geometry, masks and g_colors as make_nasg, except that every camera is mirrored
+    into the y <= 0 half-space: with sin = +sqrt(1 - cos^2) the record's lobe axes z = (c s, s s, c) all have z_y >= 0
+    (SURVEY.md NEXT-2 "quirk"), so only view directions d = normalize(mean - campos) with d_y > 0 can
+    meet a lobe peak; a camera on the other side would see nothing but lobe tails."""
     assert cfg.kind == "nasg"
     out = make_geometry(cfg, N)
+    out["campos"] = out["campos"].copy()
+    out["campos"][:, 1] = -np.abs(out["campos"][:, 1])
     N, K = out["N"], cfg.K
     euler = _rng(cfg.seed, TAG_EULER).uniform(-1.8, 1.8, size=(K, N, 3))
     b = _rng(cfg.seed, TAG_BW).uniform(cfg.bw_range[0], cfg.bw_range[1], size=(K, N, 2))
