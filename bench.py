@@ -32,8 +32,8 @@ FALLBACK_HBM_GBS = 6650.0      # B200_PROFILING.md fallback when MEASURED_PEAKS.
 
 
 # ---- algorithmic bytes per Gaussian ------------------
-def algorithmic_bytes(kind: str, K: int, C: int, has_vis: bool):
-    P = 51 if kind == "sh" else 6 + 11 * K          # parameter floats per Gaussian (means+dc/coeffs+lobes)
+def algorithmic_bytes(kind: str, K: int, C: int, has_vis: bool, paper: bool = False):
+    P = 51 if kind == "sh" else 6 + (9 if paper else 11) * K      # parameter floats per Gaussian (means+dc/coeffs+lobes)
     vis = C if has_vis else 0
     fwd = 4 * P + vis + 12 * C                      # read params + mask, write colours
     bwd = 4 * P + vis + 12 * C + 4 * P              # read params + mask + g_colors, write every gradient
@@ -179,17 +179,22 @@ class Resident:
         import torch
         self.B, self.cfg, self.norm_mode, self.torch = B, cfg, norm_mode, torch
         rcfg = S.weak_scaling_config(cfg, rank)
-        inp = W.make_sh(rcfg) if cfg.kind == "sh" else W.make_nasg(rcfg)
+        self.paper = cfg.kind == "nasg" and layout == "paper"          # the paper's own 3 + 9K record (nasg_paper_*)
+        inp = W.make_sh(rcfg) if cfg.kind == "sh" else W.make_paper(rcfg) if self.paper else W.make_nasg(rcfg)
         self.N, self.C, self.K = inp["N"], inp["C"], inp.get("K", 0)
         # tile-record parameter layout (include/nasg.h: nasg_rec_*) where it applies, else the row arrays
-        self.rec = cfg.kind == "nasg" and layout == "rec" and self.K in (2, 4, 8) and self.C <= 4
-        self.keys = ("means", "coeffs", "campos", "vis", "g_colors") if cfg.kind == "sh" else \
+        self.rec = cfg.kind == "nasg" and layout in ("rec", "paper") and self.K in (2, 4, 8) and self.C <= 4
+        assert self.rec or not self.paper
+        self.keys = ("means", "coeffs", "campos", "vis", "g_colors") if cfg.kind == "sh" else ("campos", "vis", "g_colors") if self.paper else \
                     ("means", "quat", "shape", "amp", "dc", "campos", "vis", "g_colors")
         d = {k: (None if inp.get(k) is None else torch.from_numpy(np.ascontiguousarray(inp[k])).cuda()) for k in self.keys}
         self.d = d
         self.colors = torch.empty((self.C, self.N, 3), dtype=torch.float32, device="cuda")
         self.stream = torch.cuda.current_stream()
-        if self.rec:    # the parameters LIVE in HBM as records (packed once, outside any timed region: it is the storage layout)
+        if self.paper:  # records of raw values, re-ordered on the host by the input generator (no arithmetic)
+            self.params = torch.from_numpy(W.pack_paper_records(inp["means"], inp["euler"], inp["shp"], inp["ampraw"], inp["dc"])).cuda()
+            self.g_params = torch.zeros_like(self.params)
+        elif self.rec:  # the parameters LIVE in HBM as records (packed once, outside any timed region: it is the storage layout)
             self.params = B.nasg_rec_pack(d["means"], d["quat"], d["shape"], d["amp"], d["dc"])
             self.g_params = torch.zeros_like(self.params)
             for k in ("means", "quat", "shape", "amp", "dc"):
@@ -200,7 +205,9 @@ class Resident:
 
     def fwd(self):
         B, d, st = self.B, self.d, self.stream
-        if self.rec:
+        if self.paper:
+            B.nasg_paper_eval_fwd(self.params, self.N, self.K, d["campos"], d["vis"], self.norm_mode, out=self.colors, stream=st)
+        elif self.rec:
             B.nasg_rec_eval_fwd(self.params, self.N, self.K, d["campos"], d["vis"], self.norm_mode, out=self.colors, stream=st)
         elif self.cfg.kind == "sh":
             B.sh_eval_fwd(d["means"], d["coeffs"], d["campos"], d["vis"], out=self.colors, stream=st)
@@ -210,7 +217,10 @@ class Resident:
 
     def bwd(self):
         B, d, st = self.B, self.d, self.stream
-        if self.rec:
+        if self.paper:
+            B.nasg_paper_eval_bwd(self.params, self.N, self.K, d["campos"], d["g_colors"], d["vis"], self.norm_mode,
+                                  out=self.g_params, stream=st)
+        elif self.rec:
             B.nasg_rec_eval_bwd(self.params, self.N, self.K, d["campos"], d["g_colors"], d["vis"], self.norm_mode,
                                 out=self.g_params, stream=st)
         elif self.cfg.kind == "sh":
@@ -221,7 +231,7 @@ class Resident:
 
     def kernel_name(self):
         if self.rec:
-            return "nasg_rec_bwd_kernel"
+            return "nasg_rec_bwd_kernel<PK=1>" if self.paper else "nasg_rec_bwd_kernel"
         pipe = self.C <= 4
         if self.cfg.kind == "sh":
             return "sh_bwd_pipe_kernel" if pipe else "sh_bwd_kernel"
@@ -300,8 +310,8 @@ def run_ours(args, W, cfg):
     if rec:
         host["params"] = R.params.cpu().pin_memory()
         hout = dict(colors=torch.empty((C, N, 3)).pin_memory(), g_params=torch.empty(R.params.numel()).pin_memory())
-        scratch = torch.empty(B.nasg_rec_host_scratch_bytes(N, K, C), dtype=torch.uint8, device="cuda")
-        e2e_call = lambda: B.nasg_rec_eval_fwd_bwd_host(host, hout, N, K, scratch, args.norm_mode, stream=stream)
+        scratch = torch.empty((B.nasg_paper_host_scratch_bytes if R.paper else B.nasg_rec_host_scratch_bytes)(N, K, C), dtype=torch.uint8, device="cuda")
+        e2e_call = lambda: B.nasg_rec_eval_fwd_bwd_host(host, hout, N, K, scratch, args.norm_mode, stream=stream, paper=R.paper)
     elif cfg.kind == "sh":
         hout = dict(colors=torch.empty((C, N, 3)).pin_memory(), g_means=torch.empty((N, 3)).pin_memory(),
                     g_coeffs=torch.empty((16, 3, N)).pin_memory())
@@ -330,8 +340,8 @@ def run_ours(args, W, cfg):
     peak, peak_src = measured_peak()
 
     def summary(r, f_ms, b_ms):
-        fb, bb = algorithmic_bytes(r.cfg.kind, r.K, r.C, r.has_vis)
-        return {"layout": "records" if r.rec else "rows", "kernel": r.kernel_name(), "fwd_ms": f_ms, "bwd_ms": b_ms,
+        fb, bb = algorithmic_bytes(r.cfg.kind, r.K, r.C, r.has_vis, r.paper)
+        return {"layout": "paper records (3 + 9K floats)" if r.paper else "records" if r.rec else "rows", "bytes_per_gaussian": [fb, bb], "kernel": r.kernel_name(), "fwd_ms": f_ms, "bwd_ms": b_ms,
                 "value": r.N / ((f_ms + b_ms) * 1e-3), "fwd_gbs": fb * r.N / (f_ms * 1e-3) / 1e9, "bwd_gbs": bb * r.N / (b_ms * 1e-3) / 1e9,
                 "bwd_frac": bb * r.N / (b_ms * 1e-3) / 1e9 / peak, "fwd+bwd_frac": (fb + bb) * r.N / ((f_ms + b_ms) * 1e-3) / 1e9 / peak}
 
@@ -345,6 +355,7 @@ def run_ours(args, W, cfg):
         specs = [(i, "rec") for i in (1, 2, 3, 4) if i != cfg.index]
         if rec:
             specs.append((cfg.index, "rows"))                  # the same workload through the row-array entry points
+        specs += [(i, "paper") for i in (1, 2, 4)]             # the paper's own 3 + 9K record (17 % fewer parameter bytes)
         R_keep, R = R, None
         if cfg.N > 2_000_000:
             R_keep.d = None; R_keep.params = None; R_keep.g_params = None; R_keep.colors = None
@@ -352,14 +363,14 @@ def run_ours(args, W, cfg):
         for i, layout in specs:
             r = Resident(B, W, S, W.CONFIGS[i], 0, layout, args.norm_mode)
             f_ms, b_ms, _ = r.timed(20, 5, barrier)
-            others[("cfg%d" % i) + ("" if layout == "rec" else " rows")] = dict(summary(r, f_ms, b_ms), workload=W.CONFIGS[i].name, steps=20)
+            others[("cfg%d" % i) + ("" if layout == "rec" else " " + layout)] = dict(summary(r, f_ms, b_ms), workload=W.CONFIGS[i].name, steps=20)
             del r
             torch.cuda.empty_cache()
         extra["other_configs"] = others
         R = R_keep
 
     if rank == 0:
-        fb, bb = algorithmic_bytes(cfg.kind, K, C, R.has_vis)
+        fb, bb = algorithmic_bytes(cfg.kind, K, C, R.has_vis, R.paper)
         achieved = bb * N / (bwd_ms * 1e-3) / 1e9
         clk = clocks.summary()
         line = {
@@ -367,7 +378,8 @@ def run_ours(args, W, cfg):
             "warmup": warm, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": cfg.name, "N_per_gpu": N, "K": K, "C": C,
-                       "layout": "tile records (nasg_rec_*: parameters and gradients as [N/32][6+11K][32] records)" if rec else "row arrays",
+                       "layout": "paper-native tile records (nasg_paper_*: [N/32][6+9K][32], raw values, Table 8 activations in the kernel)" if R.paper else
+                                 "tile records (nasg_rec_*: parameters and gradients as [N/32][6+11K][32] records)" if rec else "row arrays",
                        "norm_mode": {1: "exact (eq.10)", 0: "approximate (NASG normaliser, PAPER.md:223)", 2: "pure NASG, no carrier (PAPER.md:423)"}[args.norm_mode],
                        "l2": ("inputs + outputs (%.2f GB/step) larger than the 126 MB L2; no flush" if (fb + bb) * N > 2.5e8 else
                               "inputs + outputs (%.4f GB/step) FIT in the 126 MB L2 and are NOT flushed: L2-warm number") % ((fb + bb) * N / 1e9),
@@ -377,19 +389,19 @@ def run_ours(args, W, cfg):
                                 "fwd+bwd": (fb + bb) * N / ((fwd_ms + bwd_ms) * 1e-3) / 1e9,
                                 "bytes_per_gaussian": {"fwd": fb, "bwd": bb}},
             "roofline": {"bound": "hbm", "kernel": R.kernel_name(), "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": recorded(cfg.name, "dram_bytes_bwd_" + ("records" if rec else "rows")),
+                         "frac": achieved / peak, "traffic": recorded(cfg.name, "dram_bytes_bwd_" + ("paper" if R.paper else "records" if rec else "rows")),
                          "traffic_source": "recorded ncu --set full capture, not this run: profiles/traffic.json names capture and commit",
                          "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0},
             "clocks": dict(clk, window="timed region (%.0f ms) + identical untimed load up to 1 s" % (timed_wall * 1e3)),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms,
                     "gbs_each_way": [h2d / (e2e_ms * 1e-3) / 1e9, d2h / (e2e_ms * 1e-3) / 1e9],
-                    "api": "nasg_rec_eval_fwd_bwd_host" if rec else "sh_eval_fwd_bwd_host" if cfg.kind == "sh" else "nasg_eval_fwd_bwd_host"},
+                    "api": "nasg_paper_eval_fwd_bwd_host" if R.paper else "nasg_rec_eval_fwd_bwd_host" if rec else "sh_eval_fwd_bwd_host" if cfg.kind == "sh" else "nasg_eval_fwd_bwd_host"},
             "gpu_launches": int(launches),
         }
         line.update(extra)
         # issue-slot utilisation of the dominant kernel AS WRITTEN (a diagnostic, not a roofline): its executed
         # warp-instructions (committed ncu count) against the issue slots of the run at the SAMPLED SM clock
-        inst = recorded(cfg.name, "warp_instructions_per_32_gaussians_bwd_" + ("records" if rec else "rows"))
+        inst = recorded(cfg.name, "warp_instructions_per_32_gaussians_bwd_" + ("paper" if R.paper else "records" if rec else "rows"))
         if inst is not None and clk.get("sm_mhz"):
             props = torch.cuda.get_device_properties(local)
             slots = props.multi_processor_count * 4 * clk["sm_mhz"] * 1e6 * bwd_ms * 1e-3
@@ -414,7 +426,7 @@ def main():
                     help="1 = exact normaliser eq.(10) (default, the metric's configuration); 0 = the NASG normaliser the paper trained with; 2 = pure NASG lobe (no carrier)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
     ap.add_argument("--no-others", action="store_true", help="skip the sustained run and the other configs (short profiling runs)")
-    ap.add_argument("--layout", default="rec", choices=["rec", "rows"],
+    ap.add_argument("--layout", default="rec", choices=["rec", "rows", "paper"],
                     help="rec = tile-record parameter layout (nasg_rec_*, the fast path; NASGabor with even K, C <= 4); "
                          "rows = the row-array entry points (nasg_eval_fwd/bwd)")
     args = ap.parse_args()

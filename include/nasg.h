@@ -174,6 +174,10 @@ int nasg_paper_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float 
 size_t nasg_rec_host_scratch_bytes(int64_t N, int32_t K, int32_t C);
 int nasg_rec_eval_fwd_bwd_host(const nasg_rec_inputs *in, const float *g_colors, float *colors, float *g_params,
                                int norm_mode, void *dev_scratch, size_t dev_scratch_bytes, void *cuda_stream);
+/* the same for paper-native records (nasg_paper_floats(N, K) floats) */
+size_t nasg_paper_host_scratch_bytes(int64_t N, int32_t K, int32_t C);
+int nasg_paper_eval_fwd_bwd_host(const nasg_rec_inputs *in, const float *g_colors, float *colors, float *g_params,
+                                 int norm_mode, void *dev_scratch, size_t dev_scratch_bytes, void *cuda_stream);
 
 /* Bytes of device scratch nasg_eval_bwd / sh_eval_bwd need when g_campos != NULL (pass K = 0 for SH). */
 size_t nasg_workspace_bytes(int64_t N, int32_t K, int32_t C);

@@ -24,7 +24,7 @@ SYMBOLS = ("nasg_eval_fwd", "nasg_eval_bwd", "sh_eval_fwd", "sh_eval_bwd", "nasg
            "sh_eval_fwd_bwd_host", "nasg_strerror", "nasg_version", "nasg_launch_count", "nasg_debug_set_path",
            "nasg_rec_floats", "nasg_rec_pack", "nasg_rec_unpack", "nasg_rec_eval_fwd", "nasg_rec_eval_bwd",
            "nasg_rec_host_scratch_bytes", "nasg_rec_eval_fwd_bwd_host", "nasg_paper_floats", "nasg_paper_eval_fwd",
-           "nasg_paper_eval_bwd")
+           "nasg_paper_eval_bwd", "nasg_paper_host_scratch_bytes", "nasg_paper_eval_fwd_bwd_host")
 
 
 class NasgError(RuntimeError):
@@ -96,9 +96,12 @@ def _load():
     lib.nasg_rec_host_scratch_bytes.argtypes = [i64, i32, i32]
     lib.nasg_rec_host_scratch_bytes.restype = sz
     lib.nasg_rec_eval_fwd_bwd_host.argtypes = [C.POINTER(_RecInputs), vp, vp, vp, C.c_int, vp, sz, vp]
+    lib.nasg_paper_host_scratch_bytes.argtypes = [i64, i32, i32]
+    lib.nasg_paper_host_scratch_bytes.restype = sz
+    lib.nasg_paper_eval_fwd_bwd_host.argtypes = [C.POINTER(_RecInputs), vp, vp, vp, C.c_int, vp, sz, vp]
     for name in ("nasg_eval_fwd", "nasg_eval_bwd", "sh_eval_fwd", "sh_eval_bwd", "nasg_eval_fwd_bwd_host",
                  "sh_eval_fwd_bwd_host", "nasg_rec_pack", "nasg_rec_unpack", "nasg_rec_eval_fwd", "nasg_rec_eval_bwd",
-                 "nasg_rec_eval_fwd_bwd_host", "nasg_paper_eval_fwd", "nasg_paper_eval_bwd"):
+                 "nasg_rec_eval_fwd_bwd_host", "nasg_paper_eval_fwd", "nasg_paper_eval_bwd", "nasg_paper_eval_fwd_bwd_host"):
         getattr(lib, name).restype = C.c_int
     return lib
 
@@ -361,22 +364,27 @@ def nasg_rec_host_scratch_bytes(N: int, K: int, Cn: int) -> int:
     return int(_lib.nasg_rec_host_scratch_bytes(N, K, Cn))
 
 
+def nasg_paper_host_scratch_bytes(N: int, K: int, Cn: int) -> int:
+    return int(_lib.nasg_paper_host_scratch_bytes(N, K, Cn))
+
+
 def nasg_rec_eval_fwd_bwd_host(host: dict, host_out: dict, N: int, K: int, dev_scratch: torch.Tensor,
-                               norm_mode: int = NORM_EXACT, stream=None) -> None:
+                               norm_mode: int = NORM_EXACT, stream=None, paper: bool = False) -> None:
     """End-to-end call with HOST tensors on the tile-record layout: ``host`` holds params (records), campos, vis (or
-    None), g_colors; ``host_out`` holds colors and g_params (records)."""
+    None), g_colors; ``host_out`` holds colors and g_params (records). paper=True: paper-native records
+    (nasg_paper_eval_fwd_bwd_host)."""
     f32 = torch.float32
     Cn = int(host["campos"].shape[0])
-    nf = nasg_rec_floats(N, K)
+    nf = nasg_paper_floats(N, K) if paper else nasg_rec_floats(N, K)
     _chk(host["params"], "params", (nf,), f32, "cpu"); _chk(host["campos"], "campos", (Cn, 3), f32, "cpu")
     _chk(host.get("vis"), "vis", (Cn, N), torch.uint8, "cpu"); _chk(host["g_colors"], "g_colors", (Cn, N, 3), f32, "cpu")
     _chk(host_out["colors"], "colors", (Cn, N, 3), f32, "cpu"); _chk(host_out["g_params"], "g_params", (nf,), f32, "cpu")
     inp = _RecInputs(N, K, Cn, _ptr(host["params"]), _ptr(host["campos"]), _ptr(host.get("vis")))
-    rc = _lib.nasg_rec_eval_fwd_bwd_host(C.byref(inp), _ptr(host["g_colors"]), _ptr(host_out["colors"]), _ptr(host_out["g_params"]),
-                                         int(norm_mode), _ptr(dev_scratch), dev_scratch.numel() * dev_scratch.element_size(),
-                                         _stream(stream))
+    fn = _lib.nasg_paper_eval_fwd_bwd_host if paper else _lib.nasg_rec_eval_fwd_bwd_host
+    rc = fn(C.byref(inp), _ptr(host["g_colors"]), _ptr(host_out["colors"]), _ptr(host_out["g_params"]), int(norm_mode), _ptr(dev_scratch),
+            dev_scratch.numel() * dev_scratch.element_size(), _stream(stream))
     if rc != 0:
-        raise NasgError(rc, "nasg_rec_eval_fwd_bwd_host")
+        raise NasgError(rc, "nasg_paper_eval_fwd_bwd_host" if paper else "nasg_rec_eval_fwd_bwd_host")
 
 
 # ---- the paper's own parameter record (include/nasg.h: nasg_paper_*) ---------------------------------

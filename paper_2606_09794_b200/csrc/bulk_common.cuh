@@ -47,6 +47,9 @@ __device__ __forceinline__ bool elect_one()
         "}" : "=r"(pred));
     return pred != 0;
 }
+// orders this thread's earlier generic-proxy accesses to shared memory (the lanes' reads of a slot, made visible to it by
+// __syncwarp) before its later async-proxy operations (the bulk copy that refills the slot)
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 // 1-D bulk copy global -> shared of `bytes` (multiple of 16; both addresses 16-byte aligned), completing on `bar`
 __device__ __forceinline__ void bulk_g2s(unsigned dst, const void *src, unsigned bytes, unsigned bar)
 {
@@ -73,7 +76,7 @@ __device__ __forceinline__ void lds64x2(unsigned addr, T8 &a, T8 &b)
 {
     static_assert(sizeof(T8) == 8, "8-byte type");
     unsigned long long ua, ub;
-    asm volatile("ld.shared.v2.b64 {%0,%1}, [%2];" : "=l"(ua), "=l"(ub) : "r"(addr));
+    asm volatile("ld.shared.v2.b64 {%0,%1}, [%2];" : "=l"(ua), "=l"(ub) : "r"(addr) : "memory");   // (reads memory: must not be hoisted over the stores)
     memcpy(&a, &ua, 8); memcpy(&b, &ub, 8);
 }
 template <typename T8>

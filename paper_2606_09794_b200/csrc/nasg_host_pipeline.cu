@@ -333,31 +333,27 @@ int sh_eval_fwd_bwd_host(int64_t N, int32_t C, const float *means, const float *
 // ---- NASGabor, tile-record layout: a chunk of Gaussians is a contiguous range of records ---------------
 namespace {
 struct RecDev { float *params, *gparams, *gcol, *col; uint8_t *vis; };
-size_t rec_footprint(size_t n, int K, size_t c)
+size_t rec_footprint(size_t n, int K, size_t c, int pk)
 {
-    return 2 * align_up((size_t)nasg::rec_total_floats((int64_t)n, K) * 4) + align_up(c * n) + 2 * align_up(c * n * 12);
+    return 2 * align_up((size_t)nasg::rec_total_floats((int64_t)n, K, pk) * 4) + align_up(c * n) + 2 * align_up(c * n * 12);
 }
-bool carve_rec(Carver &cv, RecDev &d, size_t n, int K, size_t c)
+bool carve_rec(Carver &cv, RecDev &d, size_t n, int K, size_t c, int pk)
 {
-    const size_t rf = (size_t)nasg::rec_total_floats((int64_t)n, K);
+    const size_t rf = (size_t)nasg::rec_total_floats((int64_t)n, K, pk);
     d.params = cv.take<float>(rf); d.gparams = cv.take<float>(rf); d.vis = cv.take<uint8_t>(c * n);
     d.gcol = cv.take<float>(c * n * 3); d.col = cv.take<float>(c * n * 3);
     return cv.off <= cv.cap;
 }
-} // namespace
-
-extern "C" {
-
-size_t nasg_rec_host_scratch_bytes(int64_t N, int32_t K, int32_t C)
+size_t rec_host_scratch(int64_t N, int32_t K, int32_t C, int pk)
 {
     if (N <= 0 || !(K == 2 || K == 4 || K == 8) || C < 1) return 0;
     const size_t c = (size_t)C;
-    const size_t single = rec_footprint((size_t)N, K, c), chunked = 2 * rec_footprint((size_t)chunk_size(N, false), K, c);
+    const size_t single = rec_footprint((size_t)N, K, c, pk), chunked = 2 * rec_footprint((size_t)chunk_size(N, false), K, c, pk);
     return (single > chunked ? single : chunked) + align_up(c * 12) + SCRATCH_SLOP;
 }
 
-int nasg_rec_eval_fwd_bwd_host(const nasg_rec_inputs *in, const float *g_colors, float *colors, float *g_params,
-                               int norm_mode, void *dev_scratch, size_t dev_scratch_bytes, void *cuda_stream)
+int rec_host(const nasg_rec_inputs *in, const float *g_colors, float *colors, float *g_params, int norm_mode, void *dev_scratch,
+             size_t dev_scratch_bytes, int pk, void *cuda_stream)
 {
     if (!in) return NASG_ERR_NULL;
     if (in->N < 0 || in->N > NASG_REC_MAX_N || in->C < 1 || in->C > NASG_REC_MAX_CAMERAS) return NASG_ERR_SHAPE;
@@ -365,7 +361,7 @@ int nasg_rec_eval_fwd_bwd_host(const nasg_rec_inputs *in, const float *g_colors,
     if (norm_mode != NASG_NORM_APPROX && norm_mode != NASG_NORM_EXACT && norm_mode != NASG_NORM_NASG) return NASG_ERR_NORM_MODE;
     if (in->N == 0) return NASG_OK;
     if (!in->params || !in->campos || !g_colors || !colors || !g_params || !dev_scratch) return NASG_ERR_NULL;
-    if (dev_scratch_bytes < nasg_rec_host_scratch_bytes(in->N, in->K, in->C) || !aligned16(dev_scratch)) return NASG_ERR_WORKSPACE;
+    if (dev_scratch_bytes < rec_host_scratch(in->N, in->K, in->C, pk) || !aligned16(dev_scratch)) return NASG_ERR_WORKSPACE;
     const int64_t N = in->N;
     const int K = in->K;
     const size_t c = (size_t)in->C, Nn = (size_t)N;
@@ -375,21 +371,21 @@ int nasg_rec_eval_fwd_bwd_host(const nasg_rec_inputs *in, const float *g_colors,
     Carver cv{static_cast<char *>(dev_scratch), 0, dev_scratch_bytes};
     float *d_campos = cv.take<float>(c * 3);
     RecDev dev[2];
-    if (!carve_rec(cv, dev[0], (size_t)chunk, K, c)) return NASG_ERR_WORKSPACE;
-    if (two && !carve_rec(cv, dev[1], (size_t)chunk, K, c)) return NASG_ERR_WORKSPACE;
+    if (!carve_rec(cv, dev[0], (size_t)chunk, K, c, pk)) return NASG_ERR_WORKSPACE;
+    if (two && !carve_rec(cv, dev[1], (size_t)chunk, K, c, pk)) return NASG_ERR_WORKSPACE;
     if (!d_campos) return NASG_ERR_WORKSPACE;
 
     const cudaMemcpyKind H2D = cudaMemcpyHostToDevice, D2H = cudaMemcpyDeviceToHost;
     cudaStream_t user = (cudaStream_t)cuda_stream;
     NASG_TRY_CUDA(cudaMemcpyAsync(d_campos, in->campos, c * 12, H2D, user));     // replicated; before the pipeline's start event
     const nasg_rec_inputs host = *in;
-    const size_t rec_f = (size_t)nasg::rec_total_floats(32, K);                  // floats per record
+    const size_t rec_f = (size_t)nasg::rec_total_floats(32, K, pk);              // floats per record
 
     auto copy_in = [&](int b, int64_t n0, int64_t nc, cudaStream_t st) -> int {
         const RecDev &d = dev[b];
         const size_t o = (size_t)n0, w = (size_t)nc;
         // the chunk's records are one contiguous block: a single copy
-        NASG_TRY_CUDA(cudaMemcpyAsync(d.params, host.params + (o / 32) * rec_f, (size_t)nasg::rec_total_floats(nc, K) * 4, H2D, st));
+        NASG_TRY_CUDA(cudaMemcpyAsync(d.params, host.params + (o / 32) * rec_f, (size_t)nasg::rec_total_floats(nc, K, pk) * 4, H2D, st));
         if (host.vis) NASG_TRY_CUDA(copy_rows(d.vis, w, host.vis, Nn, 0, o, w, c, 1, H2D, st));
         NASG_TRY_CUDA(copy_rows(d.gcol, w, g_colors, Nn, 0, o, w, c, 12, H2D, st));
         return NASG_OK;
@@ -398,6 +394,10 @@ int nasg_rec_eval_fwd_bwd_host(const nasg_rec_inputs *in, const float *g_colors,
         const RecDev &d = dev[b];
         nasg_rec_inputs din = host;
         din.N = nc; din.params = d.params; din.campos = d_campos; din.vis = host.vis ? d.vis : nullptr;
+        if (pk) {
+            NASG_TRY(nasg_paper_eval_fwd(&din, d.col, norm_mode, st));
+            return nasg_paper_eval_bwd(&din, d.gcol, d.gparams, norm_mode, st);
+        }
         NASG_TRY(nasg_rec_eval_fwd(&din, d.col, norm_mode, st));
         return nasg_rec_eval_bwd(&din, d.gcol, d.gparams, norm_mode, st);
     };
@@ -405,10 +405,27 @@ int nasg_rec_eval_fwd_bwd_host(const nasg_rec_inputs *in, const float *g_colors,
         const RecDev &d = dev[b];
         const size_t o = (size_t)n0, w = (size_t)nc;
         NASG_TRY_CUDA(copy_rows(colors, Nn, d.col, w, o, 0, w, c, 12, D2H, st));
-        NASG_TRY_CUDA(cudaMemcpyAsync(g_params + (o / 32) * rec_f, d.gparams, (size_t)nasg::rec_total_floats(nc, K) * 4, D2H, st));
+        NASG_TRY_CUDA(cudaMemcpyAsync(g_params + (o / 32) * rec_f, d.gparams, (size_t)nasg::rec_total_floats(nc, K, pk) * 4, D2H, st));
         return NASG_OK;
     };
     return run_pipeline(N, chunk, user, copy_in, compute, copy_out);
+}
+
+} // namespace
+
+extern "C" {
+
+size_t nasg_rec_host_scratch_bytes(int64_t N, int32_t K, int32_t C) { return rec_host_scratch(N, K, C, 0); }
+int nasg_rec_eval_fwd_bwd_host(const nasg_rec_inputs *in, const float *g_colors, float *colors, float *g_params,
+                               int norm_mode, void *dev_scratch, size_t dev_scratch_bytes, void *cuda_stream)
+{
+    return rec_host(in, g_colors, colors, g_params, norm_mode, dev_scratch, dev_scratch_bytes, 0, cuda_stream);
+}
+size_t nasg_paper_host_scratch_bytes(int64_t N, int32_t K, int32_t C) { return rec_host_scratch(N, K, C, 1); }
+int nasg_paper_eval_fwd_bwd_host(const nasg_rec_inputs *in, const float *g_colors, float *colors, float *g_params,
+                                 int norm_mode, void *dev_scratch, size_t dev_scratch_bytes, void *cuda_stream)
+{
+    return rec_host(in, g_colors, colors, g_params, norm_mode, dev_scratch, dev_scratch_bytes, 1, cuda_stream);
 }
 
 } // extern "C"
