@@ -15,7 +15,7 @@ from typing import Optional
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SRC = [os.path.join(_HERE, "nasg_ref.c"), os.path.join(_HERE, "sh_ref.c")]
+_SRC = [os.path.join(_HERE, "nasg_ref.c"), os.path.join(_HERE, "sh_ref.c"), os.path.join(_HERE, "iso_ref.c")]
 _LIB = os.path.join(_HERE, "liboracle_ref.so")
 _lib = None
 
@@ -48,6 +48,11 @@ def lib():
         L.nasg_ref_dlnI.argtypes = [dbl, dbl, dbl, i32, dp]
         L.nasg_ref_partials.argtypes = [dbl, dbl, dbl, dbl, dbl, dbl, i32, dp]
         L.nasg_ref_frame.argtypes = [dp, dp, dp]
+        L.iso_ref_lobe.argtypes = [i32, dbl, dbl, dp]
+        L.iso_ref_fwd.argtypes = [i64, i32, i32, i32, dp, dp, dp, dp, dp, dp, u8p, dp]
+        L.iso_ref_bwd.argtypes = [i64, i32, i32, i32, dp, dp, dp, dp, dp, dp, u8p, dp, dp, dp, dp, dp, dp]
+        L.iso_ref_fwd.restype = i32
+        L.iso_ref_bwd.restype = i32
         L.nasg_ref_paper_frame.argtypes = [dp, dp, dp, dp, dp]
         L.nasg_ref_paper_fwd.argtypes = [i64, i32, i32, dp, dp, dp, dp, dp, dp, u8p, i32, dp]
         L.nasg_ref_paper_bwd.argtypes = [i64, i32, i32, dp, dp, dp, dp, dp, dp, u8p, dp, i32, dp, dp, dp, dp, dp]
@@ -198,5 +203,36 @@ def paper_bwd(inp: dict, norm_mode: int = 1, g_colors: Optional[np.ndarray] = No
                g_ampraw=np.empty((K, 3, N)), g_dc=np.empty((3, N)))
     rc = lib().nasg_ref_paper_bwd(N, K, Cn, _p(means), _p(eu), _p(sp), _p(aw), _p(dc), _p(campos), _p(vis), _p(gcol), norm_mode,
                                   _p(out["g_means"]), _p(out["g_euler"]), _p(out["g_shp"]), _p(out["g_ampraw"]), _p(out["g_dc"]))
+    assert rc == 0
+    return out
+
+
+# ---- isotropic Table-6 functions (oracle/iso_ref.c): kind 0 = Spherical Gaussian, 1 = Spherical Beta, 2 = Spherical Cauchy
+def iso_lobe(kind: int, v: float, raw: float) -> np.ndarray:
+    """[F, dF/dv, dF/draw] of one normalised lobe F = c G at v = z.d."""
+    out = np.empty(3)
+    lib().iso_ref_lobe(int(kind), float(v), float(raw), _p(out))
+    return out
+
+
+def iso_fwd(inp: dict, kind: int) -> np.ndarray:
+    """colors [C,N,3] fp64; inp holds means, axis [K,N,3], shp [K,N], amp [K,3,N], dc, campos, vis."""
+    N, K, Cn = int(inp["N"]), int(inp["K"]), int(inp["C"])
+    means, ax, sp, am, dc, campos = (_d(inp[k]) for k in ("means", "axis", "shp", "amp", "dc", "campos"))
+    vis = None if inp.get("vis") is None else np.ascontiguousarray(inp["vis"], dtype=np.uint8)
+    colors = np.empty((Cn, N, 3), dtype=np.float64)
+    rc = lib().iso_ref_fwd(N, K, Cn, int(kind), _p(means), _p(ax), _p(sp), _p(am), _p(dc), _p(campos), _p(vis), _p(colors))
+    assert rc == 0
+    return colors
+
+
+def iso_bwd(inp: dict, kind: int, g_colors: Optional[np.ndarray] = None) -> dict:
+    N, K, Cn = int(inp["N"]), int(inp["K"]), int(inp["C"])
+    means, ax, sp, am, dc, campos = (_d(inp[k]) for k in ("means", "axis", "shp", "amp", "dc", "campos"))
+    gcol = _d(inp["g_colors"] if g_colors is None else g_colors)
+    vis = None if inp.get("vis") is None else np.ascontiguousarray(inp["vis"], dtype=np.uint8)
+    out = dict(g_means=np.empty((N, 3)), g_axis=np.empty((K, N, 3)), g_shp=np.empty((K, N)), g_amp=np.empty((K, 3, N)), g_dc=np.empty((3, N)))
+    rc = lib().iso_ref_bwd(N, K, Cn, int(kind), _p(means), _p(ax), _p(sp), _p(am), _p(dc), _p(campos), _p(vis), _p(gcol),
+                           _p(out["g_means"]), _p(out["g_axis"]), _p(out["g_shp"]), _p(out["g_amp"]), _p(out["g_dc"]))
     assert rc == 0
     return out

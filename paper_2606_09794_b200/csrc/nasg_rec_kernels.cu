@@ -105,7 +105,6 @@ template <int PAIR_BYTES>
 __device__ __forceinline__ void stage_issue(const StageCursor &s, int T, unsigned dst, unsigned bar)
 {
     if (s.tile < T) {
-        fence_proxy_async();
         mbar_expect_tx(bar, PAIR_BYTES);
         bulk_g2s(dst, s.src, PAIR_BYTES, bar);
     }
@@ -119,7 +118,6 @@ __device__ __forceinline__ void hdr_issue(const HdrCursor &h, const Warp &w, uns
         const unsigned cnt = h.tile == w.T - 1 ? w.last_cnt : (unsigned)WT;
         unsigned bytes = HDR_BYTES;
         if (bulk_rows) bytes += (BWD ? CT * 12u * cnt : 0u) + (h.vis ? CT * cnt : 0u);
-        fence_proxy_async();
         mbar_expect_tx(bar, bytes);
         bulk_g2s(dst, h.src, HDR_BYTES, bar);
         if (bulk_rows) {

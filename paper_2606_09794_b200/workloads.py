@@ -120,6 +120,22 @@ def make_paper(cfg: Config, N: Optional[int] = None) -> dict:
     return out
 
 
+def make_iso(cfg: Config, N: Optional[int] = None) -> dict:
+    """The same config for the isotropic Table-6 functions (include/nasg.h: nasg_iso_*): axis [K,N,3] ~ N(0,1)^3 scaled by
+    U[0.5,2] (unnormalised on purpose), shp [K,N] raw ~ U[0, 4.5] (lambda, beta = e^raw in [1, 90]; rho = sigmoid in
+    [0.5, 0.989]), amp ~ N(0,0.3), dc ~ N(0,0.3); geometry, masks and g_colors as make_nasg."""
+    assert cfg.kind == "nasg"
+    out = make_geometry(cfg, N)
+    N, K = out["N"], cfg.K
+    r = _rng(cfg.seed, TAG_QUAT)
+    axis = r.standard_normal(size=(K, N, 3)) * r.uniform(0.5, 2.0, size=(K, N, 1))
+    shp = _rng(cfg.seed, TAG_BW).uniform(0.0, 4.5, size=(K, N))
+    amp = _rng(cfg.seed, TAG_AMP).normal(0.0, 0.3, size=(K, 3, N))
+    dc = _rng(cfg.seed, TAG_DC).normal(0.0, 0.3, size=(3, N))
+    out.update(K=K, axis=axis.astype(np.float32), shp=shp.astype(np.float32), amp=amp.astype(np.float32), dc=dc.astype(np.float32))
+    return out
+
+
 def make_sh(cfg: Config, N: Optional[int] = None) -> dict:
     """Inputs of sh_eval_fwd/bwd (config 3): geometry of config 2 plus degree-3 coefficients."""
     assert cfg.kind == "sh"
@@ -222,3 +238,25 @@ def unpack_paper_records(rec: np.ndarray, N: int, K: int) -> dict:
     means, dc, comp = _unpack(rec, N, K, 9)
     return dict(means=means, dc=dc, euler=np.ascontiguousarray(comp[..., 0:3]), shp=np.ascontiguousarray(comp[..., 3:6]),
                 ampraw=np.ascontiguousarray(comp[..., 6:9].transpose(0, 2, 1)))
+
+
+def iso_rec_floats(N: int, K: int) -> int:
+    return ((N + REC_TILE - 1) // REC_TILE) * REC_TILE * (6 + 7 * K)
+
+
+def pack_iso_records(means, axis, shp, amp, dc) -> np.ndarray:
+    """Isotropic Table-6 lobes as tile records float32 [T, 6 + 7 K, 32]: per lobe (axis x, y, z, shape raw, w_r, w_g, w_b).
+    Padding lanes get the axis (0, 0, 1) so that nothing divides by zero in lanes that are never stored."""
+    N = axis.shape[1]
+    rec = _pack(means, dc, np.concatenate([axis, shp[..., None], amp.transpose(0, 2, 1)], axis=2))
+    if N % REC_TILE:
+        K = axis.shape[0]
+        r = rec.reshape(-1, 6 + 7 * K, REC_TILE)
+        r[-1, 6:].reshape(K // 2, 7, REC_TILE, 2)[:, 2, N % REC_TILE:, :] = 1.0
+    return rec
+
+
+def unpack_iso_records(rec: np.ndarray, N: int, K: int) -> dict:
+    means, dc, comp = _unpack(rec, N, K, 7)
+    return dict(means=means, dc=dc, axis=np.ascontiguousarray(comp[..., 0:3]), shp=np.ascontiguousarray(comp[..., 3]),
+                amp=np.ascontiguousarray(comp[..., 4:7].transpose(0, 2, 1)))
