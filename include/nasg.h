@@ -167,6 +167,23 @@ int nasg_paper_eval_fwd(const nasg_rec_inputs *in, float *colors, int norm_mode,
 int nasg_paper_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float *g_params, int norm_mode,
                         void *cuda_stream);
 
+/* ---- other spherical functions of the paper's Table 6 in the same skeleton ---------
+ * colour = c0 + sum_l w_l c_l G_l(d . zhat_l) (eq.(6)) with an ISOTROPIC, normalised lobe:
+ *     NASG_ISO_SG      0   Spherical Gaussian  G = exp{lambda (z.d - 1)},  c = lambda/(2 pi (1 - e^{-2 lambda})),  lambda = e^raw
+ *     NASG_ISO_BETA    1   Spherical Beta      G = max(z.d, 0)^beta,       c = (beta + 1)/(2 pi),                  beta = e^raw
+ *     NASG_ISO_CAUCHY  2   Spherical Cauchy    G = ((1 - rho^2)/(1 + rho^2 - 2 rho z.d))^2,  c = 1/(4 pi),          rho = 1/(1 + e^-raw)
+ * (Table 6 prints the Cauchy denominator as 1 - rho^2 - 2 rho z.d; only 1 + rho^2 - 2 rho z.d integrates to 1/c: DESIGN.md R19.)
+ * zhat = z/|z| of a free 3-vector per lobe (gradient through the normalisation). Tile records with 7 components per lobe:
+ *     [192 + 448 j + 64 c + 2 lane + h],  c = 0..2 axis (x,y,z) | 3 shape (raw) | 4..6 amplitude (r,g,b);  [T][6 + 7 K][32]
+ * nasg_iso_floats(N, K) floats; the gradient record has the same layout (dL/d axis, dL/d raw, dL/d w). Same restrictions
+ * and conventions as nasg_rec_eval_* (`kind` takes the place of norm_mode; a bad kind returns NASG_ERR_NORM_MODE). */
+#define NASG_ISO_SG     0
+#define NASG_ISO_BETA   1
+#define NASG_ISO_CAUCHY 2
+size_t nasg_iso_floats(int64_t N, int32_t K);
+int nasg_iso_eval_fwd(const nasg_rec_inputs *in, float *colors, int kind, void *cuda_stream);
+int nasg_iso_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float *g_params, int kind, void *cuda_stream);
+
 /* End-to-end with HOST buffers, as nasg_eval_fwd_bwd_host below: params / g_params are HOST record arrays, campos, vis,
  * g_colors, colors HOST arrays. A chunk of Gaussians is a contiguous block of records, so each chunk moves with one
  * copy per direction for the parameters / gradients plus one strided copy each for vis, g_colors and colors. Padding

@@ -254,6 +254,21 @@ int nasg_paper_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float 
     return rec_eval_bwd(in, g_colors, g_params, norm_mode, 1, cuda_stream);
 }
 
+// ---- isotropic Table-6 functions (Spherical Gaussian / Beta / Cauchy): 7 floats per lobe
+size_t nasg_iso_floats(int64_t N, int32_t K)
+{
+    if (N <= 0 || !rec_K_ok(K)) return 0;
+    return (size_t)nasg::rec_total_floats(N, K, 2);
+}
+int nasg_iso_eval_fwd(const nasg_rec_inputs *in, float *colors, int kind, void *cuda_stream)
+{
+    return rec_eval_fwd(in, colors, kind, 2, cuda_stream);
+}
+int nasg_iso_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float *g_params, int kind, void *cuda_stream)
+{
+    return rec_eval_bwd(in, g_colors, g_params, kind, 2, cuda_stream);
+}
+
 size_t nasg_workspace_bytes(int64_t N, int32_t K, int32_t C)
 {
     (void)K;
@@ -271,7 +286,7 @@ const char *nasg_strerror(int code)
     case NASG_ERR_ALIGN: return "quat/shape (or their gradients) must be 16-byte aligned";
     case NASG_ERR_WORKSPACE: return "workspace/scratch missing, misaligned or too small";
     case NASG_ERR_CUDA: return cudaGetErrorString(t_last_cuda);
-    case NASG_ERR_NORM_MODE: return "norm_mode must be 0 (approximate), 1 (exact, eq.10) or 2 (pure NASG, no carrier)";
+    case NASG_ERR_NORM_MODE: return "norm_mode must be 0 (approximate), 1 (exact, eq.10) or 2 (pure NASG, no carrier); nasg_iso_*: kind must be 0, 1 or 2";
     default: return "unknown error code";
     }
 }

@@ -284,6 +284,98 @@ NASG_HD void lobe_pair_setup_paper(f2 th, f2 ph, f2 ta, f2 lr, f2 ar, f2 kr, Lob
     normaliser2<MODE == 1, GRAD>(fma2(lr, splat(LOG2E), scl2(lg2_2(one_pa), 0.5f)), mul2(lam, one_pa), lam, k, L.lgI, G);
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// Isotropic spherical functions of the paper's Table 6 (include/nasg.h: nasg_iso_*), normalised:
+//   KIND 0 Spherical Gaussian  F = lambda/(2 pi (1-e^{-2 lambda})) exp{lambda (v-1)}        lambda = e^raw
+//   KIND 1 Spherical Beta      F = (beta+1)/(2 pi) max(v,0)^beta                             beta = e^raw
+//   KIND 2 Spherical Cauchy    F = 1/(4 pi) ((1-rho^2)/(1+rho^2-2 rho v))^2                  rho = 1/(1+e^-raw)   (R19)
+// v = d.zhat, zhat = z/|z|. Lobe pairs on f32x2 like the NASGabor arithmetic. 1 - v is formed without cancellation as
+// h = |d - zhat|^2 / 2 (both unit vectors): every function is sharpest at v = 1, where 1 - d.zhat would lose all digits.
+// ---------------------------------------------------------------------------------------------
+struct IsoPair {
+    f2 zx, zy, zz, inv;     // unit axis and 1/|z|
+    f2 p;                   // lambda | beta | rho
+    f2 q0, q1, q2;          // per-kind constants (see iso_pair_setup)
+    f2 lgc;                 // log2 of the normalisation constant (SG, SB)
+};
+template <int KIND>
+NASG_HD void iso_pair_setup(f2 x, f2 y, f2 z, f2 raw, IsoPair &P)
+{
+    const f2 nn = fma2(x, x, fma2(y, y, mul2(z, z)));
+    f2 inv = rsqrt2(nn);
+    inv = mul2(inv, fma2(scl2(nn, -0.5f), mul2(inv, inv), splat(1.5f)));   // one Newton step
+    P.zx = mul2(x, inv); P.zy = mul2(y, inv); P.zz = mul2(z, inv); P.inv = inv;
+    const f2 one = splat(1.0f);
+    if (KIND == 0) {
+        const f2 lam = ex2_2(scl2(raw, LOG2E));
+        const f2 x2 = add2(lam, lam);
+        const f2 em = ex2_2(scl2(x2, -LOG2E));                              // e^{-2 lambda}
+        f2 ps = fma2(x2, splat(-1.0f / 720.0f), splat(1.0f / 120.0f));
+        ps = fma2(x2, ps, splat(-1.0f / 24.0f)); ps = fma2(x2, ps, splat(1.0f / 6.0f));
+        ps = fma2(x2, ps, splat(-0.5f)); ps = fma2(x2, ps, one);
+        const f2 one_m = sel2(lo(lam) > 0.125f, hi(lam) > 0.125f, sub2(one, em), mul2(x2, ps));   // 1 - e^{-2 lambda}
+        const f2 i1m = rcp2(one_m);
+        P.p = lam;
+        P.q0 = scl2(lam, LOG2E);                                            // lambda log2(e)
+        P.q1 = fma2(neg2(mul2(x2, em)), i1m, one);                          // 1 - 2 lambda e^{-2 lambda}/(1-e^{-2 lambda}) = lambda d ln c/d lambda
+        P.q2 = splat(0.f);
+        P.lgc = lg2_2(mul2(scl2(lam, INV_TWO_PI), i1m));
+    } else if (KIND == 1) {
+        const f2 beta = ex2_2(scl2(raw, LOG2E));
+        const f2 bp1 = add2(beta, one);
+        P.p = beta;
+        P.q0 = mul2(beta, rcp2(bp1));                                       // beta/(beta+1)
+        P.q1 = scl2(beta, LN2);
+        P.q2 = splat(0.f);
+        P.lgc = lg2_2(scl2(bp1, INV_TWO_PI));
+    } else {
+        const f2 t = ex2_2(scl2(raw, -LOG2E));                              // e^{-raw}
+        const f2 rho = rcp2(add2(t, one));
+        const f2 omr = mul2(t, rho);                                        // 1 - rho without cancellation
+        const f2 opr = add2(rho, one);
+        P.p = rho;
+        P.q0 = omr;
+        P.q1 = mul2(omr, opr);                                              // 1 - rho^2
+        P.q2 = mul2(scl2(mul2(rho, rho), -4.0f), rcp2(opr));                // -4 rho^2/(1+rho) = rho (1-rho) d ln(1-rho^2)^2/d rho
+        P.lgc = splat(0.f);
+    }
+}
+// F at direction d; with GRAD also Fv = dF/dv and Fr = dF/draw.
+template <int KIND, bool GRAD>
+NASG_HD f2 iso_pair_eval(const IsoPair &P, float dx, float dy, float dz, f2 &Fv, f2 &Fr)
+{
+    const f2 ex = sub2(splat(dx), P.zx), ey = sub2(splat(dy), P.zy), ez = sub2(splat(dz), P.zz);
+    const f2 h = scl2(fma2(ex, ex, fma2(ey, ey, mul2(ez, ez))), 0.5f);      // 1 - v
+    if (KIND == 0) {
+        const f2 F = ex2_2(fma2(neg2(P.q0), h, P.lgc));
+        if (GRAD) { Fv = mul2(P.p, F); Fr = mul2(F, fma2(neg2(P.p), h, P.q1)); }
+        return F;
+    } else if (KIND == 1) {
+        const f2 v = sub2(splat(1.0f), h);
+        const bool on0 = lo(v) > 0.0f, on1 = hi(v) > 0.0f;
+        const f2 vc = max2(v, TINY);
+        f2 pl = fma2(h, splat(-0.39963189f), splat(-0.47933504f));          // log2(1-h)/h on [0,1/16] (as in lobe_pair_eval)
+        pl = fma2(h, pl, splat(-0.72136736f)); pl = fma2(h, pl, splat(-1.4426950f));
+        const f2 L2 = sel2(lo(h) < 0.0625f, hi(h) < 0.0625f, mul2(h, pl), lg2_2(vc));
+        f2 F = ex2_2(fma2(P.p, L2, P.lgc));
+        F = pack(on0 ? lo(F) : 0.0f, on1 ? hi(F) : 0.0f);                   // far hemisphere: 0
+        if (GRAD) { Fv = mul2(mul2(P.p, F), rcp2(vc)); Fr = mul2(F, fma2(P.q1, L2, P.q0)); }
+        return F;
+    } else {
+        const f2 D = fma2(add2(P.p, P.p), h, mul2(P.q0, P.q0));             // (1-rho)^2 + 2 rho (1-v) = 1 + rho^2 - 2 rho v
+        const f2 iD = rcp2(D);
+        const f2 ratio = mul2(P.q1, iD);
+        const f2 F = scl2(mul2(ratio, ratio), 0.5f * INV_TWO_PI);
+        if (GRAD) {
+            const f2 r4 = scl2(P.p, 4.0f);
+            Fv = mul2(F, mul2(r4, iD));
+            Fr = mul2(F, fma2(neg2(mul2(mul2(r4, P.q0), sub2(h, P.q0))), iD, P.q2));   // rho (1-rho) dF/drho / F
+        }
+        return F;
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
 // evaluation of a lobe pair at ONE direction d (scalar-broadcast operands)
 // ---------------------------------------------------------------------------------------------

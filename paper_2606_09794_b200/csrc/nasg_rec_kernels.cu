@@ -53,8 +53,10 @@ constexpr int HDR_BYTES = HDR_FLOATS * 4;       // 768
 // PK = parameter kind of the record: 0 = quaternion + (log Lambda, log lambda, k, phi) + amplitude: 11 components per lobe;
 //      1 = the paper's own record (Table 8, Supplementary C): 3 frame angles + (lambda, a, k) + amplitude, all raw
 //          (pre-activation), no phase: 9 components per lobe (3 + 9 K appearance floats)
+//      2 = an isotropic function of Table 6 (MODE = 0 Spherical Gaussian, 1 Spherical Beta, 2 Spherical
+//          Cauchy): axis (3, unnormalised) + raw shape value + amplitude: 7 components per lobe
 template <int PK> struct Rec {
-    static constexpr int NCOMP = PK ? 9 : 11;
+    static constexpr int NCOMP = PK == 2 ? 7 : PK == 1 ? 9 : 11;
     static constexpr int PAIR_FLOATS = NCOMP * 2 * WT;
     static constexpr int PAIR_BYTES = PAIR_FLOATS * 4;        // 2816 | 2304
     __host__ __device__ static constexpr int rec_floats(int K) { return HDR_FLOATS + (K / 2) * PAIR_FLOATS; }
@@ -80,7 +82,7 @@ template <int CT, bool BWD, int PK> struct Layout {
     static constexpr int H_GC = HDR_BYTES;
     static constexpr int H_VIS = H_GC + (BWD ? CT * WT * 12 : 0);
     static constexpr int H_BYTES = H_VIS + ((CT * WT + 127) / 128) * 128;
-    static constexpr int SCRATCH = BWD ? (2 * CT + (PK ? 3 : 2)) * WT * 16 : 0;       // cam, gcm, parked frame terms (qs | trig)
+    static constexpr int SCRATCH = BWD ? (2 * CT + (PK == 1 ? 3 : PK == 2 ? 0 : 2)) * WT * 16 : 0;   // cam, gcm, parked frame terms (qs | trig | none)
     __host__ __device__ static constexpr int region(int stages, int hslots) { return stages * PAIR_BYTES + hslots * H_BYTES + SCRATCH + 64; }
 };
 
@@ -180,14 +182,14 @@ __device__ __forceinline__ void load_pair(unsigned stage, int lane, PairRegs<PK>
 template <int PK, int MODE, bool GRAD>
 __device__ __forceinline__ void setup_pair(const PairRegs<PK> &r, LobePair &Lp, LobePairGrad &Gd, f2 (&park)[6], f2 &w0, f2 &w1, f2 &w2)
 {
-    if (PK == 0) {
+    if constexpr (PK == 0) {
         lobe_pair_setup<MODE, GRAD>(r.v[0], r.v[1], r.v[2], r.v[3], r.v[4], r.v[5], r.v[6], r.v[7], Lp, Gd, park[0], park[1], park[2], park[3]);
         w0 = r.v[8]; w1 = r.v[9]; w2 = r.v[10];
-    } else {
+    } else if constexpr (PK == 1) {
         PaperTrig tr;
         lobe_pair_setup_paper<MODE, GRAD>(r.v[0], r.v[1], r.v[2], r.v[3], r.v[4], r.v[5], Lp, Gd, tr);
         if (GRAD) { park[0] = tr.st; park[1] = tr.cp; park[2] = tr.sp; park[3] = tr.cu; park[4] = tr.su; park[5] = tr.su; }
-        w0 = tanh2(r.v[6]); w1 = tanh2(r.v[7]); w2 = tanh2(r.v[PK ? 8 : 0]);
+        w0 = tanh2(r.v[6]); w1 = tanh2(r.v[7]); w2 = tanh2(r.v[8]);
     }
 }
 
@@ -281,15 +283,28 @@ __global__ void __launch_bounds__(FWD_TB, NASG_REC_FWD_MINB) nasg_rec_fwd_kernel
             if (elect_one()) stage_issue<PAIR_BYTES>(sc, w.T, stage, bar_full(w, slot));
             stage_advance<NPAIR, PAIR_BYTES>(sc, w.tstride, rec_jump);
             if (++slot == S) { slot = 0; par ^= 1u; }
-            LobePair Lp; LobePairGrad Gd; f2 park[6], w0, w1, w2;
-            setup_pair<PK, MODE, false>(r, Lp, Gd, park, w0, w1, w2);
+            if constexpr (PK == 2) {           // isotropic Table-6 function MODE
+                IsoPair Ip;
+                iso_pair_setup<MODE>(r.v[0], r.v[1], r.v[2], r.v[3], Ip);
 #pragma unroll
-            for (int t = 0; t < CT; ++t) {     // every camera slot is evaluated (iid masks: some lane always needs it); culled slots are zeroed at the store
-                EvalPair T;
-                const f2 G = lobe_pair_eval<false, MODE != 2>(Lp, dx[t], dy[t], dz[t], T);
-                col[t][0] = fma2(w0, G, col[t][0]);
-                col[t][1] = fma2(w1, G, col[t][1]);
-                col[t][2] = fma2(w2, G, col[t][2]);
+                for (int t = 0; t < CT; ++t) {
+                    f2 u0, u1;
+                    const f2 G = iso_pair_eval<MODE, false>(Ip, dx[t], dy[t], dz[t], u0, u1);
+                    col[t][0] = fma2(r.v[4], G, col[t][0]);
+                    col[t][1] = fma2(r.v[5], G, col[t][1]);
+                    col[t][2] = fma2(r.v[6], G, col[t][2]);
+                }
+            } else {
+                LobePair Lp; LobePairGrad Gd; f2 park[6], w0, w1, w2;
+                setup_pair<PK, MODE, false>(r, Lp, Gd, park, w0, w1, w2);
+#pragma unroll
+                for (int t = 0; t < CT; ++t) {     // every camera slot is evaluated (iid masks: some lane always needs it); culled slots are zeroed at the store
+                    EvalPair T;
+                    const f2 G = lobe_pair_eval<false, MODE != 2>(Lp, dx[t], dy[t], dz[t], T);
+                    col[t][0] = fma2(w0, G, col[t][0]);
+                    col[t][1] = fma2(w1, G, col[t][1]);
+                    col[t][2] = fma2(w2, G, col[t][2]);
+                }
             }
         }
         if (valid) {
@@ -388,37 +403,66 @@ __global__ void __launch_bounds__(BWD_TB, NASG_REC_BWD_MINB) nasg_rec_bwd_kernel
             if (elect_one()) stage_issue<PAIR_BYTES>(sc, w.T, stage, bar_full(w, slot));
             stage_advance<NPAIR, PAIR_BYTES>(sc, w.tstride, rec_jump);
             if (++slot == S) { slot = 0; par ^= 1u; }
-            LobePair Lp; LobePairGrad Gd;
-            f2 w0, w1, w2;
-            {       // frame terms the end of the pair needs (quaternion 2/|q| | sines and cosines of the angles) are parked in shared memory
-                f2 park[6];
-                setup_pair<PK, MODE, true>(r, Lp, Gd, park, w0, w1, w2);
-                sts64x2(scr_qs, park[0], park[1]);
-                sts64x2(scr_qs + WT * 16, park[2], park[3]);
-                if (PK) sts64x2(scr_qs + 2 * WT * 16, park[4], park[5]);
-            }
-            AccPair A;
+            f2 g[Rec<PK>::NCOMP];
+            if constexpr (PK == 2) {           // isotropic Table-6 function MODE
+                IsoPair Ip;
+                iso_pair_setup<MODE>(r.v[0], r.v[1], r.v[2], r.v[3], Ip);
+                const f2 w0 = r.v[4], w1 = r.v[5], w2 = r.v[6];
+                f2 gw0 = splat(0.f), gw1 = gw0, gw2 = gw0, gs = gw0, gzx = gw0, gzy = gw0, gzz = gw0;
 #pragma unroll
-            for (int t = 0; t < CT; ++t) {
-                const float4 cam = lds128(scr_cam + t * WT * 16);
-                const float4 gc = lds128(scr_gc + t * WT * 16);         // zero for a culled slot: every contribution vanishes
-                EvalPair T;
-                const f2 G = lobe_pair_eval<true, MODE != 2>(Lp, cam.x, cam.y, cam.z, T);
-                f2 gx = splat(0.f), gy = splat(0.f), gz = splat(0.f);
-                if (t == 0) lobe_pair_bwd<MODE != 2, true>(Lp, T, G, gc.x, gc.y, gc.z, w0, w1, w2, A, gx, gy, gz);
-                else lobe_pair_bwd<MODE != 2, false>(Lp, T, G, gc.x, gc.y, gc.z, w0, w1, w2, A, gx, gy, gz);
-                gd[t][0] += lo(gx) + hi(gx); gd[t][1] += lo(gy) + hi(gy); gd[t][2] += lo(gz) + hi(gz);
-            }
-            f2 park[6], g[Rec<PK>::NCOMP];
-            lds64x2(scr_qs, park[0], park[1]);
-            lds64x2(scr_qs + WT * 16, park[2], park[3]);
-            if (PK) {
-                lds64x2(scr_qs + 2 * WT * 16, park[4], park[5]);
-                const PaperTrig tr{park[0], park[1], park[2], park[3], park[4]};
-                lobe_pair_finish_paper<MODE>(Lp, Gd, A, tr, w0, w1, w2, g[0], g[1], g[2], g[3], g[4], g[5], g[6], g[7], g[PK ? 8 : 0]);
+                for (int t = 0; t < CT; ++t) {
+                    const float4 cam = lds128(scr_cam + t * WT * 16);
+                    const float4 gc = lds128(scr_gc + t * WT * 16);     // zero for a culled slot: every contribution vanishes
+                    f2 Fv, Fr;
+                    const f2 F = iso_pair_eval<MODE, true>(Ip, cam.x, cam.y, cam.z, Fv, Fr);
+                    const f2 c0 = splat(gc.x), c1 = splat(gc.y), c2 = splat(gc.z);
+                    const f2 gF = fma2(w0, c0, fma2(w1, c1, mul2(w2, c2)));             // dL/dF, eq.(6)
+                    gw0 = fma2(F, c0, gw0); gw1 = fma2(F, c1, gw1); gw2 = fma2(F, c2, gw2);
+                    gs = fma2(gF, Fr, gs);
+                    const f2 gv = mul2(gF, Fv);                                         // v = d . zhat
+                    gzx = fma2(gv, splat(cam.x), gzx); gzy = fma2(gv, splat(cam.y), gzy); gzz = fma2(gv, splat(cam.z), gzz);
+                    const f2 gx = mul2(gv, Ip.zx), gy = mul2(gv, Ip.zy), gz = mul2(gv, Ip.zz);
+                    gd[t][0] += lo(gx) + hi(gx); gd[t][1] += lo(gy) + hi(gy); gd[t][2] += lo(gz) + hi(gz);
+                }
+                // zhat = z/|z|: (I - zhat zhat^T)/|z|
+                const f2 dot = fma2(Ip.zx, gzx, fma2(Ip.zy, gzy, mul2(Ip.zz, gzz)));
+                g[0] = mul2(fma2(neg2(Ip.zx), dot, gzx), Ip.inv);
+                g[1] = mul2(fma2(neg2(Ip.zy), dot, gzy), Ip.inv);
+                g[2] = mul2(fma2(neg2(Ip.zz), dot, gzz), Ip.inv);
+                g[3] = gs; g[4] = gw0; g[5] = gw1; g[6] = gw2;
             } else {
-                lobe_pair_finish2(Lp, Gd, A, park[0], park[1], park[2], park[3], g[4], g[5], g[6], g[7], g[0], g[1], g[2], g[3]);
-                g[8] = A.gw0; g[9] = A.gw1; g[PK ? 0 : 10] = A.gw2;
+                LobePair Lp; LobePairGrad Gd;
+                f2 w0, w1, w2;
+                {       // frame terms the end of the pair needs (quaternion 2/|q| | sines and cosines of the angles) are parked in shared memory
+                    f2 park[6];
+                    setup_pair<PK, MODE, true>(r, Lp, Gd, park, w0, w1, w2);
+                    sts64x2(scr_qs, park[0], park[1]);
+                    sts64x2(scr_qs + WT * 16, park[2], park[3]);
+                    if constexpr (PK == 1) sts64x2(scr_qs + 2 * WT * 16, park[4], park[5]);
+                }
+                AccPair A;
+#pragma unroll
+                for (int t = 0; t < CT; ++t) {
+                    const float4 cam = lds128(scr_cam + t * WT * 16);
+                    const float4 gc = lds128(scr_gc + t * WT * 16);         // zero for a culled slot: every contribution vanishes
+                    EvalPair T;
+                    const f2 G = lobe_pair_eval<true, MODE != 2>(Lp, cam.x, cam.y, cam.z, T);
+                    f2 gx = splat(0.f), gy = splat(0.f), gz = splat(0.f);
+                    if (t == 0) lobe_pair_bwd<MODE != 2, true>(Lp, T, G, gc.x, gc.y, gc.z, w0, w1, w2, A, gx, gy, gz);
+                    else lobe_pair_bwd<MODE != 2, false>(Lp, T, G, gc.x, gc.y, gc.z, w0, w1, w2, A, gx, gy, gz);
+                    gd[t][0] += lo(gx) + hi(gx); gd[t][1] += lo(gy) + hi(gy); gd[t][2] += lo(gz) + hi(gz);
+                }
+                f2 park[6];
+                lds64x2(scr_qs, park[0], park[1]);
+                lds64x2(scr_qs + WT * 16, park[2], park[3]);
+                if constexpr (PK == 1) {
+                    lds64x2(scr_qs + 2 * WT * 16, park[4], park[5]);
+                    const PaperTrig tr{park[0], park[1], park[2], park[3], park[4]};
+                    lobe_pair_finish_paper<MODE>(Lp, Gd, A, tr, w0, w1, w2, g[0], g[1], g[2], g[3], g[4], g[5], g[6], g[7], g[8]);
+                } else {
+                    lobe_pair_finish2(Lp, Gd, A, park[0], park[1], park[2], park[3], g[4], g[5], g[6], g[7], g[0], g[1], g[2], g[3]);
+                    g[8] = A.gw0; g[9] = A.gw1; g[10] = A.gw2;
+                }
             }
             if (valid) {
 #pragma unroll
@@ -501,7 +545,7 @@ namespace rec = lp::rec;
 // ---------------------------------------------------------------------------------------------
 int64_t rec_total_floats(int64_t N, int K, int pk)
 {
-    return ((N + rec::WT - 1) / rec::WT) * (int64_t)(pk ? rec::Rec<1>::rec_floats(K) : rec::Rec<0>::rec_floats(K));
+    return ((N + rec::WT - 1) / rec::WT) * (int64_t)(pk == 2 ? rec::Rec<2>::rec_floats(K) : pk == 1 ? rec::Rec<1>::rec_floats(K) : rec::Rec<0>::rec_floats(K));
 }
 
 template <typename Kernel>
@@ -557,7 +601,7 @@ static cudaError_t launch_rec_fwd_pk(const RecFwdParams &p, int K, int mode, cud
 }
 cudaError_t launch_nasg_rec_fwd(const RecFwdParams &p, int K, int mode, int pk, cudaStream_t st)
 {
-    return pk ? launch_rec_fwd_pk<1>(p, K, mode, st) : launch_rec_fwd_pk<0>(p, K, mode, st);
+    return pk == 2 ? launch_rec_fwd_pk<2>(p, K, mode, st) : pk == 1 ? launch_rec_fwd_pk<1>(p, K, mode, st) : launch_rec_fwd_pk<0>(p, K, mode, st);
 }
 
 template <int K, int CT, int PK>
@@ -595,7 +639,7 @@ static cudaError_t launch_rec_bwd_pk(const RecBwdParams &p, int K, int mode, cud
 }
 cudaError_t launch_nasg_rec_bwd(const RecBwdParams &p, int K, int mode, int pk, cudaStream_t st)
 {
-    return pk ? launch_rec_bwd_pk<1>(p, K, mode, st) : launch_rec_bwd_pk<0>(p, K, mode, st);
+    return pk == 2 ? launch_rec_bwd_pk<2>(p, K, mode, st) : pk == 1 ? launch_rec_bwd_pk<1>(p, K, mode, st) : launch_rec_bwd_pk<0>(p, K, mode, st);
 }
 
 cudaError_t launch_rec_pack(int64_t N, int K, const float *means, const float *quat, const float *shape, const float *amp, const float *dc,
