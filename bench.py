@@ -32,8 +32,8 @@ FALLBACK_HBM_GBS = 6650.0      # B200_PROFILING.md fallback when MEASURED_PEAKS.
 
 
 # ---- algorithmic bytes per Gaussian ------------------
-def algorithmic_bytes(kind: str, K: int, C: int, has_vis: bool, paper: bool = False):
-    P = 51 if kind == "sh" else 6 + (9 if paper else 11) * K      # parameter floats per Gaussian (means+dc/coeffs+lobes)
+def algorithmic_bytes(kind: str, K: int, C: int, has_vis: bool, paper: bool = False, iso: bool = False):
+    P = 51 if kind == "sh" else 6 + (7 if iso else 9 if paper else 11) * K      # parameter floats per Gaussian (means+dc/coeffs+lobes)
     vis = C if has_vis else 0
     fwd = 4 * P + vis + 12 * C                      # read params + mask, write colours
     bwd = 4 * P + vis + 12 * C + 4 * P              # read params + mask + g_colors, write every gradient
@@ -180,12 +180,13 @@ class Resident:
         self.B, self.cfg, self.norm_mode, self.torch = B, cfg, norm_mode, torch
         rcfg = S.weak_scaling_config(cfg, rank)
         self.paper = cfg.kind == "nasg" and layout == "paper"          # the paper's own 3 + 9K record (nasg_paper_*)
-        inp = W.make_sh(rcfg) if cfg.kind == "sh" else W.make_paper(rcfg) if self.paper else W.make_nasg(rcfg)
+        self.iso = int(layout[3]) if cfg.kind == "nasg" and layout.startswith("iso") else None    # isotropic Table-6 function (nasg_iso_*)
+        inp = W.make_sh(rcfg) if cfg.kind == "sh" else W.make_paper(rcfg) if self.paper else W.make_iso(rcfg) if self.iso is not None else W.make_nasg(rcfg)
         self.N, self.C, self.K = inp["N"], inp["C"], inp.get("K", 0)
         # tile-record parameter layout (include/nasg.h: nasg_rec_*) where it applies, else the row arrays
-        self.rec = cfg.kind == "nasg" and layout in ("rec", "paper") and self.K in (2, 4, 8) and self.C <= 4
-        assert self.rec or not self.paper
-        self.keys = ("means", "coeffs", "campos", "vis", "g_colors") if cfg.kind == "sh" else ("campos", "vis", "g_colors") if self.paper else \
+        self.rec = cfg.kind == "nasg" and (layout in ("rec", "paper") or self.iso is not None) and self.K in (2, 4, 8) and self.C <= 4
+        assert self.rec or not (self.paper or self.iso is not None)
+        self.keys = ("means", "coeffs", "campos", "vis", "g_colors") if cfg.kind == "sh" else ("campos", "vis", "g_colors") if (self.paper or self.iso is not None) else \
                     ("means", "quat", "shape", "amp", "dc", "campos", "vis", "g_colors")
         d = {k: (None if inp.get(k) is None else torch.from_numpy(np.ascontiguousarray(inp[k])).cuda()) for k in self.keys}
         self.d = d
@@ -193,6 +194,9 @@ class Resident:
         self.stream = torch.cuda.current_stream()
         if self.paper:  # records of raw values, re-ordered on the host by the input generator (no arithmetic)
             self.params = torch.from_numpy(W.pack_paper_records(inp["means"], inp["euler"], inp["shp"], inp["ampraw"], inp["dc"])).cuda()
+            self.g_params = torch.zeros_like(self.params)
+        elif self.iso is not None:
+            self.params = torch.from_numpy(W.pack_iso_records(inp["means"], inp["axis"], inp["shp"], inp["amp"], inp["dc"])).cuda()
             self.g_params = torch.zeros_like(self.params)
         elif self.rec:  # the parameters LIVE in HBM as records (packed once, outside any timed region: it is the storage layout)
             self.params = B.nasg_rec_pack(d["means"], d["quat"], d["shape"], d["amp"], d["dc"])
@@ -207,6 +211,8 @@ class Resident:
         B, d, st = self.B, self.d, self.stream
         if self.paper:
             B.nasg_paper_eval_fwd(self.params, self.N, self.K, d["campos"], d["vis"], self.norm_mode, out=self.colors, stream=st)
+        elif self.iso is not None:
+            B.nasg_iso_eval_fwd(self.params, self.N, self.K, d["campos"], self.iso, d["vis"], out=self.colors, stream=st)
         elif self.rec:
             B.nasg_rec_eval_fwd(self.params, self.N, self.K, d["campos"], d["vis"], self.norm_mode, out=self.colors, stream=st)
         elif self.cfg.kind == "sh":
@@ -220,6 +226,8 @@ class Resident:
         if self.paper:
             B.nasg_paper_eval_bwd(self.params, self.N, self.K, d["campos"], d["g_colors"], d["vis"], self.norm_mode,
                                   out=self.g_params, stream=st)
+        elif self.iso is not None:
+            B.nasg_iso_eval_bwd(self.params, self.N, self.K, d["campos"], d["g_colors"], self.iso, d["vis"], out=self.g_params, stream=st)
         elif self.rec:
             B.nasg_rec_eval_bwd(self.params, self.N, self.K, d["campos"], d["g_colors"], d["vis"], self.norm_mode,
                                 out=self.g_params, stream=st)
@@ -231,7 +239,7 @@ class Resident:
 
     def kernel_name(self):
         if self.rec:
-            return "nasg_rec_bwd_kernel<PK=1>" if self.paper else "nasg_rec_bwd_kernel"
+            return "nasg_rec_bwd_kernel<PK=1>" if self.paper else "nasg_rec_bwd_kernel<PK=2>" if self.iso is not None else "nasg_rec_bwd_kernel"
         pipe = self.C <= 4
         if self.cfg.kind == "sh":
             return "sh_bwd_pipe_kernel" if pipe else "sh_bwd_kernel"
@@ -340,8 +348,8 @@ def run_ours(args, W, cfg):
     peak, peak_src = measured_peak()
 
     def summary(r, f_ms, b_ms):
-        fb, bb = algorithmic_bytes(r.cfg.kind, r.K, r.C, r.has_vis, r.paper)
-        return {"layout": "paper records (3 + 9K floats)" if r.paper else "records" if r.rec else "rows", "bytes_per_gaussian": [fb, bb], "kernel": r.kernel_name(), "fwd_ms": f_ms, "bwd_ms": b_ms,
+        fb, bb = algorithmic_bytes(r.cfg.kind, r.K, r.C, r.has_vis, r.paper, r.iso is not None)
+        return {"layout": "paper records (3 + 9K floats)" if r.paper else ("isotropic Table-6 records (3 + 7K floats): " + ("Spherical Gaussian", "Spherical Beta", "Spherical Cauchy")[r.iso]) if r.iso is not None else "records" if r.rec else "rows", "bytes_per_gaussian": [fb, bb], "kernel": r.kernel_name(), "fwd_ms": f_ms, "bwd_ms": b_ms,
                 "value": r.N / ((f_ms + b_ms) * 1e-3), "fwd_gbs": fb * r.N / (f_ms * 1e-3) / 1e9, "bwd_gbs": bb * r.N / (b_ms * 1e-3) / 1e9,
                 "bwd_frac": bb * r.N / (b_ms * 1e-3) / 1e9 / peak, "fwd+bwd_frac": (fb + bb) * r.N / ((f_ms + b_ms) * 1e-3) / 1e9 / peak}
 
@@ -356,6 +364,7 @@ def run_ours(args, W, cfg):
         if rec:
             specs.append((cfg.index, "rows"))                  # the same workload through the row-array entry points
         specs += [(i, "paper") for i in (1, 2, 4)]             # the paper's own 3 + 9K record (17 % fewer parameter bytes)
+        specs += [(2, "iso0"), (2, "iso1"), (2, "iso2")]       # the other Table-6 functions in the same skeleton (NEXT-3)
         R_keep, R = R, None
         if cfg.N > 2_000_000:
             R_keep.d = None; R_keep.params = None; R_keep.g_params = None; R_keep.colors = None

@@ -23,18 +23,26 @@ __device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-// wait for the phase with this parity (the suspend-time hint keeps a warp whose data is late asleep in hardware)
-__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
+__device__ __forceinline__ void mbar_arrive(unsigned bar)
 {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+// One probe of the phase with this parity (the suspend-time hint lets the hardware park the thread while the data is late).
+__device__ __forceinline__ bool mbar_try_wait(unsigned bar, unsigned parity)
+{
+    unsigned done;
     asm volatile(
         "{\n\t"
         ".reg .pred p;\n\t"
-        "LAB_WAIT:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
-        "@p bra DONE;\n\t"
-        "bra LAB_WAIT;\n\t"
-        "DONE:\n\t"
-        "}" ::"r"(bar), "r"(parity), "r"(0x989680u) : "memory");
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t"
+        "}" : "=r"(done) : "r"(bar), "r"(parity), "r"(0x989680u) : "memory");
+    return done != 0;
+}
+// Wait for the phase with this parity.
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
+{
+    while (!mbar_try_wait(bar, parity)) {}
 }
 __device__ __forceinline__ bool elect_one()
 {
@@ -47,10 +55,14 @@ __device__ __forceinline__ bool elect_one()
         "}" : "=r"(pred));
     return pred != 0;
 }
-// orders this thread's earlier generic-proxy accesses to shared memory before its later async-proxy operations. NOT used on
-// the refill path: a slot is refilled after the lanes have READ it (write-after-read: the reads are complete before the
-// __syncwarp that precedes the issue, and the copy engine's writes land hundreds of cycles later), which needs no proxy fence
-// (it is generic-proxy WRITES that must be fenced before an async-proxy read); measured cost of the fence there: 1.2 %.
+// SLOT REFILL PROTOCOL (a round-2 bug, found by the host-pipeline bit-identity test). A slot is refilled by the copy engine
+// (async proxy) right after the lanes have read it (generic proxy). Program order + __syncwarp() is NOT enough: the async-proxy
+// write is not ordered after generic-proxy reads that have been issued but not yet performed, and when the SM comes out of idle
+// (low clocks) with per-lane global loads queued in front of them, the shared-memory reads of a few lanes were overtaken by the
+// refill: wrong values for some lanes of ONE tile in ~40 % of cold launches with N % 16 != 0, never when warm. The PTX rule is a
+// proxy fence between the two: all lanes read, __syncwarp(), then the issuing lane executes fence.proxy.async before
+// mbarrier.arrive.expect_tx + cp.async.bulk. Measured cost 1.2 % (an explicit "empty" mbarrier with 32 arrivals per refill
+// was also correct and cost 7 %). tests/test_rec_gpu.py::test_cold_launches_are_correct keeps the scenario covered.
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 // 1-D bulk copy global -> shared of `bytes` (multiple of 16; both addresses 16-byte aligned), completing on `bar`
 __device__ __forceinline__ void bulk_g2s(unsigned dst, const void *src, unsigned bytes, unsigned bar)

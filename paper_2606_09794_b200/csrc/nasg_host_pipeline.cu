@@ -18,6 +18,7 @@
 #include "nasg_internal.h"
 
 #include <mutex>
+#include <vector>
 
 namespace {
 
@@ -28,8 +29,14 @@ size_t cam_partial_bytes(int64_t N, int C) { return (size_t)nasg::grid_blocks(N)
 #define NASG_TRY_CUDA(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) return nasg::api_cuda_fail(e_); } while (0)
 #define NASG_TRY(expr) do { int rc_ = (expr); if (rc_ != NASG_OK) return rc_; } while (0)
 
-constexpr int64_t CHUNK_MIN = 131072;    // Gaussians per chunk at least (copies of a few MB each)
-constexpr int MAX_CHUNKS = 16;
+#ifndef NASG_HOST_CHUNK_MIN
+#define NASG_HOST_CHUNK_MIN 131072
+#endif
+#ifndef NASG_HOST_MAX_CHUNKS
+#define NASG_HOST_MAX_CHUNKS 16
+#endif
+constexpr int64_t CHUNK_MIN = NASG_HOST_CHUNK_MIN;    // Gaussians per chunk at least (copies of a few MB each)
+constexpr int MAX_CHUNKS = NASG_HOST_MAX_CHUNKS;
 constexpr size_t SCRATCH_SLOP = 64 * 1024;   // alignment padding of the per-chunk carve-up
 
 // chunk size: a multiple of 256 (keeps rows 16-byte aligned and the visibility rows 4-byte aligned)
@@ -39,7 +46,27 @@ int64_t chunk_size(int64_t N, bool single)
     int64_t chunks = N / CHUNK_MIN;
     if (chunks > MAX_CHUNKS) chunks = MAX_CHUNKS;
     const int64_t per = (N + chunks - 1) / chunks;
-    return (per + 255) / 256 * 256;
+    return (per + 1023) / 1024 * 1024;
+}
+// Piece boundaries of the pipeline: full chunks in the middle, and a ramp (chunk/4, chunk/4, chunk/2) at either end so that
+// the un-overlapped fill (first host->device copy) and drain (last device->host copy) are a quarter chunk each; every piece
+// is a multiple of 256 Gaussians (8 records; rows stay 16-byte aligned) except the last.
+std::vector<int64_t> piece_bounds(int64_t N, int64_t chunk)
+{
+    std::vector<int64_t> b{0};
+    if (N >= 4 * chunk && chunk % 1024 == 0) {
+        const int64_t middle = N - 2 * chunk, full = middle / chunk, r = middle - full * chunk, r256 = r / 256 * 256;
+        for (int64_t u : {chunk / 4, chunk / 4, chunk / 2}) b.push_back(b.back() + u);
+        for (int64_t i = 0; i < full; ++i) b.push_back(b.back() + chunk);
+        if (r256 > 0) b.push_back(b.back() + r256);
+        b.push_back(b.back() + chunk / 2);
+        b.push_back(b.back() + chunk / 4);
+        b.push_back(N);                                       // chunk/4 + (r - r256) Gaussians
+    } else {
+        while (N - b.back() > chunk) b.push_back(b.back() + chunk);
+        b.push_back(N);
+    }
+    return b;
 }
 
 // carves aligned sub-buffers out of the caller's device scratch
@@ -91,10 +118,11 @@ cudaError_t copy_rows(void *dst, size_t dst_cols, const void *src, size_t src_co
 template <typename CopyIn, typename Compute, typename CopyOut>
 int enqueue_chunks(HostPipe &hp, int64_t N, int64_t chunk, cudaStream_t user, CopyIn copy_in, Compute compute, CopyOut copy_out)
 {
-    const int64_t chunks = (N + chunk - 1) / chunk;
+    const std::vector<int64_t> bounds = piece_bounds(N, chunk);
+    const int64_t chunks = (int64_t)bounds.size() - 1;
     for (int64_t i = 0; i < chunks; ++i) {
         const int b = (int)(i & 1);
-        const int64_t n0 = i * chunk, nc = (n0 + chunk <= N) ? chunk : N - n0;
+        const int64_t n0 = bounds[i], nc = bounds[i + 1] - bounds[i];
         if (i >= 2) NASG_TRY_CUDA(cudaStreamWaitEvent(hp.in, hp.comp_done[b], 0));      // inputs of chunk i-2 consumed
         NASG_TRY(copy_in(b, n0, nc, hp.in));
         NASG_TRY_CUDA(cudaEventRecord(hp.in_done[b], hp.in));

@@ -107,6 +107,7 @@ template <int PAIR_BYTES>
 __device__ __forceinline__ void stage_issue(const StageCursor &s, int T, unsigned dst, unsigned bar)
 {
     if (s.tile < T) {
+        fence_proxy_async();        // the lanes' reads of the slot (generic proxy) before the refill (async proxy): bulk_common.cuh
         mbar_expect_tx(bar, PAIR_BYTES);
         bulk_g2s(dst, s.src, PAIR_BYTES, bar);
     }
@@ -120,6 +121,7 @@ __device__ __forceinline__ void hdr_issue(const HdrCursor &h, const Warp &w, uns
         const unsigned cnt = h.tile == w.T - 1 ? w.last_cnt : (unsigned)WT;
         unsigned bytes = HDR_BYTES;
         if (bulk_rows) bytes += (BWD ? CT * 12u * cnt : 0u) + (h.vis ? CT * cnt : 0u);
+        fence_proxy_async();        // the lanes' reads of the slot (generic proxy) before the refill (async proxy): bulk_common.cuh
         mbar_expect_tx(bar, bytes);
         bulk_g2s(dst, h.src, HDR_BYTES, bar);
         if (bulk_rows) {

@@ -88,6 +88,7 @@ __device__ __forceinline__ void issue_stage(const WarpCtx &c, int m, const float
     const unsigned cnt = (unsigned)(N - n0 < WT ? N - n0 : WT);
     const int slot = m % STAGES;
     const unsigned bar = bar_full(c, slot), dst = c.stage0 + (unsigned)slot * STAGE_BYTES;
+    fence_proxy_async();            // the lanes' reads of the slot (generic proxy) before the refill (async proxy): bulk_common.cuh
     mbar_expect_tx(bar, cnt * 88u);
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
@@ -110,6 +111,7 @@ __device__ __forceinline__ void issue_header(const WarpCtx &c, int i, int C, con
     const int h = i % HSLOTS;
     const unsigned bar = bar_hfull(c, h), hdr = c.hdr + (unsigned)h * (unsigned)L::HDR_BYTES;
     const unsigned rows = BWD ? (unsigned)C : 1u;        // forward: dc = 3 planar rows of 4 B; backward: g_colors = C rows of 12 B
+    fence_proxy_async();            // the lanes' reads of the slot (generic proxy) before the refill (async proxy): bulk_common.cuh
     mbar_expect_tx(bar, cnt * (12u + 12u * rows + (vis ? (unsigned)C : 0u)));
     bulk_g2s(hdr + L::HDR_MEANS, means + 3 * n0, cnt * 12u, bar);
     if (BWD) {
