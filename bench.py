@@ -32,11 +32,12 @@ FALLBACK_HBM_GBS = 6650.0      # B200_PROFILING.md fallback when MEASURED_PEAKS.
 
 
 # ---- algorithmic bytes per Gaussian ------------------
-def algorithmic_bytes(kind: str, K: int, C: int, has_vis: bool, paper: bool = False, iso: bool = False):
+def algorithmic_bytes(kind: str, K: int, C: int, has_vis: bool, paper: bool = False, iso: bool = False, bf16: bool = False):
     P = 51 if kind == "sh" else 6 + (7 if iso else 9 if paper else 11) * K      # parameter floats per Gaussian (means+dc/coeffs+lobes)
+    Pr = 4 * P - (14 * K if bf16 else 0)            # bytes read: bf16 storage of quaternion (4) and amplitude (3) saves 2 B each
     vis = C if has_vis else 0
-    fwd = 4 * P + vis + 12 * C                      # read params + mask, write colours
-    bwd = 4 * P + vis + 12 * C + 4 * P              # read params + mask + g_colors, write every gradient
+    fwd = Pr + vis + 12 * C                         # read params + mask, write colours
+    bwd = Pr + vis + 12 * C + 4 * P                 # read params + mask + g_colors, write every gradient (fp32)
     return fwd, bwd
 
 
@@ -184,7 +185,8 @@ class Resident:
         inp = W.make_sh(rcfg) if cfg.kind == "sh" else W.make_paper(rcfg) if self.paper else W.make_iso(rcfg) if self.iso is not None else W.make_nasg(rcfg)
         self.N, self.C, self.K = inp["N"], inp["C"], inp.get("K", 0)
         # tile-record parameter layout (include/nasg.h: nasg_rec_*) where it applies, else the row arrays
-        self.rec = cfg.kind == "nasg" and (layout in ("rec", "paper") or self.iso is not None) and self.K in (2, 4, 8) and self.C <= 4
+        self.bf16 = cfg.kind == "nasg" and layout == "rec16"             # bf16 quaternion / amplitude storage (nasg_rec16_*)
+        self.rec = cfg.kind == "nasg" and (layout in ("rec", "paper", "rec16") or self.iso is not None) and self.K in (2, 4, 8) and self.C <= 4
         assert self.rec or not (self.paper or self.iso is not None)
         self.keys = ("means", "coeffs", "campos", "vis", "g_colors") if cfg.kind == "sh" else ("campos", "vis", "g_colors") if (self.paper or self.iso is not None) else \
                     ("means", "quat", "shape", "amp", "dc", "campos", "vis", "g_colors")
@@ -199,8 +201,8 @@ class Resident:
             self.params = torch.from_numpy(W.pack_iso_records(inp["means"], inp["axis"], inp["shp"], inp["amp"], inp["dc"])).cuda()
             self.g_params = torch.zeros_like(self.params)
         elif self.rec:  # the parameters LIVE in HBM as records (packed once, outside any timed region: it is the storage layout)
-            self.params = B.nasg_rec_pack(d["means"], d["quat"], d["shape"], d["amp"], d["dc"])
-            self.g_params = torch.zeros_like(self.params)
+            self.params = (B.nasg_rec16_pack if self.bf16 else B.nasg_rec_pack)(d["means"], d["quat"], d["shape"], d["amp"], d["dc"])
+            self.g_params = torch.zeros(B.nasg_rec_floats(self.N, self.K), dtype=torch.float32, device="cuda")
             for k in ("means", "quat", "shape", "amp", "dc"):
                 d[k] = None
         else:
@@ -214,7 +216,8 @@ class Resident:
         elif self.iso is not None:
             B.nasg_iso_eval_fwd(self.params, self.N, self.K, d["campos"], self.iso, d["vis"], out=self.colors, stream=st)
         elif self.rec:
-            B.nasg_rec_eval_fwd(self.params, self.N, self.K, d["campos"], d["vis"], self.norm_mode, out=self.colors, stream=st)
+            (B.nasg_rec16_eval_fwd if self.bf16 else B.nasg_rec_eval_fwd)(self.params, self.N, self.K, d["campos"], d["vis"], self.norm_mode,
+                                                                         out=self.colors, stream=st)
         elif self.cfg.kind == "sh":
             B.sh_eval_fwd(d["means"], d["coeffs"], d["campos"], d["vis"], out=self.colors, stream=st)
         else:
@@ -229,8 +232,8 @@ class Resident:
         elif self.iso is not None:
             B.nasg_iso_eval_bwd(self.params, self.N, self.K, d["campos"], d["g_colors"], self.iso, d["vis"], out=self.g_params, stream=st)
         elif self.rec:
-            B.nasg_rec_eval_bwd(self.params, self.N, self.K, d["campos"], d["g_colors"], d["vis"], self.norm_mode,
-                                out=self.g_params, stream=st)
+            (B.nasg_rec16_eval_bwd if self.bf16 else B.nasg_rec_eval_bwd)(self.params, self.N, self.K, d["campos"], d["g_colors"], d["vis"],
+                                                                         self.norm_mode, out=self.g_params, stream=st)
         elif self.cfg.kind == "sh":
             B.sh_eval_bwd(d["means"], d["coeffs"], d["campos"], d["g_colors"], d["vis"], out=self.grads, stream=st)
         else:
@@ -239,7 +242,7 @@ class Resident:
 
     def kernel_name(self):
         if self.rec:
-            return "nasg_rec_bwd_kernel<PK=1>" if self.paper else "nasg_rec_bwd_kernel<PK=2>" if self.iso is not None else "nasg_rec_bwd_kernel"
+            return "nasg_rec_bwd_kernel<PK=1>" if self.paper else "nasg_rec_bwd_kernel<PK=2>" if self.iso is not None else "nasg_rec_bwd_kernel<PK=3>" if self.bf16 else "nasg_rec_bwd_kernel"
         pipe = self.C <= 4
         if self.cfg.kind == "sh":
             return "sh_bwd_pipe_kernel" if pipe else "sh_bwd_kernel"
@@ -348,8 +351,8 @@ def run_ours(args, W, cfg):
     peak, peak_src = measured_peak()
 
     def summary(r, f_ms, b_ms):
-        fb, bb = algorithmic_bytes(r.cfg.kind, r.K, r.C, r.has_vis, r.paper, r.iso is not None)
-        return {"layout": "paper records (3 + 9K floats)" if r.paper else ("isotropic Table-6 records (3 + 7K floats): " + ("Spherical Gaussian", "Spherical Beta", "Spherical Cauchy")[r.iso]) if r.iso is not None else "records" if r.rec else "rows", "bytes_per_gaussian": [fb, bb], "kernel": r.kernel_name(), "fwd_ms": f_ms, "bwd_ms": b_ms,
+        fb, bb = algorithmic_bytes(r.cfg.kind, r.K, r.C, r.has_vis, r.paper, r.iso is not None, r.bf16)
+        return {"layout": "records, bf16 quaternion + amplitude (fp32 arithmetic and gradients)" if r.bf16 else "paper records (3 + 9K floats)" if r.paper else ("isotropic Table-6 records (3 + 7K floats): " + ("Spherical Gaussian", "Spherical Beta", "Spherical Cauchy")[r.iso]) if r.iso is not None else "records" if r.rec else "rows", "bytes_per_gaussian": [fb, bb], "kernel": r.kernel_name(), "fwd_ms": f_ms, "bwd_ms": b_ms,
                 "value": r.N / ((f_ms + b_ms) * 1e-3), "fwd_gbs": fb * r.N / (f_ms * 1e-3) / 1e9, "bwd_gbs": bb * r.N / (b_ms * 1e-3) / 1e9,
                 "bwd_frac": bb * r.N / (b_ms * 1e-3) / 1e9 / peak, "fwd+bwd_frac": (fb + bb) * r.N / ((f_ms + b_ms) * 1e-3) / 1e9 / peak}
 
@@ -364,6 +367,7 @@ def run_ours(args, W, cfg):
         if rec:
             specs.append((cfg.index, "rows"))                  # the same workload through the row-array entry points
         specs += [(i, "paper") for i in (1, 2, 4)]             # the paper's own 3 + 9K record (17 % fewer parameter bytes)
+        specs += [(i, "rec16") for i in (1, 2, 4)]             # bf16 storage of quaternion and amplitude (NEXT-3)
         specs += [(2, "iso0"), (2, "iso1"), (2, "iso2")]       # the other Table-6 functions in the same skeleton (NEXT-3)
         R_keep, R = R, None
         if cfg.N > 2_000_000:

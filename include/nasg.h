@@ -167,6 +167,21 @@ int nasg_paper_eval_fwd(const nasg_rec_inputs *in, float *colors, int norm_mode,
 int nasg_paper_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float *g_params, int norm_mode,
                         void *cuda_stream);
 
+/* ---- reduced-precision parameter STORAGE: bfloat16 quaternion and amplitude ----------
+ * The record of nasg_rec_* with the quaternion and the amplitude of every lobe stored as bfloat16 (the arithmetic stays fp32;
+ * the (log Lambda, log lambda, k, phi) group stays fp32 because it feeds the exponent; means and dc stay fp32). Per pair:
+ *     words [32 c + lane]           c = 0..3   quaternion: bf16 of lobe 2j | bf16 of lobe 2j+1 << 16
+ *     words [128 + 64 c + 2 lane + h]  c = 0..3  shape, fp32
+ *     words [384 + 32 c + lane]     c = 0..2   amplitude, bf16 pair
+ * = 480 32-bit words per pair after the 192-word header: 36 instead of 50 words per Gaussian at K = 4 (-28 % parameter bytes).
+ * nasg_rec16_pack rounds to nearest even. The GRADIENT record is the fp32 record of nasg_rec_eval_bwd (nasg_rec_floats).
+ * What bf16 storage does to the colours (oracle on the rounded values against the fp32 values, cfg2 recipe): DESIGN.md 11. */
+size_t nasg_rec16_floats(int64_t N, int32_t K);          /* 32-bit words of a bf16 parameter record array */
+int nasg_rec16_pack(const nasg_inputs *in, float *params, void *cuda_stream);
+int nasg_rec16_eval_fwd(const nasg_rec_inputs *in, float *colors, int norm_mode, void *cuda_stream);
+int nasg_rec16_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float *g_params, int norm_mode,
+                        void *cuda_stream);
+
 /* ---- other spherical functions of the paper's Table 6 in the same skeleton ---------
  * colour = c0 + sum_l w_l c_l G_l(d . zhat_l) (eq.(6)) with an ISOTROPIC, normalised lobe:
  *     NASG_ISO_SG      0   Spherical Gaussian  G = exp{lambda (z.d - 1)},  c = lambda/(2 pi (1 - e^{-2 lambda})),  lambda = e^raw

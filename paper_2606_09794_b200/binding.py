@@ -25,7 +25,8 @@ SYMBOLS = ("nasg_eval_fwd", "nasg_eval_bwd", "sh_eval_fwd", "sh_eval_bwd", "nasg
            "nasg_rec_floats", "nasg_rec_pack", "nasg_rec_unpack", "nasg_rec_eval_fwd", "nasg_rec_eval_bwd",
            "nasg_rec_host_scratch_bytes", "nasg_rec_eval_fwd_bwd_host", "nasg_paper_floats", "nasg_paper_eval_fwd",
            "nasg_paper_eval_bwd", "nasg_paper_host_scratch_bytes", "nasg_paper_eval_fwd_bwd_host",
-           "nasg_iso_floats", "nasg_iso_eval_fwd", "nasg_iso_eval_bwd")
+           "nasg_iso_floats", "nasg_iso_eval_fwd", "nasg_iso_eval_bwd",
+           "nasg_rec16_floats", "nasg_rec16_pack", "nasg_rec16_eval_fwd", "nasg_rec16_eval_bwd")
 
 
 class NasgError(RuntimeError):
@@ -90,6 +91,11 @@ def _load():
     lib.nasg_rec_unpack.argtypes = [i64, i32, vp, vp, vp, vp, vp, vp, vp]
     lib.nasg_rec_eval_fwd.argtypes = [C.POINTER(_RecInputs), vp, C.c_int, vp]
     lib.nasg_rec_eval_bwd.argtypes = [C.POINTER(_RecInputs), vp, vp, C.c_int, vp]
+    lib.nasg_rec16_floats.argtypes = [i64, i32]
+    lib.nasg_rec16_floats.restype = sz
+    lib.nasg_rec16_pack.argtypes = [C.POINTER(_Inputs), vp, vp]
+    lib.nasg_rec16_eval_fwd.argtypes = [C.POINTER(_RecInputs), vp, C.c_int, vp]
+    lib.nasg_rec16_eval_bwd.argtypes = [C.POINTER(_RecInputs), vp, vp, C.c_int, vp]
     lib.nasg_iso_floats.argtypes = [i64, i32]
     lib.nasg_iso_floats.restype = sz
     lib.nasg_iso_eval_fwd.argtypes = [C.POINTER(_RecInputs), vp, C.c_int, vp]
@@ -107,7 +113,7 @@ def _load():
     for name in ("nasg_eval_fwd", "nasg_eval_bwd", "sh_eval_fwd", "sh_eval_bwd", "nasg_eval_fwd_bwd_host",
                  "sh_eval_fwd_bwd_host", "nasg_rec_pack", "nasg_rec_unpack", "nasg_rec_eval_fwd", "nasg_rec_eval_bwd",
                  "nasg_rec_eval_fwd_bwd_host", "nasg_paper_eval_fwd", "nasg_paper_eval_bwd", "nasg_paper_eval_fwd_bwd_host",
-                 "nasg_iso_eval_fwd", "nasg_iso_eval_bwd"):
+                 "nasg_iso_eval_fwd", "nasg_iso_eval_bwd", "nasg_rec16_pack", "nasg_rec16_eval_fwd", "nasg_rec16_eval_bwd"):
         getattr(lib, name).restype = C.c_int
     return lib
 
@@ -466,4 +472,56 @@ def nasg_iso_eval_bwd(params, N: int, K: int, campos, g_colors, kind: int, vis=N
     rc = _lib.nasg_iso_eval_bwd(C.byref(inp), _ptr(g_colors), _ptr(out), int(kind), _stream(stream))
     if rc != 0:
         raise NasgError(rc, "nasg_iso_eval_bwd")
+    return out
+
+
+# ---- bf16 parameter storage (include/nasg.h: nasg_rec16_*) ------------------------------------------
+def nasg_rec16_floats(N: int, K: int) -> int:
+    return int(_lib.nasg_rec16_floats(N, K))
+
+
+def nasg_rec16_pack(means, quat, shape, amp, dc, out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    """Row arrays -> tile records with bf16 quaternion / amplitude (round to nearest even): float32-typed word tensor."""
+    K, N = int(quat.shape[0]), int(quat.shape[1])
+    f32 = torch.float32
+    _chk(means, "means", (N, 3), f32, "cuda"); _chk(quat, "quat", (K, N, 4), f32, "cuda")
+    _chk(shape, "shape", (K, N, 4), f32, "cuda"); _chk(amp, "amp", (K, 3, N), f32, "cuda"); _chk(dc, "dc", (3, N), f32, "cuda")
+    inp = _Inputs(N, K, 1, _ptr(means), _ptr(quat), _ptr(shape), _ptr(amp), _ptr(dc), None, None)
+    if out is None:
+        out = torch.empty(nasg_rec16_floats(N, K), dtype=f32, device=means.device)
+    _chk(out, "params", (nasg_rec16_floats(N, K),), f32, "cuda")
+    rc = _lib.nasg_rec16_pack(C.byref(inp), _ptr(out), _stream(stream))
+    if rc != 0:
+        raise NasgError(rc, "nasg_rec16_pack")
+    return out
+
+
+def nasg_rec16_eval_fwd(params, N: int, K: int, campos, vis=None, norm_mode: int = NORM_EXACT,
+                        out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    Cn = int(campos.shape[0])
+    _chk(params, "params", (nasg_rec16_floats(N, K),), torch.float32, "cuda")
+    _chk(campos, "campos", (Cn, 3), torch.float32, "cuda"); _chk(vis, "vis", (Cn, N), torch.uint8, "cuda")
+    inp = _RecInputs(N, K, Cn, _ptr(params), _ptr(campos), _ptr(vis))
+    if out is None:
+        out = torch.empty((Cn, N, 3), dtype=torch.float32, device=params.device)
+    _chk(out, "colors", (Cn, N, 3), torch.float32, "cuda")
+    rc = _lib.nasg_rec16_eval_fwd(C.byref(inp), _ptr(out), int(norm_mode), _stream(stream))
+    if rc != 0:
+        raise NasgError(rc, "nasg_rec16_eval_fwd")
+    return out
+
+
+def nasg_rec16_eval_bwd(params, N: int, K: int, campos, g_colors, vis=None, norm_mode: int = NORM_EXACT,
+                        out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    """fp32 gradient record array (layout of nasg_rec_eval_bwd: nasg_rec_floats(N, K) floats)."""
+    Cn = int(campos.shape[0])
+    _chk(params, "params", (nasg_rec16_floats(N, K),), torch.float32, "cuda"); _chk(g_colors, "g_colors", (Cn, N, 3), torch.float32, "cuda")
+    _chk(campos, "campos", (Cn, 3), torch.float32, "cuda"); _chk(vis, "vis", (Cn, N), torch.uint8, "cuda")
+    inp = _RecInputs(N, K, Cn, _ptr(params), _ptr(campos), _ptr(vis))
+    if out is None:
+        out = torch.zeros(nasg_rec_floats(N, K), dtype=torch.float32, device=params.device)
+    _chk(out, "g_params", (nasg_rec_floats(N, K),), torch.float32, "cuda")
+    rc = _lib.nasg_rec16_eval_bwd(C.byref(inp), _ptr(g_colors), _ptr(out), int(norm_mode), _stream(stream))
+    if rc != 0:
+        raise NasgError(rc, "nasg_rec16_eval_bwd")
     return out

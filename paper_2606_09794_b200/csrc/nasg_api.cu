@@ -254,6 +254,34 @@ int nasg_paper_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float 
     return rec_eval_bwd(in, g_colors, g_params, norm_mode, 1, cuda_stream);
 }
 
+// ---- bf16 parameter storage: quaternion and amplitude as bfloat16 (fp32 arithmetic, fp32 gradient records)
+size_t nasg_rec16_floats(int64_t N, int32_t K)
+{
+    if (N <= 0 || !rec_K_ok(K)) return 0;
+    return (size_t)nasg::rec_total_floats(N, K, 3);
+}
+int nasg_rec16_pack(const nasg_inputs *in, float *params, void *cuda_stream)
+{
+    if (!in) return NASG_ERR_NULL;
+    if (in->N < 0 || in->N > NASG_REC_MAX_N) return NASG_ERR_SHAPE;
+    if (!rec_K_ok(in->K)) return NASG_ERR_UNSUPPORTED_K;
+    if (in->N == 0) return NASG_OK;
+    if (!in->means || !in->quat || !in->shape || !in->amp || !in->dc || !params) return NASG_ERR_NULL;
+    if (!aligned16(in->quat) || !aligned16(in->shape) || !aligned16(params)) return NASG_ERR_ALIGN;
+    cudaError_t e = nasg::launch_rec16_pack(in->N, in->K, in->means, in->quat, in->shape, in->amp, in->dc, params, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(e);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return NASG_OK;
+}
+int nasg_rec16_eval_fwd(const nasg_rec_inputs *in, float *colors, int norm_mode, void *cuda_stream)
+{
+    return rec_eval_fwd(in, colors, norm_mode, 3, cuda_stream);
+}
+int nasg_rec16_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float *g_params, int norm_mode, void *cuda_stream)
+{
+    return rec_eval_bwd(in, g_colors, g_params, norm_mode, 3, cuda_stream);
+}
+
 // ---- isotropic Table-6 functions (Spherical Gaussian / Beta / Cauchy): 7 floats per lobe
 size_t nasg_iso_floats(int64_t N, int32_t K)
 {

@@ -67,11 +67,13 @@ bool tile_path_ok(int64_t N, int K, int C, const void *means, const void *amp, c
 cudaError_t launch_nasg_fwd_tile(const FwdParams &p, int K, int mode, cudaStream_t st);
 cudaError_t launch_nasg_bwd_tile(const BwdParams &p, int K, int mode, cudaStream_t st);
 // headline path (nasg_rec_kernels.cu): tile-record parameter layout, even K, C <= 4
-int64_t rec_total_floats(int64_t N, int K, int pk = 0);     // pk: 0 = quaternion records (11 floats per lobe), 1 = paper records (9)
+int64_t rec_total_floats(int64_t N, int K, int pk = 0);     // pk: 0 = quaternion records (11 floats per lobe), 1 = paper records (9), 2 = isotropic (7), 3 = bf16 quat/amp
 cudaError_t launch_nasg_rec_fwd(const RecFwdParams &p, int K, int mode, int pk, cudaStream_t st);
 cudaError_t launch_nasg_rec_bwd(const RecBwdParams &p, int K, int mode, int pk, cudaStream_t st);
 cudaError_t launch_rec_pack(int64_t N, int K, const float *means, const float *quat, const float *shape, const float *amp, const float *dc,
                             float *rec_out, cudaStream_t st);
+cudaError_t launch_rec16_pack(int64_t N, int K, const float *means, const float *quat, const float *shape, const float *amp, const float *dc,
+                              float *rec_out, cudaStream_t st);
 cudaError_t launch_rec_unpack(int64_t N, int K, const float *rec_in, float *means, float *quat, float *shape, float *amp, float *dc,
                               cudaStream_t st);
 cudaError_t launch_campos_reduce(const float *partial, int64_t nblocks, int C, float *out, cudaStream_t st);

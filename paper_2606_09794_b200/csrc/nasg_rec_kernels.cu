@@ -55,10 +55,14 @@ constexpr int HDR_BYTES = HDR_FLOATS * 4;       // 768
 //          (pre-activation), no phase: 9 components per lobe (3 + 9 K appearance floats)
 //      2 = an isotropic function of Table 6 (MODE = 0 Spherical Gaussian, 1 Spherical Beta, 2 Spherical
 //          Cauchy): axis (3, unnormalised) + raw shape value + amplitude: 7 components per lobe
+//      3 = kind 0 with the quaternion and the amplitude stored as bfloat16 (fp32 arithmetic):
+//          per pair 4 x 128 B (quat: one 32-bit word per lane = bf16 of lobe 2j | bf16 of lobe 2j+1 << 16), 4 x 256 B (shape,
+//          fp32 pairs), 3 x 128 B (amplitude, bf16 pairs) = 1,920 B; the header and the GRADIENT record stay fp32 (kind 0)
 template <int PK> struct Rec {
     static constexpr int NCOMP = PK == 2 ? 7 : PK == 1 ? 9 : 11;
-    static constexpr int PAIR_FLOATS = NCOMP * 2 * WT;
-    static constexpr int PAIR_BYTES = PAIR_FLOATS * 4;        // 2816 | 2304
+    static constexpr int PAIR_FLOATS = PK == 3 ? 480 : NCOMP * 2 * WT;          // 32-bit words of a pair
+    static constexpr int PAIR_BYTES = PAIR_FLOATS * 4;        // 2816 | 2304 | 1792 | 1920
+    static constexpr int GPK = PK == 3 ? 0 : PK;             // layout of the gradient record
     __host__ __device__ static constexpr int rec_floats(int K) { return HDR_FLOATS + (K / 2) * PAIR_FLOATS; }
 };
 
@@ -82,7 +86,7 @@ template <int CT, bool BWD, int PK> struct Layout {
     static constexpr int H_GC = HDR_BYTES;
     static constexpr int H_VIS = H_GC + (BWD ? CT * WT * 12 : 0);
     static constexpr int H_BYTES = H_VIS + ((CT * WT + 127) / 128) * 128;
-    static constexpr int SCRATCH = BWD ? (2 * CT + (PK == 1 ? 3 : PK == 2 ? 0 : 2)) * WT * 16 : 0;   // cam, gcm, parked frame terms (qs | trig | none)
+    static constexpr int SCRATCH = BWD ? (2 * CT + (PK == 1 ? 3 : PK == 2 ? 0 : 2)) * WT * 16 : 0;     // (PK 0 and 3: 2)   // cam, gcm, parked frame terms (qs | trig | none)
     __host__ __device__ static constexpr int region(int stages, int hslots) { return stages * PAIR_BYTES + hslots * H_BYTES + SCRATCH + 64; }
 };
 
@@ -173,18 +177,33 @@ __device__ __forceinline__ unsigned bar_hfull(const Warp &w, int h) { return w.b
 
 // the operand pairs (lobe 2j, lobe 2j+1) of this lane: 64-bit loads, conflict-free, no re-assembly
 template <int PK> struct PairRegs { f2 v[Rec<PK>::NCOMP]; };
+__device__ __forceinline__ f2 bf16x2_to_f2(unsigned w)        // (bf16 lo | bf16 hi << 16) -> packed fp32 pair: exact
+{
+    return pack(__uint_as_float(w << 16), __uint_as_float(w & 0xffff0000u));
+}
+__device__ __forceinline__ unsigned lds32u(unsigned addr) { return *reinterpret_cast<const unsigned *>(__cvta_shared_to_generic(addr)); }
 template <int PK>
 __device__ __forceinline__ void load_pair(unsigned stage, int lane, PairRegs<PK> &r)
 {
-    const unsigned a = stage + lane * 8;
+    if constexpr (PK == 3) {
+        const unsigned h = stage + lane * 4, a = stage + 512 + lane * 8;
 #pragma unroll
-    for (int c = 0; c < Rec<PK>::NCOMP; ++c) r.v[c] = lds64<f2>(a + 256 * c);
+        for (int c = 0; c < 4; ++c) r.v[c] = bf16x2_to_f2(lds32u(h + 128 * c));
+#pragma unroll
+        for (int c = 0; c < 4; ++c) r.v[4 + c] = lds64<f2>(a + 256 * c);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) r.v[8 + c] = bf16x2_to_f2(lds32u(h + 1536 + 128 * c));
+    } else {
+        const unsigned a = stage + lane * 8;
+#pragma unroll
+        for (int c = 0; c < Rec<PK>::NCOMP; ++c) r.v[c] = lds64<f2>(a + 256 * c);
+    }
 }
 // set-up of the pair from its record components; w = the (activated) amplitudes
 template <int PK, int MODE, bool GRAD>
 __device__ __forceinline__ void setup_pair(const PairRegs<PK> &r, LobePair &Lp, LobePairGrad &Gd, f2 (&park)[6], f2 &w0, f2 &w1, f2 &w2)
 {
-    if constexpr (PK == 0) {
+    if constexpr (PK == 0 || PK == 3) {
         lobe_pair_setup<MODE, GRAD>(r.v[0], r.v[1], r.v[2], r.v[3], r.v[4], r.v[5], r.v[6], r.v[7], Lp, Gd, park[0], park[1], park[2], park[3]);
         w0 = r.v[8]; w1 = r.v[9]; w2 = r.v[10];
     } else if constexpr (PK == 1) {
@@ -332,8 +351,8 @@ __global__ void __launch_bounds__(BWD_TB, NASG_REC_BWD_MINB) nasg_rec_bwd_kernel
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int S = NASG_REC_BWD_STAGES, NPAIR = K / 2;
     using L = Layout<CT, true, PK>;
-    constexpr int PAIR_BYTES = Rec<PK>::PAIR_BYTES, PAIR_FLOATS = Rec<PK>::PAIR_FLOATS;
-    constexpr int RECF = Rec<PK>::rec_floats(K), RECB = RECF * 4;
+    constexpr int PAIR_BYTES = Rec<PK>::PAIR_BYTES, RECB = Rec<PK>::rec_floats(K) * 4;
+    constexpr int GPAIR_FLOATS = Rec<Rec<PK>::GPK>::PAIR_FLOATS, GRECF = Rec<Rec<PK>::GPK>::rec_floats(K);     // gradient record
     const int lane = threadIdx.x & 31;
     const int64_t N = p.N;
     const bool bulk_rows = p.bulk_rows != 0;
@@ -359,7 +378,7 @@ __global__ void __launch_bounds__(BWD_TB, NASG_REC_BWD_MINB) nasg_rec_bwd_kernel
     for (int tile = w.tile0; tile < w.T; tile += w.tstride) {
         const int64_t n = (int64_t)tile * WT + lane;
         const bool valid = n < N;
-        float *grec = p.g_params + (int64_t)tile * RECF + lane;         // this lane's column of the gradient record
+        float *grec = p.g_params + (int64_t)tile * GRECF + lane;         // this lane's column of the gradient record
         // ---- header: directions and masked g_colors -> this lane's scratch column; g_dc; then the slot is re-armed
         mbar_wait(bar_hfull(w, 0), hpar);
         hpar ^= 1u;
@@ -470,7 +489,7 @@ __global__ void __launch_bounds__(BWD_TB, NASG_REC_BWD_MINB) nasg_rec_bwd_kernel
 #pragma unroll
                 for (int c = 0; c < Rec<PK>::NCOMP; ++c) st_cs2(gpair + 64 * c, g[c]);
             }
-            gpair += PAIR_FLOATS;
+            gpair += GPAIR_FLOATS;
         }
         if (valid) {        // through d = Delta/|Delta|: (I - d d^T)/|Delta|   (gd of a culled slot is exactly 0)
             float gm0 = 0.f, gm1 = 0.f, gm2 = 0.f;
@@ -518,6 +537,52 @@ __global__ void __launch_bounds__(256) rec_pack_kernel(int64_t N, int K, const f
         o[512] = a0; o[576] = a1; o[640] = a2;
     }
 }
+// bf16 records (kind 3): quaternion and amplitude rounded to bfloat16 (round to nearest even)
+__device__ __forceinline__ unsigned short f2bf(float x)
+{
+    unsigned u = __float_as_uint(x);
+    u += 0x7fffu + ((u >> 16) & 1u);
+    return (unsigned short)(u >> 16);
+}
+__global__ void __launch_bounds__(256) rec16_pack_kernel(int64_t N, int K, const float *means, const float *quat, const float *shape,
+                                                          const float *amp, const float *dc, unsigned *rec)
+{
+    const int64_t n = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t T = (N + WT - 1) / WT;
+    if (n >= T * WT) return;
+    const int lane = (int)(n & 31);
+    unsigned *r = rec + (n >> 5) * Rec<3>::rec_floats(K);
+    const bool valid = n < N;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        r[c * WT + lane] = __float_as_uint(valid ? means[3 * n + c] : 0.f);
+        r[(3 + c) * WT + lane] = __float_as_uint(valid ? dc[(int64_t)c * N + n] : 0.f);
+    }
+    for (int j = 0; j < K / 2; ++j) {
+        unsigned *o = r + HDR_FLOATS + j * Rec<3>::PAIR_FLOATS;
+        float4 q[2], s[2]; float a[2][3];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int l = 2 * j + h;
+            q[h] = make_float4(1.f, 0.f, 0.f, 0.f); s[h] = make_float4(0.f, 0.f, 0.f, 0.f); a[h][0] = a[h][1] = a[h][2] = 0.f;
+            if (valid) {
+                q[h] = reinterpret_cast<const float4 *>(quat)[(int64_t)l * N + n];
+                s[h] = reinterpret_cast<const float4 *>(shape)[(int64_t)l * N + n];
+                for (int ch = 0; ch < 3; ++ch) a[h][ch] = amp[((int64_t)l * 3 + ch) * N + n];
+            }
+        }
+        const float qv[2][4] = {{q[0].x, q[0].y, q[0].z, q[0].w}, {q[1].x, q[1].y, q[1].z, q[1].w}};
+        const float sv[2][4] = {{s[0].x, s[0].y, s[0].z, s[0].w}, {s[1].x, s[1].y, s[1].z, s[1].w}};
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            o[32 * c + lane] = (unsigned)f2bf(qv[0][c]) | ((unsigned)f2bf(qv[1][c]) << 16);
+            o[128 + 64 * c + 2 * lane] = __float_as_uint(sv[0][c]);
+            o[128 + 64 * c + 2 * lane + 1] = __float_as_uint(sv[1][c]);
+        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c) o[384 + 32 * c + lane] = (unsigned)f2bf(a[0][c]) | ((unsigned)f2bf(a[1][c]) << 16);
+    }
+}
 __global__ void __launch_bounds__(256) rec_unpack_kernel(int64_t N, int K, const float *rec, float *means, float *quat, float *shape,
                                                           float *amp, float *dc)
 {
@@ -547,7 +612,7 @@ namespace rec = lp::rec;
 // ---------------------------------------------------------------------------------------------
 int64_t rec_total_floats(int64_t N, int K, int pk)
 {
-    return ((N + rec::WT - 1) / rec::WT) * (int64_t)(pk == 2 ? rec::Rec<2>::rec_floats(K) : pk == 1 ? rec::Rec<1>::rec_floats(K) : rec::Rec<0>::rec_floats(K));
+    return ((N + rec::WT - 1) / rec::WT) * (int64_t)(pk == 3 ? rec::Rec<3>::rec_floats(K) : pk == 2 ? rec::Rec<2>::rec_floats(K) : pk == 1 ? rec::Rec<1>::rec_floats(K) : rec::Rec<0>::rec_floats(K));
 }
 
 template <typename Kernel>
@@ -603,7 +668,8 @@ static cudaError_t launch_rec_fwd_pk(const RecFwdParams &p, int K, int mode, cud
 }
 cudaError_t launch_nasg_rec_fwd(const RecFwdParams &p, int K, int mode, int pk, cudaStream_t st)
 {
-    return pk == 2 ? launch_rec_fwd_pk<2>(p, K, mode, st) : pk == 1 ? launch_rec_fwd_pk<1>(p, K, mode, st) : launch_rec_fwd_pk<0>(p, K, mode, st);
+    return pk == 3 ? launch_rec_fwd_pk<3>(p, K, mode, st) : pk == 2 ? launch_rec_fwd_pk<2>(p, K, mode, st)
+                   : pk == 1 ? launch_rec_fwd_pk<1>(p, K, mode, st) : launch_rec_fwd_pk<0>(p, K, mode, st);
 }
 
 template <int K, int CT, int PK>
@@ -641,7 +707,8 @@ static cudaError_t launch_rec_bwd_pk(const RecBwdParams &p, int K, int mode, cud
 }
 cudaError_t launch_nasg_rec_bwd(const RecBwdParams &p, int K, int mode, int pk, cudaStream_t st)
 {
-    return pk == 2 ? launch_rec_bwd_pk<2>(p, K, mode, st) : pk == 1 ? launch_rec_bwd_pk<1>(p, K, mode, st) : launch_rec_bwd_pk<0>(p, K, mode, st);
+    return pk == 3 ? launch_rec_bwd_pk<3>(p, K, mode, st) : pk == 2 ? launch_rec_bwd_pk<2>(p, K, mode, st)
+                   : pk == 1 ? launch_rec_bwd_pk<1>(p, K, mode, st) : launch_rec_bwd_pk<0>(p, K, mode, st);
 }
 
 cudaError_t launch_rec_pack(int64_t N, int K, const float *means, const float *quat, const float *shape, const float *amp, const float *dc,
@@ -649,6 +716,13 @@ cudaError_t launch_rec_pack(int64_t N, int K, const float *means, const float *q
 {
     const int64_t threads = ((N + rec::WT - 1) / rec::WT) * rec::WT;
     rec::rec_pack_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(N, K, means, quat, shape, amp, dc, rec_out);
+    return cudaGetLastError();
+}
+cudaError_t launch_rec16_pack(int64_t N, int K, const float *means, const float *quat, const float *shape, const float *amp, const float *dc,
+                              float *rec_out, cudaStream_t st)
+{
+    const int64_t threads = ((N + rec::WT - 1) / rec::WT) * rec::WT;
+    rec::rec16_pack_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(N, K, means, quat, shape, amp, dc, reinterpret_cast<unsigned *>(rec_out));
     return cudaGetLastError();
 }
 cudaError_t launch_rec_unpack(int64_t N, int K, const float *rec_in, float *means, float *quat, float *shape, float *amp, float *dc,

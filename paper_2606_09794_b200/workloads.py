@@ -260,3 +260,39 @@ def unpack_iso_records(rec: np.ndarray, N: int, K: int) -> dict:
     means, dc, comp = _unpack(rec, N, K, 7)
     return dict(means=means, dc=dc, axis=np.ascontiguousarray(comp[..., 0:3]), shp=np.ascontiguousarray(comp[..., 3]),
                 amp=np.ascontiguousarray(comp[..., 4:7].transpose(0, 2, 1)))
+
+
+# ---- bf16 parameter storage (include/nasg.h: nasg_rec16_*): quaternion and amplitude as bfloat16, the rest fp32 -------
+def to_bf16(a: np.ndarray) -> np.ndarray:
+    """Round an fp32 array to bfloat16 (round to nearest even) and return it as fp32: the values a bf16 record holds."""
+    u = np.ascontiguousarray(a, dtype=np.float32).view(np.uint32).astype(np.uint64)
+    u = (u + 0x7FFF + ((u >> 16) & 1)) & 0xFFFF0000
+    return u.astype(np.uint32).view(np.float32).reshape(np.shape(a))
+
+
+def rec16_words(N: int, K: int) -> int:
+    """32-bit words of a bf16 record array: header 192 words, 480 words per lobe pair (4 x 32 quat pairs, 4 x 64 shape, 3 x 32 amp pairs)."""
+    return ((N + REC_TILE - 1) // REC_TILE) * (192 + 480 * (K // 2))
+
+
+def pack_records16(means, quat, shape, amp, dc) -> np.ndarray:
+    """Tile records with bf16 quaternion / amplitude: uint32 words [T, 192 + 480 K/2]. Per pair: quat component c at words
+    [32 c + lane] = (bf16 of lobe 2j) | (bf16 of lobe 2j+1) << 16; shape component c at [128 + 64 c + 2 lane + h] (fp32);
+    amplitude c at [384 + 32 c + lane] (bf16 pair). quat and amp must already be bf16-representable (to_bf16)."""
+    K, N = quat.shape[0], quat.shape[1]
+    T = (N + REC_TILE - 1) // REC_TILE
+    Np = T * REC_TILE
+    full = pack_records(means, quat, shape, amp, dc).view(np.uint32).reshape(T, 6 + 11 * K, REC_TILE)   # fp32 records (padding: unit q)
+    out = np.empty((T, 192 + 480 * (K // 2)), dtype=np.uint32)
+    out[:, :192] = full[:, :6].reshape(T, 192)
+    pairs = full[:, 6:].reshape(T, K // 2, 11, REC_TILE, 2)
+    for j in range(K // 2):
+        base = 192 + 480 * j
+        for c in range(4):
+            w = pairs[:, j, c]
+            out[:, base + 32 * c: base + 32 * c + 32] = (w[..., 0] >> 16) | (w[..., 1] & 0xFFFF0000)
+        out[:, base + 128: base + 384] = pairs[:, j, 4:8].reshape(T, 256)
+        for c in range(3):
+            w = pairs[:, j, 8 + c]
+            out[:, base + 384 + 32 * c: base + 384 + 32 * c + 32] = (w[..., 0] >> 16) | (w[..., 1] & 0xFFFF0000)
+    return out.reshape(-1)

@@ -98,3 +98,26 @@ def check_sh(B, oracle, inp: dict, want_campos=False, label=""):
             errs[k] = rel_err(g[k], rg[k])
         _assert_errs(errs, label + " [+g_campos]")
     return col, g, errs
+
+
+def near_antipode(inp: dict, v_max: float = -0.99, lam_max: float = 4.0) -> np.ndarray:
+    """Gaussians with a visible (lobe, camera) evaluation close to d = -z of a broad lobe (d.z < v_max, lambda <= lam_max).
+    DESIGN.md R11: eq.(9) is discontinuous at d = -z (0 along the x meridian, e^{-2 lambda} along y), so next to it the
+    azimuth u/s decides the value and a relative perturbation of 6e-8 of the mean (one fp32 rounding) moves the gradients by
+    ~1e-4 of their size: no fp32 evaluation can be held to the tolerance there, the oracle's own result is that sensitive.
+    Returns a boolean [N] mask; the test that uses it reports how many Gaussians it excludes."""
+    q = np.asarray(inp["quat"], dtype=np.float64)
+    q = q / np.linalg.norm(q, axis=2, keepdims=True)
+    w, x, y, z = q[..., 0], q[..., 1], q[..., 2], q[..., 3]
+    Z = np.stack([2 * (x * z + w * y), 2 * (y * z - w * x), 1 - 2 * (x * x + y * y)], axis=2)           # [K,N,3], column 2 of R(q)
+    lam = np.exp(np.asarray(inp["shape"], dtype=np.float64)[..., 1])                                    # [K,N]
+    bad = np.zeros(q.shape[1], dtype=bool)
+    for c in range(inp["campos"].shape[0]):
+        d = np.asarray(inp["means"], dtype=np.float64) - np.asarray(inp["campos"], dtype=np.float64)[c]
+        d /= np.linalg.norm(d, axis=1, keepdims=True)
+        v = np.einsum("kni,ni->kn", Z, d)
+        hit = ((v < v_max) & (lam <= lam_max)).any(axis=0)
+        if inp.get("vis") is not None:
+            hit &= inp["vis"][c] != 0
+        bad |= hit
+    return bad

@@ -314,3 +314,82 @@ def test_cold_launches_are_correct(B, W, oracle):
         torch.cuda.synchronize()
         for gk, pk in GRADS:
             assert rel_err(g[pk], rg[gk]) <= BWD_TOL, (it, gk)
+
+
+# ---- bf16 parameter storage (nasg_rec16_*): quaternion and amplitude as bfloat16, fp32 arithmetic ----
+def _bf16_inputs(W, cfg, N):
+    inp = W.make(cfg, N)
+    return dict(inp, quat=W.to_bf16(inp["quat"]), amp=W.to_bf16(inp["amp"]))      # what the bf16 record holds, as fp32: the oracle's input
+
+
+def test_rec16_pack_rounds_to_nearest_even_and_matches_the_layout(B, W):
+    inp = W.make(2, 4_099)                                      # NOT pre-rounded: the pack kernel rounds
+    d = to_dev(inp, NASG_KEYS)
+    rec = B.nasg_rec16_pack(d["means"], d["quat"], d["shape"], d["amp"], d["dc"])
+    want = W.pack_records16(inp["means"], W.to_bf16(inp["quat"]), inp["shape"], W.to_bf16(inp["amp"]), inp["dc"])
+    assert rec.numel() == B.nasg_rec16_floats(4_099, 4) == W.rec16_words(4_099, 4) == want.size
+    assert np.array_equal(rec.cpu().numpy().view(np.uint32), want)
+    assert np.array_equal(W.to_bf16(inp["amp"]), torch.from_numpy(inp["amp"]).to(torch.bfloat16).float().numpy())
+
+
+@pytest.mark.parametrize("cfg,N,mode", [(0, None, 1), (1, 70_001, 1), (2, 50_003, 1), (2, 50_016, 0), (4, 40_007, 1), (2, 2_101, 2)])
+def test_rec16_parity(B, W, oracle, cfg, N, mode):
+    """The oracle evaluates the bf16-rounded values (promoted exactly): the arithmetic is fp32 as in nasg_rec_*, so the
+    tolerances are the same."""
+    inp = _bf16_inputs(W, cfg, N)
+    if mode == 2:
+        z = dict(inp, shape=inp["shape"].copy()); z["shape"][..., 2:] = 0.0
+        rc, rg = oracle.nasg_fwd(z, 0), oracle.nasg_bwd(z, 0)
+    else:
+        rc, rg = oracle.nasg_fwd(inp, mode), oracle.nasg_bwd(inp, mode)
+    d = to_dev(inp, NASG_KEYS)
+    N_, K = inp["N"], inp["K"]
+    params = B.nasg_rec16_pack(d["means"], d["quat"], d["shape"], d["amp"], d["dc"])
+    col = B.nasg_rec16_eval_fwd(params, N_, K, d["campos"], d["vis"], mode)
+    g = B.nasg_rec_unpack(B.nasg_rec16_eval_bwd(params, N_, K, d["campos"], d["g_colors"], d["vis"], mode), N_, K)
+    torch.cuda.synchronize()
+    assert rel_err(col, rc) <= FWD_TOL
+    for gk, pk in GRADS:
+        if mode == 2 and gk == "g_shape":
+            assert rel_err(g[pk][..., :2], rg[gk][..., :2]) <= BWD_TOL and (g[pk][..., 2:] == 0).all()
+        else:
+            assert rel_err(g[pk], rg[gk]) <= BWD_TOL, gk
+
+
+def test_rec16_full_size_every_element(B, W, oracle):
+    """cfg2 at full N on bf16-rounded quaternions / amplitudes. This input set happens to contain a Gaussian next to the
+    d = -z discontinuity of a broad lobe (R11: n = 1266176, d.z = -0.99945, lambda = 1.08, a = 116), where the
+    fp32-record kernels give the bit-identical deviation (1.3e-4 of max|g_means|): the function, not the storage format, is
+    ill-conditioned there. Gaussians with a visible evaluation at d.z < -0.999 of a lobe with lambda <= 2
+    (gpu_util.near_antipode: < 0.5 % of them) are therefore left out of the 1e-4 max-norm check, every Gaussian is held to
+    2e-4, and the whole result must equal that of the fp32-record kernels on the same values bit for bit (which
+    test_rec_full_size_every_element holds to 1e-4 everywhere on the unrounded values)."""
+    from gpu_util import near_antipode
+    inp = _bf16_inputs(W, 2, None)
+    d = to_dev(inp, NASG_KEYS)
+    N, K = inp["N"], inp["K"]
+    params = B.nasg_rec16_pack(d["means"], d["quat"], d["shape"], d["amp"], d["dc"])
+    col = B.nasg_rec16_eval_fwd(params, N, K, d["campos"], d["vis"], 1)
+    grec = B.nasg_rec16_eval_bwd(params, N, K, d["campos"], d["g_colors"], d["vis"], 1)
+    p32 = B.nasg_rec_pack(d["means"], d["quat"], d["shape"], d["amp"], d["dc"])       # the same (bf16-representable) values as fp32 records
+    assert torch.equal(col, B.nasg_rec_eval_fwd(p32, N, K, d["campos"], d["vis"], 1))
+    assert torch.equal(grec, B.nasg_rec_eval_bwd(p32, N, K, d["campos"], d["g_colors"], d["vis"], 1))
+    g = B.nasg_rec_unpack(grec, N, K)
+    torch.cuda.synchronize()
+    excl = near_antipode(inp, v_max=-0.999, lam_max=2.0)
+    assert 0 < excl.sum() < 5e-3 * N, excl.sum()
+    keep = ~excl
+    rc = oracle.nasg_fwd(inp, 1)
+    errs = {"colors": rel_err(col, rc)}
+    del rc, col
+    rg = oracle.nasg_bwd(inp, 1)
+    sl = {"g_means": (keep,), "g_quat": (slice(None), keep), "g_shape": (slice(None), keep), "g_amp": (slice(None), slice(None), keep), "g_dc": (slice(None), keep)}
+    for gk, pk in GRADS:
+        a, b = g[pk].cpu().numpy(), rg[gk]
+        errs[gk] = float(np.abs(a[sl[gk]] - b[sl[gk]]).max() / np.abs(b).max())
+        errs[gk + "(all)"] = rel_err(a, b)
+    print(f"rec16 cfg2 full N={N}, {int(excl.sum())} Gaussians near d = -z excluded:", " ".join(f"{k}={v:.2e}" for k, v in errs.items()))
+    assert errs["colors"] <= FWD_TOL
+    for gk, _ in GRADS:
+        assert errs[gk] <= BWD_TOL, (gk, errs[gk])
+        assert errs[gk + "(all)"] <= 2 * BWD_TOL, (gk, errs[gk + "(all)"])          # and even there the deviation stays small
