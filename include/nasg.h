@@ -127,6 +127,12 @@ int sh_eval_bwd(int64_t N, int32_t C, const float *means, const float *coeffs, c
  * g_colors / vis rows are moved with bulk copies when N % 4 == 0 (N % 16 == 0 with a mask) and the pointers are
  * 16-byte aligned; otherwise they are loaded per lane (correct, slower). Everything else is as above: device
  * pointers, caller-owned, asynchronous on cuda_stream, outputs overwritten, CUDA-graph capturable. */
+/* Optional hint, OR-ed into norm_mode of nasg_rec_eval_fwd / nasg_rec_eval_bwd: the visibility mask is spatially coherent
+ * (the scene is stored in spatial order, so frustum culling removes runs of consecutive Gaussians). The kernels then test per
+ * warp of 32 Gaussians which cameras ANY of them sees, skip the lobe evaluations of the others, and skip all lobe arithmetic of
+ * a tile culled in every camera (step F0). Results are identical with and without the hint; with iid masks it only costs time
+ * (~5 % of the forward), which is why it is a hint and not the default. Ignored by the other record kinds and for C = 1. */
+#define NASG_HINT_COHERENT_VIS 0x100
 #define NASG_REC_MAX_CAMERAS 4
 #define NASG_REC_MAX_N ((int64_t)1 << 35)
 

@@ -18,6 +18,7 @@ import torch
 from . import build as _build
 
 NORM_APPROX, NORM_EXACT, NORM_NASG = 0, 1, 2
+HINT_COHERENT_VIS = 0x100       # OR into norm_mode of nasg_rec_eval_fwd / bwd (include/nasg.h)
 MAX_CAMERAS = 64
 SYMBOLS = ("nasg_eval_fwd", "nasg_eval_bwd", "sh_eval_fwd", "sh_eval_bwd", "nasg_workspace_bytes",
            "nasg_host_scratch_bytes", "nasg_eval_fwd_bwd_host", "sh_host_scratch_bytes",

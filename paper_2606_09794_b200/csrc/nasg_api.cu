@@ -194,7 +194,7 @@ static int check_rec_inputs(const nasg_rec_inputs *in, int norm_mode)
     if (!in) return NASG_ERR_NULL;
     if (in->N < 0 || in->N > NASG_REC_MAX_N || in->C < 1 || in->C > NASG_REC_MAX_CAMERAS) return NASG_ERR_SHAPE;
     if (!rec_K_ok(in->K)) return NASG_ERR_UNSUPPORTED_K;
-    if (!norm_ok(norm_mode)) return NASG_ERR_NORM_MODE;
+    if (!norm_ok(norm_mode & ~NASG_HINT_COHERENT_VIS)) return NASG_ERR_NORM_MODE;
     if (in->N == 0) return NASG_OK;
     if (!in->params || !in->campos) return NASG_ERR_NULL;
     if (!aligned16(in->params)) return NASG_ERR_ALIGN;

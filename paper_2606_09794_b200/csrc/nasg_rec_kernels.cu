@@ -23,6 +23,7 @@
 // Structure (as nasg_tile_kernels.cu): persistent grid; every WARP runs its own pipeline over its tiles with bulk
 // copies (cp.async.bulk, the TMA engine) issued by one elected lane and completed on mbarriers of that warp; warps
 // never wait for each other (no __syncthreads, no atomics). Arithmetic: lobe pairs on packed f32x2 (nasg_lp_math.cuh).
+#include <type_traits>
 #include "bulk_common.cuh"
 #include "nasg_internal.h"
 #include "nasg_lp_math.cuh"
@@ -232,7 +233,9 @@ __device__ __forceinline__ void st_cs2(float *p, f2 v)
 // ---------------------------------------------------------------------------------------------
 // forward
 // ---------------------------------------------------------------------------------------------
-template <int K, int CT, int MODE, int PK>
+// SKIP (NASG_HINT_COHERENT_VIS): test per warp which cameras are seen by any lane and skip the others; a separate
+// instantiation, because the extra control flow costs the iid case ~5 % of the forward (measured), which never skips anything.
+template <int K, int CT, int MODE, int PK, bool SKIP>
 __global__ void __launch_bounds__(FWD_TB, NASG_REC_FWD_MINB) nasg_rec_fwd_kernel(RecFwdParams p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -281,6 +284,10 @@ __global__ void __launch_bounds__(FWD_TB, NASG_REC_FWD_MINB) nasg_rec_fwd_kernel
             mask = (1u << CT) - 1u;
         }
         mask = valid ? mask : 0u;
+        // cameras that SOME lane of this warp sees: with spatially coherent visibility (frustum culling of a sorted scene) whole
+        // warps lose cameras and skip their evaluations; with iid masks wmask is full and the unrolled path below runs
+        constexpr unsigned FULL = (1u << CT) - 1u;
+        const unsigned wmask = SKIP ? __reduce_or_sync(0xffffffffu, mask) : FULL;     // (every lane takes part: never under a per-lane condition)
         __syncwarp();
         if (elect_one()) hdr_issue<CT, false>(hc, w, hdr, bar_hfull(w, hslot), bulk_rows, N);
         hdr_advance<false>(hc, w.tstride, RECB);
@@ -293,41 +300,50 @@ __global__ void __launch_bounds__(FWD_TB, NASG_REC_FWD_MINB) nasg_rec_fwd_kernel
             direction(mx, my, mz, p.campos, t, dx[t], dy[t], dz[t], inv);
             col[t][0] = pack(dc0, 0.f); col[t][1] = pack(dc1, 0.f); col[t][2] = pack(dc2, 0.f);
         }
-        // ---- lobe pairs
+        // ---- lobe pairs. Two copies of the loop: ALL = every camera is seen by some lane (always with iid masks): straight-line
+        // code, the CT evaluations of a pair interleave and the next pair's wait / loads / set-up overlap them; otherwise cameras
+        // no lane sees are skipped with warp-uniform branches, and a tile culled in every camera skips all lobe arithmetic (F0).
+        auto run_pairs = [&](auto all_tag) {
+            constexpr bool ALL = decltype(all_tag)::value;
 #pragma unroll
-        for (int j = 0; j < NPAIR; ++j) {
-            const unsigned stage = w.stage0 + (unsigned)slot * PAIR_BYTES;
-            mbar_wait(bar_full(w, slot), par);
-            PairRegs<PK> r;
-            load_pair<PK>(stage, lane, r);
-            __syncwarp();
-            if (elect_one()) stage_issue<PAIR_BYTES>(sc, w.T, stage, bar_full(w, slot));
-            stage_advance<NPAIR, PAIR_BYTES>(sc, w.tstride, rec_jump);
-            if (++slot == S) { slot = 0; par ^= 1u; }
-            if constexpr (PK == 2) {           // isotropic Table-6 function MODE
-                IsoPair Ip;
-                iso_pair_setup<MODE>(r.v[0], r.v[1], r.v[2], r.v[3], Ip);
+            for (int j = 0; j < NPAIR; ++j) {
+                const unsigned stage = w.stage0 + (unsigned)slot * PAIR_BYTES;
+                mbar_wait(bar_full(w, slot), par);
+                PairRegs<PK> r;
+                load_pair<PK>(stage, lane, r);
+                __syncwarp();
+                if (elect_one()) stage_issue<PAIR_BYTES>(sc, w.T, stage, bar_full(w, slot));
+                stage_advance<NPAIR, PAIR_BYTES>(sc, w.tstride, rec_jump);
+                if (++slot == S) { slot = 0; par ^= 1u; }
+                if constexpr (PK == 2) {           // isotropic Table-6 function MODE
+                    IsoPair Ip;
+                    iso_pair_setup<MODE>(r.v[0], r.v[1], r.v[2], r.v[3], Ip);
 #pragma unroll
-                for (int t = 0; t < CT; ++t) {
-                    f2 u0, u1;
-                    const f2 G = iso_pair_eval<MODE, false>(Ip, dx[t], dy[t], dz[t], u0, u1);
-                    col[t][0] = fma2(r.v[4], G, col[t][0]);
-                    col[t][1] = fma2(r.v[5], G, col[t][1]);
-                    col[t][2] = fma2(r.v[6], G, col[t][2]);
-                }
-            } else {
-                LobePair Lp; LobePairGrad Gd; f2 park[6], w0, w1, w2;
-                setup_pair<PK, MODE, false>(r, Lp, Gd, park, w0, w1, w2);
+                    for (int t = 0; t < CT; ++t) {
+                        f2 u0, u1;
+                        const f2 G = iso_pair_eval<MODE, false>(Ip, dx[t], dy[t], dz[t], u0, u1);
+                        col[t][0] = fma2(r.v[4], G, col[t][0]);
+                        col[t][1] = fma2(r.v[5], G, col[t][1]);
+                        col[t][2] = fma2(r.v[6], G, col[t][2]);
+                    }
+                } else if (ALL || wmask != 0u) {
+                    LobePair Lp; LobePairGrad Gd; f2 park[6], w0, w1, w2;
+                    setup_pair<PK, MODE, false>(r, Lp, Gd, park, w0, w1, w2);
 #pragma unroll
-                for (int t = 0; t < CT; ++t) {     // every camera slot is evaluated (iid masks: some lane always needs it); culled slots are zeroed at the store
-                    EvalPair T;
-                    const f2 G = lobe_pair_eval<false, MODE != 2>(Lp, dx[t], dy[t], dz[t], T);
-                    col[t][0] = fma2(w0, G, col[t][0]);
-                    col[t][1] = fma2(w1, G, col[t][1]);
-                    col[t][2] = fma2(w2, G, col[t][2]);
+                    for (int t = 0; t < CT; ++t) {
+                        if (ALL || (wmask & (1u << t))) {      // culled slots of a camera some lane sees are evaluated and zeroed at the store
+                            EvalPair T;
+                            const f2 G = lobe_pair_eval<false, MODE != 2>(Lp, dx[t], dy[t], dz[t], T);
+                            col[t][0] = fma2(w0, G, col[t][0]);
+                            col[t][1] = fma2(w1, G, col[t][1]);
+                            col[t][2] = fma2(w2, G, col[t][2]);
+                        }
+                    }
                 }
             }
-        }
+        };
+        if (!SKIP || PK == 2 || wmask == FULL) run_pairs(std::true_type{});
+        else run_pairs(std::false_type{});
         if (valid) {
             float *o = p.colors + n * 3;
 #pragma unroll
@@ -345,7 +361,7 @@ __global__ void __launch_bounds__(FWD_TB, NASG_REC_FWD_MINB) nasg_rec_fwd_kernel
 // ---------------------------------------------------------------------------------------------
 // backward
 // ---------------------------------------------------------------------------------------------
-template <int K, int CT, int MODE, int PK>
+template <int K, int CT, int MODE, int PK, bool SKIP>
 __global__ void __launch_bounds__(BWD_TB, NASG_REC_BWD_MINB) nasg_rec_bwd_kernel(RecBwdParams p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -382,6 +398,7 @@ __global__ void __launch_bounds__(BWD_TB, NASG_REC_BWD_MINB) nasg_rec_bwd_kernel
         // ---- header: directions and masked g_colors -> this lane's scratch column; g_dc; then the slot is re-armed
         mbar_wait(bar_hfull(w, 0), hpar);
         hpar ^= 1u;
+        unsigned mask = 0;
         {
             const float mx = lds32(w.hdr0 + lane * 4), my = lds32(w.hdr0 + 128 + lane * 4), mz = lds32(w.hdr0 + 256 + lane * 4);
             float gdc0 = 0.f, gdc1 = 0.f, gdc2 = 0.f;
@@ -391,6 +408,7 @@ __global__ void __launch_bounds__(BWD_TB, NASG_REC_BWD_MINB) nasg_rec_bwd_kernel
                 if (p.vis) on = on && (bulk_rows ? lds8(w.hdr0 + L::H_VIS + t * WT + lane) : (valid ? (unsigned)p.vis[(int64_t)t * N + n] : 0u)) != 0;
                 float4 cam, gc = make_float4(0.f, 0.f, 0.f, 0.f);
                 direction(mx, my, mz, p.campos, t, cam.x, cam.y, cam.z, cam.w);
+                mask |= (on ? 1u : 0u) << t;
                 if (on) {       // g_colors of a culled pair is never read as a value (it may be NaN or uninitialised)
                     if (bulk_rows) {
                         const unsigned g = w.hdr0 + L::H_GC + t * WT * 12 + lane * 12;
@@ -406,6 +424,8 @@ __global__ void __launch_bounds__(BWD_TB, NASG_REC_BWD_MINB) nasg_rec_bwd_kernel
             }
             if (valid) { st_cs(grec + 96, gdc0); st_cs(grec + 128, gdc1); st_cs(grec + 160, gdc2); }
         }
+        constexpr unsigned FULL = (1u << CT) - 1u;
+        const unsigned wmask = SKIP ? __reduce_or_sync(0xffffffffu, mask) : FULL;     // (every lane takes part: never under a per-lane condition)     // cameras some lane of this warp sees
         __syncwarp();
         if (elect_one()) hdr_issue<CT, true>(hc, w, w.hdr0, bar_hfull(w, 0), bulk_rows, N);
         hdr_advance<true>(hc, w.tstride, RECB);
@@ -451,6 +471,9 @@ __global__ void __launch_bounds__(BWD_TB, NASG_REC_BWD_MINB) nasg_rec_bwd_kernel
                 g[1] = mul2(fma2(neg2(Ip.zy), dot, gzy), Ip.inv);
                 g[2] = mul2(fma2(neg2(Ip.zz), dot, gzz), Ip.inv);
                 g[3] = gs; g[4] = gw0; g[5] = gw1; g[6] = gw2;
+            } else if (SKIP && wmask == 0u) {  // (warp-uniform) a tile culled in every camera: zero gradients, no arithmetic (F0)
+#pragma unroll
+                for (int c = 0; c < Rec<PK>::NCOMP; ++c) g[c] = splat(0.f);
             } else {
                 LobePair Lp; LobePairGrad Gd;
                 f2 w0, w1, w2;
@@ -462,16 +485,24 @@ __global__ void __launch_bounds__(BWD_TB, NASG_REC_BWD_MINB) nasg_rec_bwd_kernel
                     if constexpr (PK == 1) sts64x2(scr_qs + 2 * WT * 16, park[4], park[5]);
                 }
                 AccPair A;
-#pragma unroll
-                for (int t = 0; t < CT; ++t) {
+                auto cam_bwd = [&](int t, auto first) {
                     const float4 cam = lds128(scr_cam + t * WT * 16);
                     const float4 gc = lds128(scr_gc + t * WT * 16);         // zero for a culled slot: every contribution vanishes
                     EvalPair T;
                     const f2 G = lobe_pair_eval<true, MODE != 2>(Lp, cam.x, cam.y, cam.z, T);
                     f2 gx = splat(0.f), gy = splat(0.f), gz = splat(0.f);
-                    if (t == 0) lobe_pair_bwd<MODE != 2, true>(Lp, T, G, gc.x, gc.y, gc.z, w0, w1, w2, A, gx, gy, gz);
-                    else lobe_pair_bwd<MODE != 2, false>(Lp, T, G, gc.x, gc.y, gc.z, w0, w1, w2, A, gx, gy, gz);
+                    lobe_pair_bwd<MODE != 2, decltype(first)::value>(Lp, T, G, gc.x, gc.y, gc.z, w0, w1, w2, A, gx, gy, gz);
                     gd[t][0] += lo(gx) + hi(gx); gd[t][1] += lo(gy) + hi(gy); gd[t][2] += lo(gz) + hi(gz);
+                };
+                if (!SKIP || wmask == FULL) {      // all camera slots, unrolled (the evaluations interleave); the first initialises the accumulators
+                    cam_bwd(0, std::true_type{});
+#pragma unroll
+                    for (int t = 1; t < CT; ++t) cam_bwd(t, std::false_type{});
+                } else {                           // some camera is seen by no lane of the warp: skip it (uniform branches)
+                    acc_zero(A);
+#pragma unroll
+                    for (int t = 0; t < CT; ++t)
+                        if (wmask & (1u << t)) cam_bwd(t, std::false_type{});
                 }
                 f2 park[6];
                 lds64x2(scr_qs, park[0], park[1]);
@@ -633,26 +664,28 @@ static int rec_grid(Kernel kernel, int TB, size_t smem, int64_t N, int *cached)
     return (int)(need < resident ? need : resident);
 }
 
-template <int K, int CT, int PK>
+template <int K, int CT, int PK, bool SKIP>
 static cudaError_t launch_rec_fwd_kc(const RecFwdParams &p, int mode, cudaStream_t st)
 {
     constexpr int TB = rec::FWD_TB;
     constexpr size_t smem = (size_t)(TB / 32) * rec::Layout<CT, false, PK>::region(NASG_REC_FWD_STAGES, NASG_REC_FWD_HSLOTS);
     static int cache[3][64] = {{0}};
     using namespace rec;
-    if (mode == 1) nasg_rec_fwd_kernel<K, CT, 1, PK><<<rec_grid(nasg_rec_fwd_kernel<K, CT, 1, PK>, TB, smem, p.N, cache[1]), TB, smem, st>>>(p);
-    else if (mode == 0) nasg_rec_fwd_kernel<K, CT, 0, PK><<<rec_grid(nasg_rec_fwd_kernel<K, CT, 0, PK>, TB, smem, p.N, cache[0]), TB, smem, st>>>(p);
-    else nasg_rec_fwd_kernel<K, CT, 2, PK><<<rec_grid(nasg_rec_fwd_kernel<K, CT, 2, PK>, TB, smem, p.N, cache[2]), TB, smem, st>>>(p);
+    if (mode == 1) nasg_rec_fwd_kernel<K, CT, 1, PK, SKIP><<<rec_grid(nasg_rec_fwd_kernel<K, CT, 1, PK, SKIP>, TB, smem, p.N, cache[1]), TB, smem, st>>>(p);
+    else if (mode == 0) nasg_rec_fwd_kernel<K, CT, 0, PK, SKIP><<<rec_grid(nasg_rec_fwd_kernel<K, CT, 0, PK, SKIP>, TB, smem, p.N, cache[0]), TB, smem, st>>>(p);
+    else nasg_rec_fwd_kernel<K, CT, 2, PK, SKIP><<<rec_grid(nasg_rec_fwd_kernel<K, CT, 2, PK, SKIP>, TB, smem, p.N, cache[2]), TB, smem, st>>>(p);
     return cudaGetLastError();
 }
 template <int K, int PK>
-static cudaError_t launch_rec_fwd_k(const RecFwdParams &p, int mode, cudaStream_t st)
+static cudaError_t launch_rec_fwd_k(const RecFwdParams &p, int mode_and_hint, cudaStream_t st)
 {
+    const int mode = mode_and_hint & 0xff;
+    const bool skip = (mode_and_hint & 0x100) != 0;           // NASG_HINT_COHERENT_VIS (quaternion records with C > 1 only)
     switch (p.C) {
-    case 1: return launch_rec_fwd_kc<K, 1, PK>(p, mode, st);
-    case 2: return launch_rec_fwd_kc<K, 2, PK>(p, mode, st);
-    case 3: return launch_rec_fwd_kc<K, 3, PK>(p, mode, st);
-    case 4: return launch_rec_fwd_kc<K, 4, PK>(p, mode, st);
+    case 1: return (PK == 0 && 1 > 1 && skip) ? launch_rec_fwd_kc<K, 1, PK, PK == 0 && (1 > 1)>(p, mode, st) : launch_rec_fwd_kc<K, 1, PK, false>(p, mode, st);
+    case 2: return (PK == 0 && 2 > 1 && skip) ? launch_rec_fwd_kc<K, 2, PK, PK == 0 && (2 > 1)>(p, mode, st) : launch_rec_fwd_kc<K, 2, PK, false>(p, mode, st);
+    case 3: return (PK == 0 && 3 > 1 && skip) ? launch_rec_fwd_kc<K, 3, PK, PK == 0 && (3 > 1)>(p, mode, st) : launch_rec_fwd_kc<K, 3, PK, false>(p, mode, st);
+    case 4: return (PK == 0 && 4 > 1 && skip) ? launch_rec_fwd_kc<K, 4, PK, PK == 0 && (4 > 1)>(p, mode, st) : launch_rec_fwd_kc<K, 4, PK, false>(p, mode, st);
     default: return cudaErrorInvalidValue;
     }
 }
@@ -672,26 +705,28 @@ cudaError_t launch_nasg_rec_fwd(const RecFwdParams &p, int K, int mode, int pk, 
                    : pk == 1 ? launch_rec_fwd_pk<1>(p, K, mode, st) : launch_rec_fwd_pk<0>(p, K, mode, st);
 }
 
-template <int K, int CT, int PK>
+template <int K, int CT, int PK, bool SKIP>
 static cudaError_t launch_rec_bwd_kc(const RecBwdParams &p, int mode, cudaStream_t st)
 {
     constexpr int TB = rec::BWD_TB;
     constexpr size_t smem = (size_t)(TB / 32) * rec::Layout<CT, true, PK>::region(NASG_REC_BWD_STAGES, 1);
     static int cache[3][64] = {{0}};
     using namespace rec;
-    if (mode == 1) nasg_rec_bwd_kernel<K, CT, 1, PK><<<rec_grid(nasg_rec_bwd_kernel<K, CT, 1, PK>, TB, smem, p.N, cache[1]), TB, smem, st>>>(p);
-    else if (mode == 0) nasg_rec_bwd_kernel<K, CT, 0, PK><<<rec_grid(nasg_rec_bwd_kernel<K, CT, 0, PK>, TB, smem, p.N, cache[0]), TB, smem, st>>>(p);
-    else nasg_rec_bwd_kernel<K, CT, 2, PK><<<rec_grid(nasg_rec_bwd_kernel<K, CT, 2, PK>, TB, smem, p.N, cache[2]), TB, smem, st>>>(p);
+    if (mode == 1) nasg_rec_bwd_kernel<K, CT, 1, PK, SKIP><<<rec_grid(nasg_rec_bwd_kernel<K, CT, 1, PK, SKIP>, TB, smem, p.N, cache[1]), TB, smem, st>>>(p);
+    else if (mode == 0) nasg_rec_bwd_kernel<K, CT, 0, PK, SKIP><<<rec_grid(nasg_rec_bwd_kernel<K, CT, 0, PK, SKIP>, TB, smem, p.N, cache[0]), TB, smem, st>>>(p);
+    else nasg_rec_bwd_kernel<K, CT, 2, PK, SKIP><<<rec_grid(nasg_rec_bwd_kernel<K, CT, 2, PK, SKIP>, TB, smem, p.N, cache[2]), TB, smem, st>>>(p);
     return cudaGetLastError();
 }
 template <int K, int PK>
-static cudaError_t launch_rec_bwd_k(const RecBwdParams &p, int mode, cudaStream_t st)
+static cudaError_t launch_rec_bwd_k(const RecBwdParams &p, int mode_and_hint, cudaStream_t st)
 {
+    const int mode = mode_and_hint & 0xff;
+    const bool skip = (mode_and_hint & 0x100) != 0;           // NASG_HINT_COHERENT_VIS (quaternion records with C > 1 only)
     switch (p.C) {
-    case 1: return launch_rec_bwd_kc<K, 1, PK>(p, mode, st);
-    case 2: return launch_rec_bwd_kc<K, 2, PK>(p, mode, st);
-    case 3: return launch_rec_bwd_kc<K, 3, PK>(p, mode, st);
-    case 4: return launch_rec_bwd_kc<K, 4, PK>(p, mode, st);
+    case 1: return (PK == 0 && 1 > 1 && skip) ? launch_rec_bwd_kc<K, 1, PK, PK == 0 && (1 > 1)>(p, mode, st) : launch_rec_bwd_kc<K, 1, PK, false>(p, mode, st);
+    case 2: return (PK == 0 && 2 > 1 && skip) ? launch_rec_bwd_kc<K, 2, PK, PK == 0 && (2 > 1)>(p, mode, st) : launch_rec_bwd_kc<K, 2, PK, false>(p, mode, st);
+    case 3: return (PK == 0 && 3 > 1 && skip) ? launch_rec_bwd_kc<K, 3, PK, PK == 0 && (3 > 1)>(p, mode, st) : launch_rec_bwd_kc<K, 3, PK, false>(p, mode, st);
+    case 4: return (PK == 0 && 4 > 1 && skip) ? launch_rec_bwd_kc<K, 4, PK, PK == 0 && (4 > 1)>(p, mode, st) : launch_rec_bwd_kc<K, 4, PK, false>(p, mode, st);
     default: return cudaErrorInvalidValue;
     }
 }

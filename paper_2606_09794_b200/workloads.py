@@ -54,8 +54,11 @@ def _rng(seed: int, tag: int) -> np.random.Generator:
     return np.random.Generator(np.random.PCG64([seed, tag]))
 
 
-def make_geometry(cfg: Config, N: Optional[int] = None) -> dict:
-    """means, campos, vis, g_colors: the arrays config 3 shares with config 2 (same seed/tags)."""
+def make_geometry(cfg: Config, N: Optional[int] = None, vis_cluster: int = 1) -> dict:
+    """means, campos, vis, g_colors: the arrays config 3 shares with config 2 (same seed/tags). vis_cluster > 1: the
+    Bernoulli draw is per (camera, run of vis_cluster consecutive Gaussians) instead of per (camera, Gaussian): the
+    spatially coherent visibility of a scene stored in spatial order, where frustum culling removes whole runs (a labelled
+    variant; the BASELINE configs use vis_cluster = 1, iid, the pessimistic case)."""
     N = cfg.N if N is None else int(N)
     C = cfg.C
     means = _rng(cfg.seed, TAG_MEANS).uniform(-1.0, 1.0, size=(N, 3)).astype(np.float32)
@@ -67,15 +70,20 @@ def make_geometry(cfg: Config, N: Optional[int] = None) -> dict:
     if cfg.vis_p is None:
         vis = None
     else:
-        vis = (_rng(cfg.seed, TAG_VIS).random(size=(C, N)) < cfg.vis_p).astype(np.uint8)
+        if vis_cluster > 1:
+            runs = (N + vis_cluster - 1) // vis_cluster
+            vis = np.repeat((_rng(cfg.seed, TAG_VIS).random(size=(C, runs)) < cfg.vis_p).astype(np.uint8), vis_cluster, axis=1)[:, :N]
+            vis = np.ascontiguousarray(vis)
+        else:
+            vis = (_rng(cfg.seed, TAG_VIS).random(size=(C, N)) < cfg.vis_p).astype(np.uint8)
     g_colors = _rng(cfg.seed, TAG_GCOL).standard_normal(size=(C, N, 3)).astype(np.float32)
     return dict(N=N, C=C, means=means, campos=campos, vis=vis, g_colors=g_colors)
 
 
-def make_nasg(cfg: Config, N: Optional[int] = None) -> dict:
+def make_nasg(cfg: Config, N: Optional[int] = None, vis_cluster: int = 1) -> dict:
     """Inputs of nasg_eval_fwd/bwd for a NASGabor config."""
     assert cfg.kind == "nasg"
-    out = make_geometry(cfg, N)
+    out = make_geometry(cfg, N, vis_cluster)
     N, K = out["N"], cfg.K
     q = _rng(cfg.seed, TAG_QUAT).standard_normal(size=(K, N, 4))
     q /= np.linalg.norm(q, axis=2, keepdims=True)

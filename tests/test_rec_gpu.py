@@ -40,7 +40,7 @@ def run_rec(B, d, N, K, mode=1):
 def check_rec(B, oracle, inp, mode=1, label=""):
     d = to_dev(inp, NASG_KEYS)
     col, g, _, _ = run_rec(B, d, inp["N"], inp["K"], mode)
-    rc, rg = oracle.nasg_fwd(inp, mode), oracle.nasg_bwd(inp, mode)
+    rc, rg = oracle.nasg_fwd(inp, mode & 0xff), oracle.nasg_bwd(inp, mode & 0xff)
     errs = {"colors": rel_err(col, rc)}
     for gk, pk in GRADS:
         errs[gk] = rel_err(g[pk], rg[gk])
@@ -393,3 +393,17 @@ def test_rec16_full_size_every_element(B, W, oracle):
     for gk, _ in GRADS:
         assert errs[gk] <= BWD_TOL, (gk, errs[gk])
         assert errs[gk + "(all)"] <= 2 * BWD_TOL, (gk, errs[gk + "(all)"])          # and even there the deviation stays small
+
+
+@pytest.mark.parametrize("cluster,N", [(32, 20_011), (256, 50_016), (1024, 50_003)])
+def test_rec_clustered_visibility_skips_cameras_and_tiles(B, W, oracle, cluster, N):
+    """Spatially coherent masks: warps that see a camera in no lane skip its evaluations, tiles culled in every camera skip
+    all lobe arithmetic (step F0) and write zero colours / zero gradients; results equal the oracle's as with iid masks."""
+    inp = W.make_nasg(W.CONFIGS[2], N, vis_cluster=cluster)
+    assert (inp["vis"].reshape(4, -1)[:, :cluster] == inp["vis"][:, :1]).all()
+    col0, g0 = check_rec(B, oracle, inp, 1, label=f"rec clustered({cluster}) N={N}, no hint")
+    col, g = check_rec(B, oracle, inp, 1 | B.HINT_COHERENT_VIS, label=f"rec clustered({cluster}) N={N}, NASG_HINT_COHERENT_VIS")
+    assert torch.equal(col, col0) and all(torch.equal(g[k], g0[k]) for k in g)          # the hint changes time, not results
+    dead = ~(inp["vis"] != 0).any(0)
+    assert dead.sum() > 0
+    assert (col.cpu().numpy()[:, dead] == 0).all() and (g["quat"].cpu().numpy()[:, dead] == 0).all() and (g["means"].cpu().numpy()[dead] == 0).all()
