@@ -15,7 +15,8 @@ from typing import Optional
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SRC = [os.path.join(_HERE, "nasg_ref.c"), os.path.join(_HERE, "sh_ref.c"), os.path.join(_HERE, "iso_ref.c")]
+_SRC = [os.path.join(_HERE, "nasg_ref.c"), os.path.join(_HERE, "sh_ref.c"), os.path.join(_HERE, "iso_ref.c"),
+        os.path.join(_HERE, "asg_ref.c")]
 _LIB = os.path.join(_HERE, "liboracle_ref.so")
 _lib = None
 
@@ -53,6 +54,10 @@ def lib():
         L.iso_ref_bwd.argtypes = [i64, i32, i32, i32, dp, dp, dp, dp, dp, dp, u8p, dp, dp, dp, dp, dp, dp]
         L.iso_ref_fwd.restype = i32
         L.iso_ref_bwd.restype = i32
+        L.asg_ref_frame.argtypes = [dp, dp, dp, dp]
+        L.asg_ref_lobe.argtypes = [dbl, dbl, dbl, dbl, dbl, dp]
+        L.asg_ref_fwd.argtypes = [i64, i32, i32, dp, dp, dp, dp, dp, dp, u8p, dp]
+        L.asg_ref_bwd.argtypes = [i64, i32, i32, dp, dp, dp, dp, dp, dp, u8p, dp, dp, dp, dp, dp, dp]
         L.nasg_ref_paper_frame.argtypes = [dp, dp, dp, dp, dp]
         L.nasg_ref_paper_fwd.argtypes = [i64, i32, i32, dp, dp, dp, dp, dp, dp, u8p, i32, dp]
         L.nasg_ref_paper_bwd.argtypes = [i64, i32, i32, dp, dp, dp, dp, dp, dp, u8p, dp, i32, dp, dp, dp, dp, dp]
@@ -234,5 +239,44 @@ def iso_bwd(inp: dict, kind: int, g_colors: Optional[np.ndarray] = None) -> dict
     out = dict(g_means=np.empty((N, 3)), g_axis=np.empty((K, N, 3)), g_shp=np.empty((K, N)), g_amp=np.empty((K, 3, N)), g_dc=np.empty((3, N)))
     rc = lib().iso_ref_bwd(N, K, Cn, int(kind), _p(means), _p(ax), _p(sp), _p(am), _p(dc), _p(campos), _p(vis), _p(gcol),
                            _p(out["g_means"]), _p(out["g_axis"]), _p(out["g_shp"]), _p(out["g_amp"]), _p(out["g_dc"]))
+    assert rc == 0
+    return out
+
+
+# ---- Anisotropic Spherical Gaussian of Table 6 (oracle/asg_ref.c)
+def asg_frame(q) -> tuple:
+    """Columns (x, y, z) of R(q/|q|), q = (w,x,y,z)."""
+    q = _d(np.asarray(q, dtype=np.float64))
+    X, Y, Z = np.empty(3), np.empty(3), np.empty(3)
+    lib().asg_ref_frame(_p(q), _p(X), _p(Y), _p(Z))
+    return X, Y, Z
+
+
+def asg_lobe(u: float, t: float, v: float, raw_mu: float, raw_lam: float) -> np.ndarray:
+    """[G, G_u, G_t, G_v, G_rawmu, G_rawlambda] at (u, t, v) = (d.x, d.y, d.z)."""
+    out = np.empty(6)
+    lib().asg_ref_lobe(float(u), float(t), float(v), float(raw_mu), float(raw_lam), _p(out))
+    return out
+
+
+def asg_fwd(inp: dict) -> np.ndarray:
+    """colors [C,N,3] fp64; inp holds means, quat [K,N,4], shp [K,N,2] (raw mu, raw lambda), amp [K,3,N], dc, campos, vis."""
+    N, K, Cn = int(inp["N"]), int(inp["K"]), int(inp["C"])
+    means, qu, sp, am, dc, campos = (_d(inp[k]) for k in ("means", "quat", "shp", "amp", "dc", "campos"))
+    vis = None if inp.get("vis") is None else np.ascontiguousarray(inp["vis"], dtype=np.uint8)
+    colors = np.empty((Cn, N, 3), dtype=np.float64)
+    rc = lib().asg_ref_fwd(N, K, Cn, _p(means), _p(qu), _p(sp), _p(am), _p(dc), _p(campos), _p(vis), _p(colors))
+    assert rc == 0
+    return colors
+
+
+def asg_bwd(inp: dict, g_colors: Optional[np.ndarray] = None) -> dict:
+    N, K, Cn = int(inp["N"]), int(inp["K"]), int(inp["C"])
+    means, qu, sp, am, dc, campos = (_d(inp[k]) for k in ("means", "quat", "shp", "amp", "dc", "campos"))
+    gcol = _d(inp["g_colors"] if g_colors is None else g_colors)
+    vis = None if inp.get("vis") is None else np.ascontiguousarray(inp["vis"], dtype=np.uint8)
+    out = dict(g_means=np.empty((N, 3)), g_quat=np.empty((K, N, 4)), g_shp=np.empty((K, N, 2)), g_amp=np.empty((K, 3, N)), g_dc=np.empty((3, N)))
+    rc = lib().asg_ref_bwd(N, K, Cn, _p(means), _p(qu), _p(sp), _p(am), _p(dc), _p(campos), _p(vis), _p(gcol),
+                           _p(out["g_means"]), _p(out["g_quat"]), _p(out["g_shp"]), _p(out["g_amp"]), _p(out["g_dc"]))
     assert rc == 0
     return out
