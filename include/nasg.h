@@ -205,6 +205,17 @@ size_t nasg_iso_floats(int64_t N, int32_t K);
 int nasg_iso_eval_fwd(const nasg_rec_inputs *in, float *colors, int kind, void *cuda_stream);
 int nasg_iso_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float *g_params, int kind, void *cuda_stream);
 
+/* Anisotropic Spherical Gaussian (Table 6, [XSD*13]), not normalised (Table 6: "Not analytical"):
+ *     G(d) = max(d.z, 0) exp{-mu (d.x)^2 - lambda (d.y)^2},   [x y z] = R(q/|q|) (Hamilton (w,x,y,z), as nasg_inputs.quat),
+ *     mu = e^raw0, lambda = e^raw1;   colour = c0 + sum_l w_l G_l(d) (eq.(6)).
+ * At d.z = 0 the lobe has a kink; the derivative there is taken as 0 (the far side). Tile records with 9 components per lobe:
+ *     [192 + 576 j + 64 c + 2 lane + h],  c = 0..3 quaternion (w,x,y,z) | 4 raw mu | 5 raw lambda | 6..8 amplitude (r,g,b);
+ *     [T][6 + 9 K][32] floats = nasg_asg_floats(N, K); the gradient record has the same layout (dL/dq through the
+ * normalisation, dL/draw, dL/dw). Same restrictions and conventions as nasg_rec_eval_* (no norm_mode). */
+size_t nasg_asg_floats(int64_t N, int32_t K);
+int nasg_asg_eval_fwd(const nasg_rec_inputs *in, float *colors, void *cuda_stream);
+int nasg_asg_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float *g_params, void *cuda_stream);
+
 /* End-to-end with HOST buffers, as nasg_eval_fwd_bwd_host below: params / g_params are HOST record arrays, campos, vis,
  * g_colors, colors HOST arrays. A chunk of Gaussians is a contiguous block of records, so each chunk moves with one
  * copy per direction for the parameters / gradients plus one strided copy each for vis, g_colors and colors. Padding

@@ -27,6 +27,7 @@ SYMBOLS = ("nasg_eval_fwd", "nasg_eval_bwd", "sh_eval_fwd", "sh_eval_bwd", "nasg
            "nasg_rec_host_scratch_bytes", "nasg_rec_eval_fwd_bwd_host", "nasg_paper_floats", "nasg_paper_eval_fwd",
            "nasg_paper_eval_bwd", "nasg_paper_host_scratch_bytes", "nasg_paper_eval_fwd_bwd_host",
            "nasg_iso_floats", "nasg_iso_eval_fwd", "nasg_iso_eval_bwd",
+           "nasg_asg_floats", "nasg_asg_eval_fwd", "nasg_asg_eval_bwd",
            "nasg_rec16_floats", "nasg_rec16_pack", "nasg_rec16_eval_fwd", "nasg_rec16_eval_bwd")
 
 
@@ -101,6 +102,10 @@ def _load():
     lib.nasg_iso_floats.restype = sz
     lib.nasg_iso_eval_fwd.argtypes = [C.POINTER(_RecInputs), vp, C.c_int, vp]
     lib.nasg_iso_eval_bwd.argtypes = [C.POINTER(_RecInputs), vp, vp, C.c_int, vp]
+    lib.nasg_asg_floats.argtypes = [i64, i32]
+    lib.nasg_asg_floats.restype = sz
+    lib.nasg_asg_eval_fwd.argtypes = [C.POINTER(_RecInputs), vp, vp]
+    lib.nasg_asg_eval_bwd.argtypes = [C.POINTER(_RecInputs), vp, vp, vp]
     lib.nasg_paper_floats.argtypes = [i64, i32]
     lib.nasg_paper_floats.restype = sz
     lib.nasg_paper_eval_fwd.argtypes = [C.POINTER(_RecInputs), vp, C.c_int, vp]
@@ -114,7 +119,7 @@ def _load():
     for name in ("nasg_eval_fwd", "nasg_eval_bwd", "sh_eval_fwd", "sh_eval_bwd", "nasg_eval_fwd_bwd_host",
                  "sh_eval_fwd_bwd_host", "nasg_rec_pack", "nasg_rec_unpack", "nasg_rec_eval_fwd", "nasg_rec_eval_bwd",
                  "nasg_rec_eval_fwd_bwd_host", "nasg_paper_eval_fwd", "nasg_paper_eval_bwd", "nasg_paper_eval_fwd_bwd_host",
-                 "nasg_iso_eval_fwd", "nasg_iso_eval_bwd", "nasg_rec16_pack", "nasg_rec16_eval_fwd", "nasg_rec16_eval_bwd"):
+                 "nasg_iso_eval_fwd", "nasg_iso_eval_bwd", "nasg_asg_eval_fwd", "nasg_asg_eval_bwd", "nasg_rec16_pack", "nasg_rec16_eval_fwd", "nasg_rec16_eval_bwd"):
         getattr(lib, name).restype = C.c_int
     return lib
 
@@ -473,6 +478,40 @@ def nasg_iso_eval_bwd(params, N: int, K: int, campos, g_colors, kind: int, vis=N
     rc = _lib.nasg_iso_eval_bwd(C.byref(inp), _ptr(g_colors), _ptr(out), int(kind), _stream(stream))
     if rc != 0:
         raise NasgError(rc, "nasg_iso_eval_bwd")
+    return out
+
+
+# ---- Anisotropic Spherical Gaussian of Table 6 (include/nasg.h: nasg_asg_*) -------------------------
+def nasg_asg_floats(N: int, K: int) -> int:
+    return int(_lib.nasg_asg_floats(N, K))
+
+
+def nasg_asg_eval_fwd(params, N: int, K: int, campos, vis=None, out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    Cn = int(campos.shape[0])
+    _chk(params, "params", (nasg_asg_floats(N, K),), torch.float32, "cuda")
+    _chk(campos, "campos", (Cn, 3), torch.float32, "cuda"); _chk(vis, "vis", (Cn, N), torch.uint8, "cuda")
+    inp = _RecInputs(N, K, Cn, _ptr(params), _ptr(campos), _ptr(vis))
+    if out is None:
+        out = torch.empty((Cn, N, 3), dtype=torch.float32, device=params.device)
+    _chk(out, "colors", (Cn, N, 3), torch.float32, "cuda")
+    rc = _lib.nasg_asg_eval_fwd(C.byref(inp), _ptr(out), _stream(stream))
+    if rc != 0:
+        raise NasgError(rc, "nasg_asg_eval_fwd")
+    return out
+
+
+def nasg_asg_eval_bwd(params, N: int, K: int, campos, g_colors, vis=None, out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    Cn = int(campos.shape[0])
+    nf = nasg_asg_floats(N, K)
+    _chk(params, "params", (nf,), torch.float32, "cuda"); _chk(g_colors, "g_colors", (Cn, N, 3), torch.float32, "cuda")
+    _chk(campos, "campos", (Cn, 3), torch.float32, "cuda"); _chk(vis, "vis", (Cn, N), torch.uint8, "cuda")
+    inp = _RecInputs(N, K, Cn, _ptr(params), _ptr(campos), _ptr(vis))
+    if out is None:
+        out = torch.zeros(nf, dtype=torch.float32, device=params.device)
+    _chk(out, "g_params", (nf,), torch.float32, "cuda")
+    rc = _lib.nasg_asg_eval_bwd(C.byref(inp), _ptr(g_colors), _ptr(out), _stream(stream))
+    if rc != 0:
+        raise NasgError(rc, "nasg_asg_eval_bwd")
     return out
 
 

@@ -297,6 +297,21 @@ int nasg_iso_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float *g
     return rec_eval_bwd(in, g_colors, g_params, kind, 2, cuda_stream);
 }
 
+// ---- Anisotropic Spherical Gaussian of Table 6: 9 floats per lobe
+size_t nasg_asg_floats(int64_t N, int32_t K)
+{
+    if (N <= 0 || !rec_K_ok(K)) return 0;
+    return (size_t)nasg::rec_total_floats(N, K, 4);
+}
+int nasg_asg_eval_fwd(const nasg_rec_inputs *in, float *colors, void *cuda_stream)
+{
+    return rec_eval_fwd(in, colors, 0, 4, cuda_stream);
+}
+int nasg_asg_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float *g_params, void *cuda_stream)
+{
+    return rec_eval_bwd(in, g_colors, g_params, 0, 4, cuda_stream);
+}
+
 size_t nasg_workspace_bytes(int64_t N, int32_t K, int32_t C)
 {
     (void)K;

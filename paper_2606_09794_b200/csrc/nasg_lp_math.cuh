@@ -377,6 +377,92 @@ NASG_HD f2 iso_pair_eval(const IsoPair &P, float dx, float dy, float dz, f2 &Fv,
 }
 
 // ---------------------------------------------------------------------------------------------
+// Anisotropic Spherical Gaussian of the paper's Table 6 ([XSD*13]; include/nasg.h: nasg_asg_*):
+//   G = max(d.z, 0) exp{-mu (d.x)^2 - lambda (d.y)^2},  [x y z] = R(q/|q|),  mu = e^raw0, lambda = e^raw1, no normaliser.
+// Nothing cancels here (the exponent is a sum of squares of plain dot products), so the arithmetic is the direct one.
+// The frame gradient is accumulated as a rotation vector in the lobe frame like the NASGabor backward's:
+// with p = (u, t, v) the direction in the lobe frame and g = dL/dp, g_theta = g x p, then g_q = qs (x) (0, g_theta).
+// ---------------------------------------------------------------------------------------------
+struct AsgPair {
+    f2 Xx, Xy, Xz, Yx, Yy, Yz, Zx, Zy, Zz;   // columns of R(q/|q|)
+    f2 mu, lam;                               // bandwidths
+};
+struct AsgEval { f2 u, t, v, uu, tt, S; };    // what the backward needs from the recomputed forward
+struct AsgAcc { f2 gw0, gw1, gw2, Sm, Sl, th0, th1, th2; };
+// qs (GRAD only) = qhat * 2/|q|
+template <bool GRAD>
+NASG_HD void asg_pair_setup(f2 w, f2 x, f2 y, f2 z, f2 raw_mu, f2 raw_lam, AsgPair &P, f2 &qsw, f2 &qsx, f2 &qsy, f2 &qsz)
+{
+    const f2 qq = fma2(w, w, fma2(x, x, fma2(y, y, mul2(z, z))));
+    f2 inv = rsqrt2(qq);
+    inv = mul2(inv, fma2(scl2(qq, -0.5f), mul2(inv, inv), splat(1.5f)));   // one Newton step
+    w = mul2(w, inv); x = mul2(x, inv); y = mul2(y, inv); z = mul2(z, inv);
+    const f2 x2 = add2(x, x), y2 = add2(y, y), z2 = add2(z, z);
+    const f2 one = splat(1.0f);
+    P.Xx = sub2(one, fma2(y2, y, mul2(z2, z))); P.Xy = fma2(x2, y, mul2(z2, w)); P.Xz = fma2(x2, z, neg2(mul2(y2, w)));
+    P.Yx = fma2(x2, y, neg2(mul2(z2, w))); P.Yy = sub2(one, fma2(x2, x, mul2(z2, z))); P.Yz = fma2(y2, z, mul2(x2, w));
+    P.Zx = fma2(x2, z, mul2(y2, w)); P.Zy = fma2(y2, z, neg2(mul2(x2, w))); P.Zz = sub2(one, fma2(x2, x, mul2(y2, y)));
+    if (GRAD) {
+        const f2 i2 = add2(inv, inv);
+        qsw = mul2(w, i2); qsx = mul2(x, i2); qsy = mul2(y, i2); qsz = mul2(z, i2);
+    }
+    P.mu = ex2_2(scl2(raw_mu, LOG2E));
+    P.lam = ex2_2(scl2(raw_lam, LOG2E));
+}
+template <bool FULL>
+NASG_HD f2 asg_pair_eval(const AsgPair &P, float dx, float dy, float dz, AsgEval &T)
+{
+    const f2 ddx = splat(dx), ddy = splat(dy), ddz = splat(dz);
+    const f2 u = fma2(P.Xx, ddx, fma2(P.Xy, ddy, mul2(P.Xz, ddz)));
+    const f2 t = fma2(P.Yx, ddx, fma2(P.Yy, ddy, mul2(P.Yz, ddz)));
+    const f2 v = fma2(P.Zx, ddx, fma2(P.Zy, ddy, mul2(P.Zz, ddz)));
+    const f2 uu = mul2(u, u), tt = mul2(t, t);
+    const f2 S = ex2_2(scl2(fma2(P.mu, uu, mul2(P.lam, tt)), -LOG2E));
+    if (FULL) { T.u = u; T.t = t; T.v = v; T.uu = uu; T.tt = tt; T.S = S; }
+    return mul2(max2(v, 0.0f), S);
+}
+// Backward of one (lobe pair, camera); FIRST initialises the accumulators. Returns the pair's dL/dd in gdx, gdy, gdz.
+template <bool FIRST>
+NASG_HD void asg_pair_bwd(const AsgPair &P, const AsgEval &T, f2 G, float gc0, float gc1, float gc2, f2 w0, f2 w1, f2 w2,
+                          AsgAcc &A, f2 &gdx, f2 &gdy, f2 &gdz)
+{
+    const f2 c0 = splat(gc0), c1 = splat(gc1), c2 = splat(gc2);
+    const f2 gG = fma2(w0, c0, fma2(w1, c1, mul2(w2, c2)));                 // dL/dG, eq.(6)
+    const f2 gGG = mul2(gG, G);
+    const f2 m2 = scl2(gGG, -2.0f);
+    const f2 gu = mul2(mul2(m2, P.mu), T.u);                                // gG dG/du = -2 mu u G
+    const f2 gt = mul2(mul2(m2, P.lam), T.t);                               // gG dG/dt = -2 lambda t G
+    const f2 gS = mul2(gG, T.S);
+    const f2 gv = pack(lo(T.v) > 0.0f ? lo(gS) : 0.0f, hi(T.v) > 0.0f ? hi(gS) : 0.0f);   // gG dG/dv = S on the lobe side, 0 beyond the kink
+    if (FIRST) {
+        A.gw0 = mul2(G, c0); A.gw1 = mul2(G, c1); A.gw2 = mul2(G, c2);
+        A.Sm = mul2(gGG, T.uu); A.Sl = mul2(gGG, T.tt);
+        A.th0 = fma2(gt, T.v, mul2(neg2(gv), T.t));
+        A.th1 = fma2(gv, T.u, mul2(neg2(gu), T.v));
+        A.th2 = fma2(gu, T.t, mul2(neg2(gt), T.u));
+    } else {
+        A.gw0 = fma2(G, c0, A.gw0); A.gw1 = fma2(G, c1, A.gw1); A.gw2 = fma2(G, c2, A.gw2);
+        A.Sm = fma2(gGG, T.uu, A.Sm); A.Sl = fma2(gGG, T.tt, A.Sl);
+        A.th0 = fma2(gt, T.v, fma2(neg2(gv), T.t, A.th0));                  // g_theta = g x p, p = (u, t, v)
+        A.th1 = fma2(gv, T.u, fma2(neg2(gu), T.v, A.th1));
+        A.th2 = fma2(gu, T.t, fma2(neg2(gt), T.u, A.th2));
+    }
+    gdx = fma2(gu, P.Xx, fma2(gt, P.Yx, fma2(gv, P.Zx, gdx)));
+    gdy = fma2(gu, P.Xy, fma2(gt, P.Yy, fma2(gv, P.Zy, gdy)));
+    gdz = fma2(gu, P.Xz, fma2(gt, P.Yz, fma2(gv, P.Zz, gdz)));
+}
+// gradients of the raw bandwidths and of the (unnormalised) quaternion: (w, v) (x) (0, t) = ( -v.t ,  w t + v cross t )
+NASG_HD void asg_pair_finish(const AsgPair &P, const AsgAcc &A, f2 qw, f2 qx, f2 qy, f2 qz, f2 &gmu, f2 &glam, f2 &gqw, f2 &gqx, f2 &gqy, f2 &gqz)
+{
+    gmu = mul2(neg2(P.mu), A.Sm);                                           // d/draw = mu d/dmu
+    glam = mul2(neg2(P.lam), A.Sl);
+    gqw = neg2(fma2(qx, A.th0, fma2(qy, A.th1, mul2(qz, A.th2))));
+    gqx = fma2(qw, A.th0, fma2(qy, A.th2, mul2(neg2(qz), A.th1)));
+    gqy = fma2(qw, A.th1, fma2(qz, A.th0, mul2(neg2(qx), A.th2)));
+    gqz = fma2(qw, A.th2, fma2(qx, A.th1, mul2(neg2(qy), A.th0)));
+}
+
+// ---------------------------------------------------------------------------------------------
 // evaluation of a lobe pair at ONE direction d (scalar-broadcast operands)
 // ---------------------------------------------------------------------------------------------
 struct EvalPair {       // what the backward needs from the recomputed forward

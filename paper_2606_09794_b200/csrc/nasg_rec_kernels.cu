@@ -59,8 +59,10 @@ constexpr int HDR_BYTES = HDR_FLOATS * 4;       // 768
 //      3 = kind 0 with the quaternion and the amplitude stored as bfloat16 (fp32 arithmetic):
 //          per pair 4 x 128 B (quat: one 32-bit word per lane = bf16 of lobe 2j | bf16 of lobe 2j+1 << 16), 4 x 256 B (shape,
 //          fp32 pairs), 3 x 128 B (amplitude, bf16 pairs) = 1,920 B; the header and the GRADIENT record stay fp32 (kind 0)
+//      4 = the Anisotropic Spherical Gaussian of Table 6: quaternion + (raw mu, raw lambda) + amplitude:
+//          9 components per lobe (MODE unused: 0)
 template <int PK> struct Rec {
-    static constexpr int NCOMP = PK == 2 ? 7 : PK == 1 ? 9 : 11;
+    static constexpr int NCOMP = PK == 2 ? 7 : (PK == 1 || PK == 4) ? 9 : 11;
     static constexpr int PAIR_FLOATS = PK == 3 ? 480 : NCOMP * 2 * WT;          // 32-bit words of a pair
     static constexpr int PAIR_BYTES = PAIR_FLOATS * 4;        // 2816 | 2304 | 1792 | 1920
     static constexpr int GPK = PK == 3 ? 0 : PK;             // layout of the gradient record
@@ -87,7 +89,7 @@ template <int CT, bool BWD, int PK> struct Layout {
     static constexpr int H_GC = HDR_BYTES;
     static constexpr int H_VIS = H_GC + (BWD ? CT * WT * 12 : 0);
     static constexpr int H_BYTES = H_VIS + ((CT * WT + 127) / 128) * 128;
-    static constexpr int SCRATCH = BWD ? (2 * CT + (PK == 1 ? 3 : PK == 2 ? 0 : 2)) * WT * 16 : 0;     // (PK 0 and 3: 2)   // cam, gcm, parked frame terms (qs | trig | none)
+    static constexpr int SCRATCH = BWD ? (2 * CT + (PK == 1 ? 3 : (PK == 2 || PK == 4) ? 0 : 2)) * WT * 16 : 0;     // (PK 0 and 3: 2)   // cam, gcm, parked frame terms (qs | trig | none)
     __host__ __device__ static constexpr int region(int stages, int hslots) { return stages * PAIR_BYTES + hslots * H_BYTES + SCRATCH + 64; }
 };
 
@@ -326,6 +328,17 @@ __global__ void __launch_bounds__(FWD_TB, NASG_REC_FWD_MINB) nasg_rec_fwd_kernel
                         col[t][1] = fma2(r.v[5], G, col[t][1]);
                         col[t][2] = fma2(r.v[6], G, col[t][2]);
                     }
+                } else if constexpr (PK == 4) {    // Anisotropic Spherical Gaussian
+                    AsgPair Ap; f2 q0, q1, q2, q3;
+                    asg_pair_setup<false>(r.v[0], r.v[1], r.v[2], r.v[3], r.v[4], r.v[5], Ap, q0, q1, q2, q3);
+#pragma unroll
+                    for (int t = 0; t < CT; ++t) {
+                        AsgEval T;
+                        const f2 G = asg_pair_eval<false>(Ap, dx[t], dy[t], dz[t], T);
+                        col[t][0] = fma2(r.v[6], G, col[t][0]);
+                        col[t][1] = fma2(r.v[7], G, col[t][1]);
+                        col[t][2] = fma2(r.v[8], G, col[t][2]);
+                    }
                 } else if (ALL || wmask != 0u) {
                     LobePair Lp; LobePairGrad Gd; f2 park[6], w0, w1, w2;
                     setup_pair<PK, MODE, false>(r, Lp, Gd, park, w0, w1, w2);
@@ -342,7 +355,7 @@ __global__ void __launch_bounds__(FWD_TB, NASG_REC_FWD_MINB) nasg_rec_fwd_kernel
                 }
             }
         };
-        if (!SKIP || PK == 2 || wmask == FULL) run_pairs(std::true_type{});
+        if (!SKIP || PK == 2 || PK == 4 || wmask == FULL) run_pairs(std::true_type{});
         else run_pairs(std::false_type{});
         if (valid) {
             float *o = p.colors + n * 3;
@@ -471,6 +484,25 @@ __global__ void __launch_bounds__(BWD_TB, NASG_REC_BWD_MINB) nasg_rec_bwd_kernel
                 g[1] = mul2(fma2(neg2(Ip.zy), dot, gzy), Ip.inv);
                 g[2] = mul2(fma2(neg2(Ip.zz), dot, gzz), Ip.inv);
                 g[3] = gs; g[4] = gw0; g[5] = gw1; g[6] = gw2;
+            } else if constexpr (PK == 4) {    // Anisotropic Spherical Gaussian
+                AsgPair Ap; f2 q0, q1, q2, q3;
+                asg_pair_setup<true>(r.v[0], r.v[1], r.v[2], r.v[3], r.v[4], r.v[5], Ap, q0, q1, q2, q3);
+                const f2 w0 = r.v[6], w1 = r.v[7], w2 = r.v[8];
+                AsgAcc A;
+                auto cam_bwd = [&](int t, auto first) {
+                    const float4 cam = lds128(scr_cam + t * WT * 16);
+                    const float4 gc = lds128(scr_gc + t * WT * 16);         // zero for a culled slot: every contribution vanishes
+                    AsgEval T;
+                    const f2 G = asg_pair_eval<true>(Ap, cam.x, cam.y, cam.z, T);
+                    f2 gx = splat(0.f), gy = splat(0.f), gz = splat(0.f);
+                    asg_pair_bwd<decltype(first)::value>(Ap, T, G, gc.x, gc.y, gc.z, w0, w1, w2, A, gx, gy, gz);
+                    gd[t][0] += lo(gx) + hi(gx); gd[t][1] += lo(gy) + hi(gy); gd[t][2] += lo(gz) + hi(gz);
+                };
+                cam_bwd(0, std::true_type{});
+#pragma unroll
+                for (int t = 1; t < CT; ++t) cam_bwd(t, std::false_type{});
+                asg_pair_finish(Ap, A, q0, q1, q2, q3, g[4], g[5], g[0], g[1], g[2], g[3]);
+                g[6] = A.gw0; g[7] = A.gw1; g[8] = A.gw2;
             } else if (SKIP && wmask == 0u) {  // (warp-uniform) a tile culled in every camera: zero gradients, no arithmetic (F0)
 #pragma unroll
                 for (int c = 0; c < Rec<PK>::NCOMP; ++c) g[c] = splat(0.f);
@@ -643,7 +675,7 @@ namespace rec = lp::rec;
 // ---------------------------------------------------------------------------------------------
 int64_t rec_total_floats(int64_t N, int K, int pk)
 {
-    return ((N + rec::WT - 1) / rec::WT) * (int64_t)(pk == 3 ? rec::Rec<3>::rec_floats(K) : pk == 2 ? rec::Rec<2>::rec_floats(K) : pk == 1 ? rec::Rec<1>::rec_floats(K) : rec::Rec<0>::rec_floats(K));
+    return ((N + rec::WT - 1) / rec::WT) * (int64_t)(pk == 4 ? rec::Rec<4>::rec_floats(K) : pk == 3 ? rec::Rec<3>::rec_floats(K) : pk == 2 ? rec::Rec<2>::rec_floats(K) : pk == 1 ? rec::Rec<1>::rec_floats(K) : rec::Rec<0>::rec_floats(K));
 }
 
 template <typename Kernel>
@@ -671,7 +703,9 @@ static cudaError_t launch_rec_fwd_kc(const RecFwdParams &p, int mode, cudaStream
     constexpr size_t smem = (size_t)(TB / 32) * rec::Layout<CT, false, PK>::region(NASG_REC_FWD_STAGES, NASG_REC_FWD_HSLOTS);
     static int cache[3][64] = {{0}};
     using namespace rec;
-    if (mode == 1) nasg_rec_fwd_kernel<K, CT, 1, PK, SKIP><<<rec_grid(nasg_rec_fwd_kernel<K, CT, 1, PK, SKIP>, TB, smem, p.N, cache[1]), TB, smem, st>>>(p);
+    if constexpr (PK == 4) {        // one function: MODE 0 only
+        nasg_rec_fwd_kernel<K, CT, 0, PK, SKIP><<<rec_grid(nasg_rec_fwd_kernel<K, CT, 0, PK, SKIP>, TB, smem, p.N, cache[0]), TB, smem, st>>>(p);
+    } else if (mode == 1) nasg_rec_fwd_kernel<K, CT, 1, PK, SKIP><<<rec_grid(nasg_rec_fwd_kernel<K, CT, 1, PK, SKIP>, TB, smem, p.N, cache[1]), TB, smem, st>>>(p);
     else if (mode == 0) nasg_rec_fwd_kernel<K, CT, 0, PK, SKIP><<<rec_grid(nasg_rec_fwd_kernel<K, CT, 0, PK, SKIP>, TB, smem, p.N, cache[0]), TB, smem, st>>>(p);
     else nasg_rec_fwd_kernel<K, CT, 2, PK, SKIP><<<rec_grid(nasg_rec_fwd_kernel<K, CT, 2, PK, SKIP>, TB, smem, p.N, cache[2]), TB, smem, st>>>(p);
     return cudaGetLastError();
@@ -701,7 +735,7 @@ static cudaError_t launch_rec_fwd_pk(const RecFwdParams &p, int K, int mode, cud
 }
 cudaError_t launch_nasg_rec_fwd(const RecFwdParams &p, int K, int mode, int pk, cudaStream_t st)
 {
-    return pk == 3 ? launch_rec_fwd_pk<3>(p, K, mode, st) : pk == 2 ? launch_rec_fwd_pk<2>(p, K, mode, st)
+    return pk == 4 ? launch_rec_fwd_pk<4>(p, K, mode, st) : pk == 3 ? launch_rec_fwd_pk<3>(p, K, mode, st) : pk == 2 ? launch_rec_fwd_pk<2>(p, K, mode, st)
                    : pk == 1 ? launch_rec_fwd_pk<1>(p, K, mode, st) : launch_rec_fwd_pk<0>(p, K, mode, st);
 }
 
@@ -712,7 +746,9 @@ static cudaError_t launch_rec_bwd_kc(const RecBwdParams &p, int mode, cudaStream
     constexpr size_t smem = (size_t)(TB / 32) * rec::Layout<CT, true, PK>::region(NASG_REC_BWD_STAGES, 1);
     static int cache[3][64] = {{0}};
     using namespace rec;
-    if (mode == 1) nasg_rec_bwd_kernel<K, CT, 1, PK, SKIP><<<rec_grid(nasg_rec_bwd_kernel<K, CT, 1, PK, SKIP>, TB, smem, p.N, cache[1]), TB, smem, st>>>(p);
+    if constexpr (PK == 4) {        // one function: MODE 0 only
+        nasg_rec_bwd_kernel<K, CT, 0, PK, SKIP><<<rec_grid(nasg_rec_bwd_kernel<K, CT, 0, PK, SKIP>, TB, smem, p.N, cache[0]), TB, smem, st>>>(p);
+    } else if (mode == 1) nasg_rec_bwd_kernel<K, CT, 1, PK, SKIP><<<rec_grid(nasg_rec_bwd_kernel<K, CT, 1, PK, SKIP>, TB, smem, p.N, cache[1]), TB, smem, st>>>(p);
     else if (mode == 0) nasg_rec_bwd_kernel<K, CT, 0, PK, SKIP><<<rec_grid(nasg_rec_bwd_kernel<K, CT, 0, PK, SKIP>, TB, smem, p.N, cache[0]), TB, smem, st>>>(p);
     else nasg_rec_bwd_kernel<K, CT, 2, PK, SKIP><<<rec_grid(nasg_rec_bwd_kernel<K, CT, 2, PK, SKIP>, TB, smem, p.N, cache[2]), TB, smem, st>>>(p);
     return cudaGetLastError();
@@ -742,7 +778,7 @@ static cudaError_t launch_rec_bwd_pk(const RecBwdParams &p, int K, int mode, cud
 }
 cudaError_t launch_nasg_rec_bwd(const RecBwdParams &p, int K, int mode, int pk, cudaStream_t st)
 {
-    return pk == 3 ? launch_rec_bwd_pk<3>(p, K, mode, st) : pk == 2 ? launch_rec_bwd_pk<2>(p, K, mode, st)
+    return pk == 4 ? launch_rec_bwd_pk<4>(p, K, mode, st) : pk == 3 ? launch_rec_bwd_pk<3>(p, K, mode, st) : pk == 2 ? launch_rec_bwd_pk<2>(p, K, mode, st)
                    : pk == 1 ? launch_rec_bwd_pk<1>(p, K, mode, st) : launch_rec_bwd_pk<0>(p, K, mode, st);
 }
 

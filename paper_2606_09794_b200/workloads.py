@@ -144,6 +144,22 @@ def make_iso(cfg: Config, N: Optional[int] = None) -> dict:
     return out
 
 
+def make_asg(cfg: Config, N: Optional[int] = None) -> dict:
+    """The same config for the Anisotropic Spherical Gaussian of Table 6 (include/nasg.h: nasg_asg_*): quat [K,N,4] ~ N(0,1)^4
+    scaled by U[0.5,2] (unnormalised on purpose), shp [K,N,2] = (raw mu, raw lambda) ~ U[-1, 4.5] (bandwidths e^raw in
+    [0.37, 90]), amp ~ N(0,0.3), dc ~ N(0,0.3); geometry, masks and g_colors as make_nasg."""
+    assert cfg.kind == "nasg"
+    out = make_geometry(cfg, N)
+    N, K = out["N"], cfg.K
+    r = _rng(cfg.seed, TAG_QUAT)
+    quat = r.standard_normal(size=(K, N, 4)) * r.uniform(0.5, 2.0, size=(K, N, 1))
+    shp = _rng(cfg.seed, TAG_BW).uniform(-1.0, 4.5, size=(K, N, 2))
+    amp = _rng(cfg.seed, TAG_AMP).normal(0.0, 0.3, size=(K, 3, N))
+    dc = _rng(cfg.seed, TAG_DC).normal(0.0, 0.3, size=(3, N))
+    out.update(K=K, quat=quat.astype(np.float32), shp=shp.astype(np.float32), amp=amp.astype(np.float32), dc=dc.astype(np.float32))
+    return out
+
+
 def make_sh(cfg: Config, N: Optional[int] = None) -> dict:
     """Inputs of sh_eval_fwd/bwd (config 3): geometry of config 2 plus degree-3 coefficients."""
     assert cfg.kind == "sh"
@@ -268,6 +284,28 @@ def unpack_iso_records(rec: np.ndarray, N: int, K: int) -> dict:
     means, dc, comp = _unpack(rec, N, K, 7)
     return dict(means=means, dc=dc, axis=np.ascontiguousarray(comp[..., 0:3]), shp=np.ascontiguousarray(comp[..., 3]),
                 amp=np.ascontiguousarray(comp[..., 4:7].transpose(0, 2, 1)))
+
+
+def asg_rec_floats(N: int, K: int) -> int:
+    return ((N + REC_TILE - 1) // REC_TILE) * REC_TILE * (6 + 9 * K)
+
+
+def pack_asg_records(means, quat, shp, amp, dc) -> np.ndarray:
+    """Anisotropic Spherical Gaussian lobes as tile records float32 [T, 6 + 9 K, 32]: per lobe (q_w, q_x, q_y, q_z, raw mu,
+    raw lambda, w_r, w_g, w_b). Padding lanes get the unit quaternion."""
+    N = quat.shape[1]
+    rec = _pack(means, dc, np.concatenate([quat, shp, amp.transpose(0, 2, 1)], axis=2))
+    if N % REC_TILE:
+        K = quat.shape[0]
+        r = rec.reshape(-1, 6 + 9 * K, REC_TILE)
+        r[-1, 6:].reshape(K // 2, 9, REC_TILE, 2)[:, 0, N % REC_TILE:, :] = 1.0
+    return rec
+
+
+def unpack_asg_records(rec: np.ndarray, N: int, K: int) -> dict:
+    means, dc, comp = _unpack(rec, N, K, 9)
+    return dict(means=means, dc=dc, quat=np.ascontiguousarray(comp[..., 0:4]), shp=np.ascontiguousarray(comp[..., 4:6]),
+                amp=np.ascontiguousarray(comp[..., 6:9].transpose(0, 2, 1)))
 
 
 # ---- bf16 parameter storage (include/nasg.h: nasg_rec16_*): quaternion and amplitude as bfloat16, the rest fp32 -------
