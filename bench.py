@@ -187,13 +187,14 @@ class Resident:
             layout = "rec"
         self.paper = cfg.kind == "nasg" and layout == "paper"          # the paper's own 3 + 9K record (nasg_paper_*)
         self.iso = int(layout[3]) if cfg.kind == "nasg" and layout.startswith("iso") else None    # isotropic Table-6 function (nasg_iso_*)
-        inp = W.make_sh(rcfg) if cfg.kind == "sh" else W.make_paper(rcfg) if self.paper else W.make_iso(rcfg) if self.iso is not None else W.make_nasg(rcfg, vis_cluster=self.cluster)
+        self.asg = cfg.kind == "nasg" and layout == "asg"              # Anisotropic Spherical Gaussian of Table 6 (nasg_asg_*)
+        inp = W.make_sh(rcfg) if cfg.kind == "sh" else W.make_paper(rcfg) if self.paper else W.make_iso(rcfg) if self.iso is not None else W.make_asg(rcfg) if self.asg else W.make_nasg(rcfg, vis_cluster=self.cluster)
         self.N, self.C, self.K = inp["N"], inp["C"], inp.get("K", 0)
         # tile-record parameter layout (include/nasg.h: nasg_rec_*) where it applies, else the row arrays
         self.bf16 = cfg.kind == "nasg" and layout == "rec16"             # bf16 quaternion / amplitude storage (nasg_rec16_*)
-        self.rec = cfg.kind == "nasg" and (layout in ("rec", "paper", "rec16") or self.iso is not None) and self.K in (2, 4, 8) and self.C <= 4
-        assert self.rec or not (self.paper or self.iso is not None)
-        self.keys = ("means", "coeffs", "campos", "vis", "g_colors") if cfg.kind == "sh" else ("campos", "vis", "g_colors") if (self.paper or self.iso is not None) else \
+        self.rec = cfg.kind == "nasg" and (layout in ("rec", "paper", "rec16", "asg") or self.iso is not None) and self.K in (2, 4, 8) and self.C <= 4
+        assert self.rec or not (self.paper or self.asg or self.iso is not None)
+        self.keys = ("means", "coeffs", "campos", "vis", "g_colors") if cfg.kind == "sh" else ("campos", "vis", "g_colors") if (self.paper or self.asg or self.iso is not None) else \
                     ("means", "quat", "shape", "amp", "dc", "campos", "vis", "g_colors")
         d = {k: (None if inp.get(k) is None else torch.from_numpy(np.ascontiguousarray(inp[k])).cuda()) for k in self.keys}
         self.d = d
@@ -204,6 +205,9 @@ class Resident:
             self.g_params = torch.zeros_like(self.params)
         elif self.iso is not None:
             self.params = torch.from_numpy(W.pack_iso_records(inp["means"], inp["axis"], inp["shp"], inp["amp"], inp["dc"])).cuda()
+            self.g_params = torch.zeros_like(self.params)
+        elif self.asg:
+            self.params = torch.from_numpy(W.pack_asg_records(inp["means"], inp["quat"], inp["shp"], inp["amp"], inp["dc"])).cuda()
             self.g_params = torch.zeros_like(self.params)
         elif self.rec:  # the parameters LIVE in HBM as records (packed once, outside any timed region: it is the storage layout)
             self.params = (B.nasg_rec16_pack if self.bf16 else B.nasg_rec_pack)(d["means"], d["quat"], d["shape"], d["amp"], d["dc"])
@@ -220,6 +224,8 @@ class Resident:
             B.nasg_paper_eval_fwd(self.params, self.N, self.K, d["campos"], d["vis"], self.norm_mode, out=self.colors, stream=st)
         elif self.iso is not None:
             B.nasg_iso_eval_fwd(self.params, self.N, self.K, d["campos"], self.iso, d["vis"], out=self.colors, stream=st)
+        elif self.asg:
+            B.nasg_asg_eval_fwd(self.params, self.N, self.K, d["campos"], d["vis"], out=self.colors, stream=st)
         elif self.rec:
             (B.nasg_rec16_eval_fwd if self.bf16 else B.nasg_rec_eval_fwd)(self.params, self.N, self.K, d["campos"], d["vis"], self.norm_mode,
                                                                          out=self.colors, stream=st)
@@ -236,6 +242,8 @@ class Resident:
                                   out=self.g_params, stream=st)
         elif self.iso is not None:
             B.nasg_iso_eval_bwd(self.params, self.N, self.K, d["campos"], d["g_colors"], self.iso, d["vis"], out=self.g_params, stream=st)
+        elif self.asg:
+            B.nasg_asg_eval_bwd(self.params, self.N, self.K, d["campos"], d["g_colors"], d["vis"], out=self.g_params, stream=st)
         elif self.rec:
             (B.nasg_rec16_eval_bwd if self.bf16 else B.nasg_rec_eval_bwd)(self.params, self.N, self.K, d["campos"], d["g_colors"], d["vis"],
                                                                          self.norm_mode, out=self.g_params, stream=st)
@@ -247,7 +255,7 @@ class Resident:
 
     def kernel_name(self):
         if self.rec:
-            return "nasg_rec_bwd_kernel<PK=1>" if self.paper else "nasg_rec_bwd_kernel<PK=2>" if self.iso is not None else "nasg_rec_bwd_kernel<PK=3>" if self.bf16 else "nasg_rec_bwd_kernel"
+            return "nasg_rec_bwd_kernel<PK=1>" if self.paper else "nasg_rec_bwd_kernel<PK=2>" if self.iso is not None else "nasg_rec_bwd_kernel<PK=4>" if self.asg else "nasg_rec_bwd_kernel<PK=3>" if self.bf16 else "nasg_rec_bwd_kernel"
         pipe = self.C <= 4
         if self.cfg.kind == "sh":
             return "sh_bwd_pipe_kernel" if pipe else "sh_bwd_kernel"
@@ -356,8 +364,8 @@ def run_ours(args, W, cfg):
     peak, peak_src = measured_peak()
 
     def summary(r, f_ms, b_ms):
-        fb, bb = algorithmic_bytes(r.cfg.kind, r.K, r.C, r.has_vis, r.paper, r.iso is not None, r.bf16)
-        return {"layout": "records; LABELLED VARIANT: visibility drawn per (camera, run of 256 Gaussians), spatially coherent" if r.cluster > 1 else "records, bf16 quaternion + amplitude (fp32 arithmetic and gradients)" if r.bf16 else "paper records (3 + 9K floats)" if r.paper else ("isotropic Table-6 records (3 + 7K floats): " + ("Spherical Gaussian", "Spherical Beta", "Spherical Cauchy")[r.iso]) if r.iso is not None else "records" if r.rec else "rows", "bytes_per_gaussian": [fb, bb], "kernel": r.kernel_name(), "fwd_ms": f_ms, "bwd_ms": b_ms,
+        fb, bb = algorithmic_bytes(r.cfg.kind, r.K, r.C, r.has_vis, r.paper or r.asg, r.iso is not None, r.bf16)
+        return {"layout": "records; LABELLED VARIANT: visibility drawn per (camera, run of 256 Gaussians), spatially coherent" if r.cluster > 1 else "records, bf16 quaternion + amplitude (fp32 arithmetic and gradients)" if r.bf16 else "paper records (3 + 9K floats)" if r.paper else "Anisotropic Spherical Gaussian records (3 + 9K floats)" if r.asg else ("isotropic Table-6 records (3 + 7K floats): " + ("Spherical Gaussian", "Spherical Beta", "Spherical Cauchy")[r.iso]) if r.iso is not None else "records" if r.rec else "rows", "bytes_per_gaussian": [fb, bb], "kernel": r.kernel_name(), "fwd_ms": f_ms, "bwd_ms": b_ms,
                 "value": r.N / ((f_ms + b_ms) * 1e-3), "fwd_gbs": fb * r.N / (f_ms * 1e-3) / 1e9, "bwd_gbs": bb * r.N / (b_ms * 1e-3) / 1e9,
                 "bwd_frac": bb * r.N / (b_ms * 1e-3) / 1e9 / peak, "fwd+bwd_frac": (fb + bb) * r.N / ((f_ms + b_ms) * 1e-3) / 1e9 / peak}
 
@@ -374,7 +382,7 @@ def run_ours(args, W, cfg):
         specs += [(i, "paper") for i in (1, 2, 4)]             # the paper's own 3 + 9K record (17 % fewer parameter bytes)
         specs.append((2, "rec_clustered"))                     # cfg2 with visibility constant over runs of 256 Gaussians (NOT the headline)
         specs += [(i, "rec16") for i in (1, 2, 4)]             # bf16 storage of quaternion and amplitude (NEXT-3)
-        specs += [(2, "iso0"), (2, "iso1"), (2, "iso2")]       # the other Table-6 functions in the same skeleton (NEXT-3)
+        specs += [(2, "iso0"), (2, "iso1"), (2, "iso2"), (2, "asg")]       # the other Table-6 functions in the same skeleton (NEXT-3)
         R_keep, R = R, None
         if cfg.N > 2_000_000:
             R_keep.d = None; R_keep.params = None; R_keep.g_params = None; R_keep.colors = None
