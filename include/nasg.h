@@ -52,6 +52,8 @@ extern "C" {
 #define NASG_ERR_WORKSPACE      -5  /* g_campos requested but workspace NULL or too small           */
 #define NASG_ERR_CUDA           -6  /* launch / copy failed: cudaGetLastError()                     */
 #define NASG_ERR_NORM_MODE      -7  /* norm_mode not 0, 1 or 2                                      */
+#define NASG_ERR_NOALLOC_SIZE   -8  /* nasg_eval_bwd_noalloc: the problem needs more scratch than   */
+                                    /* the built-in NASG_NOALLOC_WS_BYTES (use nasg_eval_bwd)       */
 
 #define NASG_MAX_CAMERAS 64
 
@@ -230,6 +232,35 @@ int nasg_paper_eval_fwd_bwd_host(const nasg_rec_inputs *in, const float *g_color
 
 /* Bytes of device scratch nasg_eval_bwd / sh_eval_bwd need when g_campos != NULL (pass K = 0 for SH). */
 size_t nasg_workspace_bytes(int64_t N, int32_t K, int32_t C);
+
+/* ---- backward with g_campos for callers that cannot allocate device memory ----------------------------------
+ * nasg_eval_bwd asks the caller for `workspace` when g_campos is wanted. Not every caller can produce one: a plug-in
+ * that lives inside a host application (a viewer, a trainer with its own caching allocator) and must not call
+ * cudaMalloc behind that application's back; a real-time render loop, where cudaMalloc / cudaFree synchronise the
+ * device and drop frames; a process whose device memory was handed out completely at start-up; a C caller that links
+ * this library without the CUDA runtime. nasg_eval_bwd_noalloc is nasg_eval_bwd for them: same inputs, same outputs,
+ * same kernels and summation order (so the same values), but the per-block partial sums of g_campos go to a fixed
+ * array of NASG_NOALLOC_WS_BYTES that is part of the library image in device memory. The call allocates and frees
+ * nothing (no cudaMalloc / cudaFree, no allocating library routine); out->workspace and out->workspace_bytes are
+ * ignored. What to know before using it:
+ *   - Cost: every GPU on which the library is loaded holds NASG_NOALLOC_WS_BYTES (1 MiB) from module load until the
+ *     process exits, used or not.
+ *   - Limit: nasg_workspace_bytes(N, K, C) <= nasg_noalloc_workspace_bytes(), i.e. ceil(N / 256) * C <= 87,381 (for
+ *     example N <= 5.59 million at C = 4, N <= 22.3 million at C = 1). Larger problems are refused with
+ *     NASG_ERR_NOALLOC_SIZE and nothing is launched; use nasg_eval_bwd with your own workspace for those.
+ *   - out->g_campos is required (NASG_ERR_NULL otherwise): without it the backward needs no scratch and nasg_eval_bwd
+ *     already serves the caller. The other gradient pointers stay optional.
+ *   - First call on a device: the library looks up the array's device address there (cudaGetSymbolAddress, once per
+ *     device, with the calling thread's current device; this may load the module on that device). Make that first
+ *     call on each device outside of any stream capture; later calls only launch the two kernels.
+ *   - One array per device, shared by every call: two calls whose kernels can overlap on the GPU (different streams
+ *     without an ordering between them, or two host threads on different streams) race on it and both g_campos
+ *     results are garbage. Calls on one stream, or ordered by events, are safe. The array keeps the last call's
+ *     partial sums; the next call overwrites every entry it later reads, so nothing has to be cleared in between. */
+#define NASG_NOALLOC_WS_BYTES (1u << 20)
+size_t nasg_noalloc_workspace_bytes(void);            /* = NASG_NOALLOC_WS_BYTES */
+int nasg_eval_bwd_noalloc(const nasg_inputs *in, const float *g_colors, const nasg_grads *out, int norm_mode,
+                          void *cuda_stream);
 
 /* ---- end-to-end entry points with HOST buffers -------------------------------------------------
  * Same computation, forward then backward, but every array pointer in `in`, `colors`, `g_colors`

@@ -28,7 +28,8 @@ SYMBOLS = ("nasg_eval_fwd", "nasg_eval_bwd", "sh_eval_fwd", "sh_eval_bwd", "nasg
            "nasg_paper_eval_bwd", "nasg_paper_host_scratch_bytes", "nasg_paper_eval_fwd_bwd_host",
            "nasg_iso_floats", "nasg_iso_eval_fwd", "nasg_iso_eval_bwd",
            "nasg_asg_floats", "nasg_asg_eval_fwd", "nasg_asg_eval_bwd",
-           "nasg_rec16_floats", "nasg_rec16_pack", "nasg_rec16_eval_fwd", "nasg_rec16_eval_bwd")
+           "nasg_rec16_floats", "nasg_rec16_pack", "nasg_rec16_eval_fwd", "nasg_rec16_eval_bwd",
+           "nasg_noalloc_workspace_bytes", "nasg_eval_bwd_noalloc")
 
 
 class NasgError(RuntimeError):
@@ -75,6 +76,10 @@ def _load():
     lib.sh_eval_bwd.argtypes = [i64, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.nasg_workspace_bytes.argtypes = [i64, i32, i32]
     lib.nasg_workspace_bytes.restype = sz
+    lib.nasg_noalloc_workspace_bytes.argtypes = []
+    lib.nasg_noalloc_workspace_bytes.restype = sz
+    lib.nasg_eval_bwd_noalloc.argtypes = [C.POINTER(_Inputs), vp, C.POINTER(_Grads), C.c_int, vp]
+    lib.nasg_eval_bwd_noalloc.restype = C.c_int
     lib.nasg_host_scratch_bytes.argtypes = [i64, i32, i32]
     lib.nasg_host_scratch_bytes.restype = sz
     lib.sh_host_scratch_bytes.argtypes = [i64, i32]
@@ -229,6 +234,32 @@ def nasg_eval_bwd(means, quat, shape, amp, dc, campos, g_colors, vis=None, norm_
     rc = _lib.nasg_eval_bwd(C.byref(inp), _ptr(g_colors), C.byref(gs), int(norm_mode), _stream(stream))
     if rc != 0:
         raise NasgError(rc, "nasg_eval_bwd")
+    return out
+
+
+def nasg_noalloc_workspace_bytes() -> int:
+    """Capacity of the library's built-in scratch array (include/nasg.h: NASG_NOALLOC_WS_BYTES)."""
+    return int(_lib.nasg_noalloc_workspace_bytes())
+
+
+def nasg_eval_bwd_noalloc(means, quat, shape, amp, dc, campos, g_colors, out: dict, vis=None,
+                          norm_mode: int = NORM_EXACT, stream=None) -> dict:
+    """``nasg_eval_bwd`` with ``g_campos`` for callers that cannot allocate device memory (a plug-in inside a host
+    application's memory budget, a render loop that cannot afford cudaMalloc's device-wide synchronisation, a process
+    whose device memory is fully handed out): the partial sums of ``g_campos`` go to a fixed 1 MiB array inside the
+    library instead of a caller-provided workspace. Accordingly this wrapper creates no tensor either: ``out`` must
+    hold every gradient tensor the caller wants written, ``g_campos`` [C,3] among them (no ``workspace`` entry is
+    needed or looked at). Problems with ``nasg_workspace_bytes(N, K, C) > nasg_noalloc_workspace_bytes()`` raise
+    ``NasgError`` (code -8). Calls share the one array per device, so calls that may overlap on the GPU race."""
+    inp = _inputs(means, quat, shape, amp, dc, campos, vis)
+    _chk(g_colors, "g_colors", (inp.C, inp.N, 3), torch.float32, "cuda")
+    if out.get("g_campos") is None:
+        raise ValueError("nasg_eval_bwd_noalloc: out['g_campos'] [C,3] is required (without it use nasg_eval_bwd)")
+    gs = _Grads(_ptr(out.get("g_means")), _ptr(out.get("g_quat")), _ptr(out.get("g_shape")), _ptr(out.get("g_amp")),
+                _ptr(out.get("g_dc")), _ptr(out["g_campos"]), None, 0)
+    rc = _lib.nasg_eval_bwd_noalloc(C.byref(inp), _ptr(g_colors), C.byref(gs), int(norm_mode), _stream(stream))
+    if rc != 0:
+        raise NasgError(rc, "nasg_eval_bwd_noalloc")
     return out
 
 

@@ -39,6 +39,7 @@ size_t cam_partial_bytes(int64_t N, int C) { return (size_t)nasg::grid_blocks(N)
 
 namespace nasg {
 int api_cuda_fail(cudaError_t e) { return cuda_fail(e); }
+void api_count_launches(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 } // namespace nasg
 
 extern "C" {
@@ -330,6 +331,7 @@ const char *nasg_strerror(int code)
     case NASG_ERR_WORKSPACE: return "workspace/scratch missing, misaligned or too small";
     case NASG_ERR_CUDA: return cudaGetErrorString(t_last_cuda);
     case NASG_ERR_NORM_MODE: return "norm_mode must be 0 (approximate), 1 (exact, eq.10) or 2 (pure NASG, no carrier); nasg_iso_*: kind must be 0, 1 or 2";
+    case NASG_ERR_NOALLOC_SIZE: return "nasg_eval_bwd_noalloc: N and C need more scratch than the built-in 1 MiB array (nasg_workspace_bytes(N,K,C) > nasg_noalloc_workspace_bytes()); call nasg_eval_bwd with a workspace of your own";
     default: return "unknown error code";
     }
 }

@@ -57,6 +57,7 @@ struct RecBwdParams {
 
 int64_t grid_blocks(int64_t N);
 int api_cuda_fail(cudaError_t e);     // remembers e for nasg_strerror(), returns NASG_ERR_CUDA (nasg_api.cu)
+void api_count_launches(int n);       // adds to nasg_launch_count() (for entry points outside nasg_api.cu)
 cudaError_t launch_nasg_fwd(const FwdParams &p, int K, int mode, cudaStream_t st);
 cudaError_t launch_nasg_bwd(const BwdParams &p, int K, int mode, cudaStream_t st);
 // fast path (nasg_pipe_kernels.cu): C <= 4, persistent threads, cp.async lobe ring

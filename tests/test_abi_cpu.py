@@ -69,7 +69,18 @@ def test_error_codes_without_gpu(B):
     assert lib.nasg_eval_bwd(C.byref(inputs()), None, C.byref(g), 1, None) == -1
     assert lib.sh_eval_fwd(4, 0, p, p, p, None, p, None) == -2
     assert lib.sh_eval_fwd(4, 1, None, p, p, None, p, None) == -1
-    for code in (0, -1, -2, -3, -4, -5, -7):
+    # nasg_eval_bwd_noalloc (built-in scratch): argument checks come before any CUDA call, so they run without a GPU
+    noalloc = lambda inp, gr: lib.nasg_eval_bwd_noalloc(C.byref(inp), C.c_void_p(p), C.byref(gr), 1, None)
+    g = B._Grads(p, p, p, p, p, None, None, 0)
+    assert noalloc(inputs(), g) == -1                                           # g_campos is required
+    g = B._Grads(p, p, p, p, p, p, None, 0)
+    assert noalloc(inputs(K=6), g) == -3 and noalloc(inputs(Cn=65), g) == -2
+    cap = B.nasg_noalloc_workspace_bytes()
+    assert cap == 1 << 20 == B.nasg_workspace_bytes(256 * 21845, 4, 4) + 16     # 21,845 block rows of 4 x 3 floats fit
+    assert noalloc(inputs(N=256 * 21845 + 1, K=4, Cn=4), g) == -8               # one more row does not: NOALLOC_SIZE
+    assert noalloc(inputs(N=256 * 87381 + 1, K=2, Cn=1), g) == -8
+    assert "nasg_eval_bwd" in B.nasg_strerror(-8)
+    for code in (0, -1, -2, -3, -4, -5, -7, -8):
         assert B.nasg_strerror(code) and "unknown" not in B.nasg_strerror(code)
     assert "unknown" in B.nasg_strerror(-99)
 
