@@ -55,6 +55,30 @@ struct RecBwdParams {
     float *g_params;
 };
 
+// Grid of a persistent kernel: min(blocks N needs, blocks resident on the device). The occupancy query and the opt-in to
+// `smem` bytes of dynamic shared memory are made once per (kernel instantiation, device) and the resident count is kept
+// in `cached` ([64], one slot per device ordinal, zero = not set up yet). Host threads may race on a first call: the
+// slot is read and written atomically and every thread would store the same value. A failed opt-in is NOT cached: it is
+// retried by the next launch, and the launch that follows here fails and reports it through cudaGetLastError().
+template <typename Kernel>
+static int resident_grid(Kernel kernel, int threads, size_t smem, int64_t N, int *cached)
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) dev = -1;
+    const bool slot = dev >= 0 && dev < 64;
+    int resident = slot ? __atomic_load_n(&cached[dev], __ATOMIC_ACQUIRE) : 0;
+    if (resident == 0) {
+        int sms = 148, per_sm = 1;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev < 0 ? 0 : dev);
+        const cudaError_t opt_in = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
+        resident = per_sm * sms;
+        if (slot && opt_in == cudaSuccess) __atomic_store_n(&cached[dev], resident, __ATOMIC_RELEASE);
+    }
+    const int64_t need = (N + threads - 1) / threads;
+    return (int)(need < resident ? need : resident);
+}
+
 int64_t grid_blocks(int64_t N);
 int api_cuda_fail(cudaError_t e);     // remembers e for nasg_strerror(), returns NASG_ERR_CUDA (nasg_api.cu)
 void api_count_launches(int n);       // adds to nasg_launch_count() (for entry points outside nasg_api.cu)

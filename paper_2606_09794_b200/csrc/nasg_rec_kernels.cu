@@ -78,6 +78,10 @@ template <int PK> struct Rec {
 #ifndef NASG_REC_FWD_HSLOTS
 #define NASG_REC_FWD_HSLOTS 2
 #endif
+// The barrier block at the end of a warp's region is 64 bytes: full[4] at 0..31, hfull[4] at 32..63 (bar_full / bar_hfull).
+static_assert(NASG_REC_FWD_STAGES >= 1 && NASG_REC_FWD_STAGES <= 4 && NASG_REC_BWD_STAGES >= 1 && NASG_REC_BWD_STAGES <= 4 &&
+              NASG_REC_FWD_HSLOTS >= 1 && NASG_REC_FWD_HSLOTS <= 4,
+              "more than 4 stages alias the header barriers, more than 4 header slots run into the next warp's region");
 
 // ---- shared memory: one private region per warp ---------------------------------------------------
 // [ stage 0 | ... | stage S-1 ][ header slot 0 | ... ][ scratch (backward) ][ mbarriers: full[4], hfull[4] ]
@@ -681,19 +685,7 @@ int64_t rec_total_floats(int64_t N, int K, int pk)
 template <typename Kernel>
 static int rec_grid(Kernel kernel, int TB, size_t smem, int64_t N, int *cached)
 {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    int resident = (dev >= 0 && dev < 64) ? cached[dev] : 0;
-    if (resident == 0) {
-        int sms = 148, per_sm = 1;
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, TB, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
-        resident = per_sm * sms;
-        if (dev >= 0 && dev < 64) cached[dev] = resident;
-    }
-    const int64_t need = (N + TB - 1) / TB;
-    return (int)(need < resident ? need : resident);
+    return resident_grid(kernel, TB, smem, N, cached);
 }
 
 template <int K, int CT, int PK, bool SKIP>

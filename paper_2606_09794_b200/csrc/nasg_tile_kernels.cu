@@ -182,6 +182,10 @@ __device__ __forceinline__ void direction(float mx, float my, float mz, const fl
 #define NASG_TILE_FWD_MINB (512 / NASG_TB)
 #endif
 constexpr int TILE_BWD_HSLOTS = 1;  // backward: shared memory is the limit (2 blocks of 256 threads per SM)
+// The barrier block at the end of a warp's region is 64 bytes: full[4] at 0..31, hfull[4] at 32..63.
+static_assert(NASG_TILE_FWD_STAGES >= 1 && NASG_TILE_FWD_STAGES <= 4 && NASG_TILE_BWD_STAGES >= 1 && NASG_TILE_BWD_STAGES <= 4 &&
+              NASG_TILE_FWD_HSLOTS >= 1 && NASG_TILE_FWD_HSLOTS <= 4 && TILE_BWD_HSLOTS <= 4,
+              "more than 4 stages alias the header barriers, more than 4 header slots run into the next warp's region");
 constexpr int TILE_BWD_MINB = 512 / TB;
 
 // ---------------------------------------------------------------------------------------------
@@ -413,19 +417,7 @@ using lp::tile_smem_bytes;
 template <typename Kernel>
 static int tile_grid(Kernel kernel, size_t smem, int64_t N, int *cached)
 {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    int resident = (dev >= 0 && dev < 64) ? cached[dev] : 0;
-    if (resident == 0) {
-        int sms = 148, per_sm = 1;
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, TB, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
-        resident = per_sm * sms;
-        if (dev >= 0 && dev < 64) cached[dev] = resident;
-    }
-    const int64_t need = (N + TB - 1) / TB;
-    return (int)(need < resident ? need : resident);
+    return resident_grid(kernel, TB, smem, N, cached);
 }
 
 bool tile_path_ok(int64_t N, int K, int C, const void *means, const void *amp, const void *planar, const void *rows, const void *vis)

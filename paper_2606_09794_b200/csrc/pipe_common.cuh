@@ -5,6 +5,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "nasg_internal.h"   // resident_grid
+
 namespace nasg {
 
 #ifndef NASG_PBLOCK
@@ -101,19 +103,7 @@ __device__ __forceinline__ void pipe_block_sum_store(float v, float *red, float 
 template <typename Kernel>
 static int pipe_grid(Kernel kernel, size_t smem, int64_t N, int *cached /* [64], one per kernel instantiation */)
 {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    int resident = (dev >= 0 && dev < 64) ? cached[dev] : 0;
-    if (resident == 0) {
-        int sms = 148, per_sm = 1;
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, PBLOCK, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
-        resident = per_sm * sms;
-        if (dev >= 0 && dev < 64) cached[dev] = resident;
-    }
-    const int64_t need = (N + PBLOCK - 1) / PBLOCK;
-    return (int)(need < resident ? need : resident);
+    return resident_grid(kernel, PBLOCK, smem, N, cached);
 }
 
 } // namespace nasg
