@@ -71,6 +71,28 @@ def test_P3_eq10_is_only_approximate_for_anisotropic_lobes(oracle, lam, a, k, de
         assert abs(got - dev) < 0.05 * abs(dev), (lam, a, k, got)
 
 
+# the deviation of eq.(10) from scipy.dblquad (1e-11) of eq.(9), found by the survey's own probe
+# BEFORE this oracle existed and printed there to two digits. The golden file above is written by the oracle, so reading it
+# back only guards against regressions; THESE numbers are the independent pin of the anisotropic normaliser at a > 0 and
+# k > 0 at the same time: they fix Lambda = lambda (1 + a) inside Psi (with Lambda = lambda the first row would be -7.9e-2,
+# with Lambda = lambda sqrt(1 + a) -4.0e-2, not -2.8e-3) and the 1/sqrt(1 + a) of the base integral (P1 sees it only at k = 0).
+SURVEY_Q2 = [(3.0, 1.0, 2.0, -2.8e-3), (3.0, 2.0, 5.0, -1.7e-2), (1.0, 0.5, 4.0, -6.8e-2), (0.5, 4.0, 6.0, -1.2e-1),
+             (7.4, 19.0, 8.0, 9e-4), (55.0, 1.7, 8.0, 7e-5), (148.0, 0.01, 8.0, 4e-7)]
+
+
+@pytest.mark.parametrize("lam,a,k,printed", SURVEY_Q2)
+def test_P3_matches_the_surveys_independent_probe(oracle, lam, a, k, printed):
+    """The oracle's eq.(10) / fine quadrature of the oracle's eq.(9) - 1 rounds to the value SURVEY.md prints (two digits
+    for the first four, one digit for the last three: half a unit of the last printed digit), and the golden file's row
+    for the same (lambda, a, k) says the same."""
+    got = 1.0 / sphere_integral_of_G(oracle, lam, a, k, 0.0, 1) - 1.0
+    digits = 2 if abs(printed) >= 2e-3 else 1
+    half_ulp = 0.5 * 10.0 ** (np.floor(np.log10(abs(printed))) - (digits - 1))
+    assert abs(got - printed) <= half_ulp * 1.02, (lam, a, k, got, printed)
+    stored = [r[3] for r in _golden_eq10_rows() if r[:3] == (lam, a, k)]
+    assert len(stored) == 1 and abs(stored[0] - printed) <= half_ulp * 1.02
+
+
 def test_P3_eq10_gap_closes_as_k_goes_to_zero(oracle):
     devs = [abs(1.0 / sphere_integral_of_G(oracle, 3.0, 1.0, k, 0.0, 1) - 1.0) for k in (2.0, 0.5, 0.1)]
     assert devs[0] > devs[1] > devs[2] and devs[2] < 1e-5
