@@ -604,10 +604,13 @@ __global__ void __launch_bounds__(256) rec_pack_kernel(int64_t N, int K, const f
         o[512] = a0; o[576] = a1; o[640] = a2;
     }
 }
-// bf16 records (kind 3): quaternion and amplitude rounded to bfloat16 (round to nearest even)
+// bf16 records (kind 3): quaternion and amplitude rounded to bfloat16 (round to nearest even). A NaN stays a NaN (sign and
+// upper payload kept, quiet bit set): the rounding increment would carry a NaN with low mantissa bits set out of the
+// exponent field (0x7FFFFFFF -> 0x8000 = -0.0) and a NaN parameter would be stored as a finite number.
 __device__ __forceinline__ unsigned short f2bf(float x)
 {
     unsigned u = __float_as_uint(x);
+    if ((u & 0x7fffffffu) > 0x7f800000u) return (unsigned short)((u >> 16) | 0x40u);
     u += 0x7fffu + ((u >> 16) & 1u);
     return (unsigned short)(u >> 16);
 }

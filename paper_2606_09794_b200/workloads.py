@@ -100,7 +100,7 @@ def make_nasg(cfg: Config, N: Optional[int] = None, vis_cluster: int = 1) -> dic
     return out
 
 
-def make_paper(cfg: Config, N: Optional[int] = None) -> dict:
+def make_paper(cfg: Config, N: Optional[int] = None, mirror_cameras: bool = True) -> dict:
     """The same config with the paper-native parameter record (include/nasg.h: nasg_paper_*; Table 8): RAW
     (pre-activation) values, drawn directly so that this module applies no activation: euler [K,N,3] ~ U[-1.8,1.8]
     (cosines tanh(raw) in +-0.947), shp [K,N,3] = (lambda_raw = the smaller of the two log-bandwidth draws, a_raw = their
@@ -108,11 +108,13 @@ def make_paper(cfg: Config, N: Optional[int] = None) -> dict:
     ampraw ~ N(0,0.3), dc ~ N(0,0.3); geometry, masks and g_colors as make_nasg, except that every camera is mirrored
     into the y <= 0 half-space: with sin = +sqrt(1 - cos^2) the record's lobe axes z = (c s, s s, c) all have z_y >= 0
     (SURVEY.md NEXT-2 "quirk"), so only view directions d = normalize(mean - campos) with d_y > 0 can
-    meet a lobe peak; a camera on the other side would see nothing but lobe tails."""
+    meet a lobe peak; a camera on the other side would see nothing but lobe tails. mirror_cameras=False keeps the
+    cameras as drawn (on both sides), the labelled variant test_paper_unmirrored_cameras runs."""
     assert cfg.kind == "nasg"
     out = make_geometry(cfg, N)
-    out["campos"] = out["campos"].copy()
-    out["campos"][:, 1] = -np.abs(out["campos"][:, 1])
+    if mirror_cameras:
+        out["campos"] = out["campos"].copy()
+        out["campos"][:, 1] = -np.abs(out["campos"][:, 1])
     N, K = out["N"], cfg.K
     euler = _rng(cfg.seed, TAG_EULER).uniform(-1.8, 1.8, size=(K, N, 3))
     b = _rng(cfg.seed, TAG_BW).uniform(cfg.bw_range[0], cfg.bw_range[1], size=(K, N, 2))
@@ -310,10 +312,15 @@ def unpack_asg_records(rec: np.ndarray, N: int, K: int) -> dict:
 
 # ---- bf16 parameter storage (include/nasg.h: nasg_rec16_*): quaternion and amplitude as bfloat16, the rest fp32 -------
 def to_bf16(a: np.ndarray) -> np.ndarray:
-    """Round an fp32 array to bfloat16 (round to nearest even) and return it as fp32: the values a bf16 record holds."""
+    """Round an fp32 array to bfloat16 (round to nearest even) and return it as fp32: the values a bf16 record holds.
+    A NaN stays a NaN (sign and upper payload kept, quiet bit set): the rounding increment must not carry a NaN whose low
+    mantissa bits are set out of the exponent field into +-0. Infinities stay infinities; a finite value beyond the largest
+    bf16 rounds to infinity. The pack kernel (nasg_rec16_pack) does the same, bit for bit."""
     u = np.ascontiguousarray(a, dtype=np.float32).view(np.uint32).astype(np.uint64)
-    u = (u + 0x7FFF + ((u >> 16) & 1)) & 0xFFFF0000
-    return u.astype(np.uint32).view(np.float32).reshape(np.shape(a))
+    nan = (u & 0x7FFFFFFF) > 0x7F800000
+    r = (u + 0x7FFF + ((u >> 16) & 1)) & 0xFFFF0000
+    r = np.where(nan, (u & 0xFFFF0000) | 0x00400000, r)
+    return r.astype(np.uint32).view(np.float32).reshape(np.shape(a))
 
 
 def rec16_words(N: int, K: int) -> int:

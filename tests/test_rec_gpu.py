@@ -332,6 +332,23 @@ def test_rec16_pack_rounds_to_nearest_even_and_matches_the_layout(B, W):
     assert np.array_equal(W.to_bf16(inp["amp"]), torch.from_numpy(inp["amp"]).to(torch.bfloat16).float().numpy())
 
 
+def test_rec16_pack_keeps_nan_and_inf(B, W):
+    """A NaN quaternion or amplitude must reach the record as a NaN (not as +-0, which is what add-and-shift rounding
+    makes of a NaN with low mantissa bits set), infinities as infinities: the pack kernel against W.to_bf16, whose special
+    cases tests/test_workloads_cpu.py spells out bit by bit."""
+    inp = W.make(2, 70)
+    special = np.array([0x7FFFFFFF, 0xFFFFFFFF, 0x7FC00000, 0x7F800001, 0xFF80FFFF, 0x7F800000, 0xFF800000, 0x7F7FFFFF,
+                        0xFF7FFFFF, 0x7F7F7FFF, 0x00000001, 0x80000000], dtype=np.uint32).view(np.float32)
+    inp["quat"] = inp["quat"].copy(); inp["amp"] = inp["amp"].copy()
+    inp["quat"].reshape(-1)[3:3 + special.size] = special
+    inp["amp"].reshape(-1)[5:5 + special.size] = special
+    d = to_dev(inp, NASG_KEYS)
+    rec = B.nasg_rec16_pack(d["means"], d["quat"], d["shape"], d["amp"], d["dc"]).cpu().numpy().view(np.uint32)
+    want = W.pack_records16(inp["means"], W.to_bf16(inp["quat"]), inp["shape"], W.to_bf16(inp["amp"]), inp["dc"])
+    assert np.array_equal(rec, want)
+    assert np.isnan(W.to_bf16(special[:5])).all() and np.isinf(W.to_bf16(special[5:9])).all()
+
+
 @pytest.mark.parametrize("cfg,N,mode", [(0, None, 1), (1, 70_001, 1), (2, 50_003, 1), (2, 50_016, 0), (4, 40_007, 1), (2, 2_101, 2)])
 def test_rec16_parity(B, W, oracle, cfg, N, mode):
     """The oracle evaluates the bf16-rounded values (promoted exactly): the arithmetic is fp32 as in nasg_rec_*, so the
