@@ -163,7 +163,8 @@ def run_reference(args, W, cfg):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": cfg.name, "sample_gaussians_per_step": n, "note": "fp64 CPU oracle as it stands"},
+            "config": {"workload": cfg.name, "N_per_gpu": cfg.N, "K": cfg.K, "C": cfg.C,
+                       "sample_gaussians_per_step": n, "note": "fp64 CPU oracle as it stands, on a bounded prefix sample of the same workload"},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": ref.num_threads(), "kind": "oracle",
                              "sample": f"{n} Gaussians of {cfg.name} per step"},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -184,6 +185,9 @@ class Resident:
         rcfg = S.weak_scaling_config(cfg, rank)
         self.cluster = 256 if layout == "rec_clustered" else 1            # labelled variant: spatially coherent visibility
         if layout == "rec_clustered":
+            layout = "rec"
+        self.repack = layout == "rec_repack"     # labelled variant: the caller keeps ROW arrays; pack before and unpack after, every step
+        if self.repack:
             layout = "rec"
         self.paper = cfg.kind == "nasg" and layout == "paper"          # the paper's own 3 + 9K record (nasg_paper_*)
         self.iso = int(layout[3]) if cfg.kind == "nasg" and layout.startswith("iso") else None    # isotropic Table-6 function (nasg_iso_*)
@@ -212,6 +216,11 @@ class Resident:
         elif self.rec:  # the parameters LIVE in HBM as records (packed once, outside any timed region: it is the storage layout)
             self.params = (B.nasg_rec16_pack if self.bf16 else B.nasg_rec_pack)(d["means"], d["quat"], d["shape"], d["amp"], d["dc"])
             self.g_params = torch.zeros(B.nasg_rec_floats(self.N, self.K), dtype=torch.float32, device="cuda")
+            if self.repack and not self.bf16:
+                self.rows = {k: d[k] for k in ("means", "quat", "shape", "amp", "dc")}
+                self.g_rows = {k: torch.empty_like(v) for k, v in self.rows.items()}
+            else:
+                self.repack = False
             for k in ("means", "quat", "shape", "amp", "dc"):
                 d[k] = None
         else:
@@ -227,6 +236,9 @@ class Resident:
         elif self.asg:
             B.nasg_asg_eval_fwd(self.params, self.N, self.K, d["campos"], d["vis"], out=self.colors, stream=st)
         elif self.rec:
+            if self.repack:
+                r = self.rows
+                B.nasg_rec_pack(r["means"], r["quat"], r["shape"], r["amp"], r["dc"], out=self.params, stream=st)
             (B.nasg_rec16_eval_fwd if self.bf16 else B.nasg_rec_eval_fwd)(self.params, self.N, self.K, d["campos"], d["vis"], self.norm_mode,
                                                                          out=self.colors, stream=st)
         elif self.cfg.kind == "sh":
@@ -247,6 +259,8 @@ class Resident:
         elif self.rec:
             (B.nasg_rec16_eval_bwd if self.bf16 else B.nasg_rec_eval_bwd)(self.params, self.N, self.K, d["campos"], d["g_colors"], d["vis"],
                                                                          self.norm_mode, out=self.g_params, stream=st)
+            if self.repack:
+                B.nasg_rec_unpack(self.g_params, self.N, self.K, stream=st, out=self.g_rows)
         elif self.cfg.kind == "sh":
             B.sh_eval_bwd(d["means"], d["coeffs"], d["campos"], d["g_colors"], d["vis"], out=self.grads, stream=st)
         else:
@@ -365,7 +379,7 @@ def run_ours(args, W, cfg):
 
     def summary(r, f_ms, b_ms):
         fb, bb = algorithmic_bytes(r.cfg.kind, r.K, r.C, r.has_vis, r.paper or r.asg, r.iso is not None, r.bf16)
-        return {"layout": "records; LABELLED VARIANT: visibility drawn per (camera, run of 256 Gaussians), spatially coherent" if r.cluster > 1 else "records, bf16 quaternion + amplitude (fp32 arithmetic and gradients)" if r.bf16 else "paper records (3 + 9K floats)" if r.paper else "Anisotropic Spherical Gaussian records (3 + 9K floats)" if r.asg else ("isotropic Table-6 records (3 + 7K floats): " + ("Spherical Gaussian", "Spherical Beta", "Spherical Cauchy")[r.iso]) if r.iso is not None else "records" if r.rec else "rows", "bytes_per_gaussian": [fb, bb], "kernel": r.kernel_name(), "fwd_ms": f_ms, "bwd_ms": b_ms,
+        return {"layout": "records, with nasg_rec_pack (row arrays -> records) inside fwd_ms and nasg_rec_unpack (gradient records -> row arrays) inside bwd_ms every step: what a caller who keeps row arrays pays; bytes_per_gaussian and the fractions count the evaluation's bytes only" if r.repack else "records; LABELLED VARIANT: visibility drawn per (camera, run of 256 Gaussians), spatially coherent" if r.cluster > 1 else "records, bf16 quaternion + amplitude (fp32 arithmetic and gradients)" if r.bf16 else "paper records (3 + 9K floats)" if r.paper else "Anisotropic Spherical Gaussian records (3 + 9K floats)" if r.asg else ("isotropic Table-6 records (3 + 7K floats): " + ("Spherical Gaussian", "Spherical Beta", "Spherical Cauchy")[r.iso]) if r.iso is not None else "records" if r.rec else "rows", "bytes_per_gaussian": [fb, bb], "kernel": r.kernel_name(), "fwd_ms": f_ms, "bwd_ms": b_ms,
                 "value": r.N / ((f_ms + b_ms) * 1e-3), "fwd_gbs": fb * r.N / (f_ms * 1e-3) / 1e9, "bwd_gbs": bb * r.N / (b_ms * 1e-3) / 1e9,
                 "bwd_frac": bb * r.N / (b_ms * 1e-3) / 1e9 / peak, "fwd+bwd_frac": (fb + bb) * r.N / ((f_ms + b_ms) * 1e-3) / 1e9 / peak}
 
@@ -375,15 +389,16 @@ def run_ours(args, W, cfg):
         f2, b2, t2 = R.timed(1000, 0, barrier)                 # ~0.5 s of back-to-back steps: the board's power cap bites
         extra["sustained"] = {"steps": 1000, "value": N * 1000 / (t2 * 1e-3), "fwd_ms": f2, "bwd_ms": b2}
         others = {}
-        main_summary = summary(R, fwd_ms, bwd_ms)
         specs = [(i, "rec") for i in (1, 2, 3, 4) if i != cfg.index]
         if rec:
             specs.append((cfg.index, "rows"))                  # the same workload through the row-array entry points
+            specs.append((cfg.index, "rec_repack"))            # ... and through the records with pack + unpack every step
         specs += [(i, "paper") for i in (1, 2, 4)]             # the paper's own 3 + 9K record (17 % fewer parameter bytes)
         specs.append((2, "rec_clustered"))                     # cfg2 with visibility constant over runs of 256 Gaussians (NOT the headline)
         specs += [(i, "rec16") for i in (1, 2, 4)]             # bf16 storage of quaternion and amplitude (NEXT-3)
         specs += [(2, "iso0"), (2, "iso1"), (2, "iso2"), (2, "asg")]       # the other Table-6 functions in the same skeleton (NEXT-3)
         R_keep, R = R, None
+        d = None                                               # (the local alias would keep the headline's tensors alive)
         if cfg.N > 2_000_000:
             R_keep.d = None; R_keep.params = None; R_keep.g_params = None; R_keep.colors = None
             torch.cuda.empty_cache()
@@ -437,6 +452,27 @@ def run_ours(args, W, cfg):
                                          "note": "diagnostic: executed instructions of the kernel as written (recorded ncu count) / issue slots at the sampled clock; packed f32x2 and MUFU instructions hold the issue port ~2 cycles (DESIGN.md section 7)"}
         if not args.no_cpu and world == 1:
             line["cpu_baseline"] = cpu_baseline(W, cfg)
+        if rec:
+            line["config"]["layout_contract"] = ("records are the PERSISTENT training layout: the optimiser updates parameter records in place from gradient "
+                                                 "records, and the means live planar in the record header (floats 0..95 of each tile), from where a projection "
+                                                 "stage reads them; no pack/unpack runs per step and none is inside `value`. A caller that keeps row arrays "
+                                                 "instead pays other_configs['cfg%d rec_repack'] or uses the row-array entry points (rows_value)" % cfg.index)
+        oc = extra.get("other_configs", {})
+        if oc:
+            # the figures north_star is judged on, short, as the LAST key of the line (so that a truncated tail still holds them):
+            # [fwd_ms, bwd_ms, bwd fraction of the measured HBM peak, Gaussians/s], 20-step bursts in this run
+            short = lambda k: [round(oc[k]["fwd_ms"], 4), round(oc[k]["bwd_ms"], 4), round(oc[k]["bwd_frac"], 3), float("%.4g" % oc[k]["value"])] if k in oc else None
+            rows_key, repack_key = "cfg%d rows" % cfg.index, "cfg%d rec_repack" % cfg.index
+            if rows_key in oc:
+                line["config"]["rows_value"] = oc[rows_key]["value"]
+            sh = oc.get("cfg3")
+            line["summary"] = {"headline": [round(fwd_ms, 4), round(bwd_ms, 4), round(achieved / peak, 3), float("%.4g" % value)],
+                               "sustained_value": float("%.4g" % extra["sustained"]["value"]),
+                               "rows": short(rows_key), "rec_repack": short(repack_key),
+                               "cfg1": short("cfg1"), "cfg3_sh": short("cfg3"), "cfg4": short("cfg4"),
+                               "cfg1_paper": short("cfg1 paper"), "cfg2_paper": short("cfg2 paper"), "cfg4_paper": short("cfg4 paper"),
+                               "nasg_over_sh": (round((fwd_ms + bwd_ms) / (sh["fwd_ms"] + sh["bwd_ms"]), 3) if sh and cfg.index == 2 else None),
+                               "format": "[fwd_ms, bwd_ms, bwd_frac_of_measured_hbm_peak, gaussians_per_s]; nasg_over_sh = t(cfg2 NASGabor fwd+bwd) / t(cfg3 SH-3 fwd+bwd), same N, C, mask"}
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

@@ -360,14 +360,17 @@ def nasg_rec_pack(means, quat, shape, amp, dc, out: Optional[torch.Tensor] = Non
     return out
 
 
-def nasg_rec_unpack(rec: torch.Tensor, N: int, K: int, stream=None) -> dict:
-    """Tile records (parameters or gradients) -> dict of row arrays means, quat, shape, amp, dc."""
+def nasg_rec_unpack(rec: torch.Tensor, N: int, K: int, stream=None, out: Optional[dict] = None) -> dict:
+    """Tile records (parameters or gradients) -> dict of row arrays means, quat, shape, amp, dc (written into `out` if given)."""
     f32 = torch.float32
     _chk(rec, "rec", (nasg_rec_floats(N, K),), f32, "cuda")
     dev = rec.device
-    out = dict(means=torch.empty((N, 3), dtype=f32, device=dev), quat=torch.empty((K, N, 4), dtype=f32, device=dev),
-               shape=torch.empty((K, N, 4), dtype=f32, device=dev), amp=torch.empty((K, 3, N), dtype=f32, device=dev),
-               dc=torch.empty((3, N), dtype=f32, device=dev))
+    if out is None:
+        out = dict(means=torch.empty((N, 3), dtype=f32, device=dev), quat=torch.empty((K, N, 4), dtype=f32, device=dev),
+                   shape=torch.empty((K, N, 4), dtype=f32, device=dev), amp=torch.empty((K, 3, N), dtype=f32, device=dev),
+                   dc=torch.empty((3, N), dtype=f32, device=dev))
+    for name, shp in (("means", (N, 3)), ("quat", (K, N, 4)), ("shape", (K, N, 4)), ("amp", (K, 3, N)), ("dc", (3, N))):
+        _chk(out[name], name, shp, f32, "cuda")
     rc = _lib.nasg_rec_unpack(N, K, _ptr(rec), _ptr(out["means"]), _ptr(out["quat"]), _ptr(out["shape"]), _ptr(out["amp"]),
                               _ptr(out["dc"]), _stream(stream))
     if rc != 0:
