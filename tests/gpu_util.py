@@ -100,24 +100,64 @@ def check_sh(B, oracle, inp: dict, want_campos=False, label=""):
     return col, g, errs
 
 
-def near_antipode(inp: dict, v_max: float = -0.99, lam_max: float = 4.0) -> np.ndarray:
-    """Gaussians with a visible (lobe, camera) evaluation close to d = -z of a broad lobe (d.z < v_max, lambda <= lam_max).
-    DESIGN.md R11: eq.(9) is discontinuous at d = -z (0 along the x meridian, e^{-2 lambda} along y), so next to it the
-    azimuth u/s decides the value and a relative perturbation of 6e-8 of the mean (one fp32 rounding) moves the gradients by
-    ~1e-4 of their size: no fp32 evaluation can be held to the tolerance there, the oracle's own result is that sensitive.
-    Returns a boolean [N] mask; the test that uses it reports how many Gaussians it excludes."""
-    q = np.asarray(inp["quat"], dtype=np.float64)
-    q = q / np.linalg.norm(q, axis=2, keepdims=True)
-    w, x, y, z = q[..., 0], q[..., 1], q[..., 2], q[..., 3]
-    Z = np.stack([2 * (x * z + w * y), 2 * (y * z - w * x), 1 - 2 * (x * x + y * y)], axis=2)           # [K,N,3], column 2 of R(q)
-    lam = np.exp(np.asarray(inp["shape"], dtype=np.float64)[..., 1])                                    # [K,N]
-    bad = np.zeros(q.shape[1], dtype=bool)
-    for c in range(inp["campos"].shape[0]):
-        d = np.asarray(inp["means"], dtype=np.float64) - np.asarray(inp["campos"], dtype=np.float64)[c]
-        d /= np.linalg.norm(d, axis=1, keepdims=True)
-        v = np.einsum("kni,ni->kn", Z, d)
-        hit = ((v < v_max) & (lam <= lam_max)).any(axis=0)
-        if inp.get("vis") is not None:
-            hit &= inp["vis"][c] != 0
-        bad |= hit
-    return bad
+# Gaussian axis of every gradient array (quaternion records and paper records)
+GAUSSIAN_AXIS = {"g_means": 0, "g_quat": 1, "g_shape": 1, "g_amp": 2, "g_dc": 1, "g_euler": 1, "g_shp": 1, "g_ampraw": 2}
+ULP_SENS_LIMIT = 0.25 * BWD_TOL
+
+
+def one_ulp(a: np.ndarray, rng: np.random.Generator) -> np.ndarray:
+    """Every element of an fp32 array moved to a neighbouring fp32 number, up or down at random."""
+    a = np.asarray(a, dtype=np.float32)
+    toward = np.where(rng.random(a.shape) < 0.5, np.float32(-np.inf), np.float32(np.inf)).astype(np.float32)
+    return np.nextafter(a, toward).astype(np.float32)
+
+
+def oracle_ulp_sensitivity(bwd, inp: dict, float_keys, ref_grads: dict, draws: int = 3, seed: int = 2024, scale: dict = None) -> np.ndarray:
+    """How far the ORACLE's own gradients of each Gaussian move when its fp32 inputs move by one unit in the last place.
+
+    `bwd(inp) -> dict` is the fp64 oracle's backward (ref.nasg_bwd / ref.paper_bwd, norm mode bound by the caller),
+    `float_keys` the fp32 input arrays to perturb (means, campos and every parameter array), `ref_grads` the oracle's
+    gradients on the unperturbed inputs (`scale`: max|g| per array if `inp` is a subset of a larger set). For each of `draws` seeded draws every element of every one of those arrays
+    is replaced by a neighbouring fp32 number (up or down at random) and the oracle is run again; Gaussians are
+    independent, so one run yields the response of all of them. Returns [N]: per Gaussian the largest
+    |g' - g| / max|g array| over all draws, gradient arrays and components, the same max-norm scale BWD_TOL is stated in.
+
+    Why it exists (R11): eq.(9) is discontinuous at d = -z (0 along the x meridian, e^{-2 lambda} along y).
+    Next to that point, for a broad and very anisotropic lobe, the azimuth decides the value, and a single rounding of
+    ONE input already moves the oracle's gradient by 3e-5 .. 5e-5 of the array's maximum (tests/test_oracle_conditioning.py
+    measures it). An fp32 evaluation, with a dozen roundings on the way to d.x, d.y, d.z, cannot be held to 1e-4 there by
+    any implementation. The parity tests that meet such Gaussians leave out exactly those whose response exceeds
+    ULP_SENS_LIMIT = 0.25 BWD_TOL, report how many they are, and bound their deviation by a multiple of this response."""
+    rng = np.random.default_rng(seed)
+    N = int(inp["N"])
+    if scale is None:
+        scale = {k: float(np.abs(v).max()) + 1e-300 for k, v in ref_grads.items() if k in GAUSSIAN_AXIS}
+    sens = np.zeros(N)
+    for _ in range(draws):
+        moved = dict(inp)
+        for k in float_keys:
+            moved[k] = one_ulp(inp[k], rng)
+        g = bwd(moved)
+        for k, sc in scale.items():
+            diff = np.abs(g[k] - ref_grads[k])
+            axes = tuple(i for i in range(diff.ndim) if i != GAUSSIAN_AXIS[k])
+            np.maximum(sens, diff.max(axis=axes) / sc, out=sens)
+    return sens
+
+
+def split_by_conditioning(got: dict, ref_grads: dict, sens: np.ndarray, pairs) -> dict:
+    """Max-norm errors of every gradient array over the well-conditioned Gaussians (sens <= ULP_SENS_LIMIT), and for the
+    others the largest ratio of a Gaussian's own deviation to its own oracle response. `pairs`: (oracle key, got key)."""
+    keep = sens <= ULP_SENS_LIMIT
+    out = {"excluded": int((~keep).sum()), "worst_ratio": 0.0}
+    for gk, pk in pairs:
+        a = got[pk].detach().cpu().numpy() if isinstance(got[pk], torch.Tensor) else np.asarray(got[pk])
+        b = ref_grads[gk]
+        assert np.all(np.isfinite(a)), gk
+        ax = GAUSSIAN_AXIS[gk]
+        per_n = np.abs(a - b).max(axis=tuple(i for i in range(b.ndim) if i != ax)) / (np.abs(b).max() + 1e-300)    # [N]
+        out[gk] = float(per_n[keep].max())
+        out[gk + "(all)"] = float(per_n.max())
+        if (~keep).any():
+            out["worst_ratio"] = max(out["worst_ratio"], float((per_n[~keep] / sens[~keep]).max()))
+    return out
