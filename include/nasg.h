@@ -218,6 +218,38 @@ size_t nasg_asg_floats(int64_t N, int32_t K);
 int nasg_asg_eval_fwd(const nasg_rec_inputs *in, float *colors, void *cuda_stream);
 int nasg_asg_eval_bwd(const nasg_rec_inputs *in, const float *g_colors, float *g_params, void *cuda_stream);
 
+/* ---- building and decoding records of EVERY kind from C (no Python helper needed) ------------------------------------
+ * All record kinds share one skeleton: [T][6 + M K][32] floats, T = ceil(N / 32), the 192-float header (means planar,
+ * dc planar) and then, per lobe pair j, M components of 64 floats each: float [192 + 64 M j + 64 c + 2 lane + h] is
+ * component c of lobe 2 j + h of Gaussian 32 t + lane. The kinds differ in M and in what the components are:
+ *     NASG_KIND_QUAT   0   M = 11   q_w q_x q_y q_z | log Lambda, log lambda, k, phi | w_r w_g w_b        (nasg_rec_*)
+ *     NASG_KIND_PAPER  1   M =  9   raw theta, phi, tau | raw lambda, a, k | raw w_r w_g w_b                (nasg_paper_*)
+ *     NASG_KIND_ISO    2   M =  7   axis x y z | raw shape | w_r w_g w_b                                    (nasg_iso_*)
+ *     NASG_KIND_ASG    4   M =  9   q_w q_x q_y q_z | raw mu, raw lambda | w_r w_g w_b                      (nasg_asg_*)
+ * nasg_kind_pack builds such a record array from means [N,3], dc [3,N] and ONE row array comp [K,N,M] that holds the M
+ * components of every lobe in the order above (note: the amplitude sits per lobe row here, not planar as nasg_inputs.amp).
+ * Padding lanes of the last record are written as zeros, except a 1 in q_w (kinds 0, 4) or axis z (kind 2), so that the
+ * never-stored padding lanes divide by nothing. nasg_kind_unpack is the inverse, for parameter and gradient records alike
+ * (any output pointer may be NULL = skip). nasg_rec16_unpack decodes the bf16 parameter record of nasg_rec16_pack into
+ * fp32 row arrays (exact; shapes as nasg_inputs; any output may be NULL); the gradient record of the bf16 kind is a
+ * kind-0 record. A bad kind returns NASG_ERR_NORM_MODE; K must be 2, 4 or 8; rec must be 16-byte aligned. Device pointers,
+ * asynchronous on cuda_stream, nothing allocated. These kernels re-order only and are not tuned: records are the
+ * persistent layout, conversion is not a per-step operation.
+ * The host-buffer end-to-end calls below exist for the quaternion and the paper record only; the isotropic, ASG and bf16
+ * kinds are device-only by design (their records are built on the device with the calls above and stay there). */
+#define NASG_KIND_QUAT  0
+#define NASG_KIND_PAPER 1
+#define NASG_KIND_ISO   2
+#define NASG_KIND_ASG   4
+int32_t nasg_kind_components(int kind);                          /* M, or 0 for an unknown kind */
+size_t nasg_kind_floats(int kind, int64_t N, int32_t K);        /* floats of a record array (= nasg_rec/paper/iso/asg_floats) */
+int nasg_kind_pack(int kind, int64_t N, int32_t K, const float *means, const float *dc, const float *comp, float *rec,
+                   void *cuda_stream);
+int nasg_kind_unpack(int kind, int64_t N, int32_t K, const float *rec, float *means, float *dc, float *comp,
+                     void *cuda_stream);
+int nasg_rec16_unpack(int64_t N, int32_t K, const float *rec16, float *means, float *quat, float *shape, float *amp,
+                      float *dc, void *cuda_stream);
+
 /* End-to-end with HOST buffers, as nasg_eval_fwd_bwd_host below: params / g_params are HOST record arrays, campos, vis,
  * g_colors, colors HOST arrays. A chunk of Gaussians is a contiguous block of records, so each chunk moves with one
  * copy per direction for the parameters / gradients plus one strided copy each for vis, g_colors and colors. Padding

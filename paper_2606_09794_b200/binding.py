@@ -29,7 +29,8 @@ SYMBOLS = ("nasg_eval_fwd", "nasg_eval_bwd", "sh_eval_fwd", "sh_eval_bwd", "nasg
            "nasg_iso_floats", "nasg_iso_eval_fwd", "nasg_iso_eval_bwd",
            "nasg_asg_floats", "nasg_asg_eval_fwd", "nasg_asg_eval_bwd",
            "nasg_rec16_floats", "nasg_rec16_pack", "nasg_rec16_eval_fwd", "nasg_rec16_eval_bwd",
-           "nasg_noalloc_workspace_bytes", "nasg_eval_bwd_noalloc")
+           "nasg_noalloc_workspace_bytes", "nasg_eval_bwd_noalloc",
+           "nasg_kind_components", "nasg_kind_floats", "nasg_kind_pack", "nasg_kind_unpack", "nasg_rec16_unpack")
 
 
 class NasgError(RuntimeError):
@@ -115,6 +116,15 @@ def _load():
     lib.nasg_paper_floats.restype = sz
     lib.nasg_paper_eval_fwd.argtypes = [C.POINTER(_RecInputs), vp, C.c_int, vp]
     lib.nasg_paper_eval_bwd.argtypes = [C.POINTER(_RecInputs), vp, vp, C.c_int, vp]
+    lib.nasg_kind_components.argtypes = [C.c_int]
+    lib.nasg_kind_components.restype = i32
+    lib.nasg_kind_floats.argtypes = [C.c_int, i64, i32]
+    lib.nasg_kind_floats.restype = sz
+    lib.nasg_kind_pack.argtypes = [C.c_int, i64, i32, vp, vp, vp, vp, vp]
+    lib.nasg_kind_unpack.argtypes = [C.c_int, i64, i32, vp, vp, vp, vp, vp]
+    lib.nasg_rec16_unpack.argtypes = [i64, i32, vp, vp, vp, vp, vp, vp, vp]
+    for name in ("nasg_kind_pack", "nasg_kind_unpack", "nasg_rec16_unpack"):
+        getattr(lib, name).restype = C.c_int
     lib.nasg_rec_host_scratch_bytes.argtypes = [i64, i32, i32]
     lib.nasg_rec_host_scratch_bytes.restype = sz
     lib.nasg_rec_eval_fwd_bwd_host.argtypes = [C.POINTER(_RecInputs), vp, vp, vp, C.c_int, vp, sz, vp]
@@ -598,4 +608,61 @@ def nasg_rec16_eval_bwd(params, N: int, K: int, campos, g_colors, vis=None, norm
     rc = _lib.nasg_rec16_eval_bwd(C.byref(inp), _ptr(g_colors), _ptr(out), int(norm_mode), _stream(stream))
     if rc != 0:
         raise NasgError(rc, "nasg_rec16_eval_bwd")
+    return out
+
+
+# ---- records of every kind from row arrays and back (include/nasg.h: nasg_kind_*) -----------------------
+KIND_QUAT, KIND_PAPER, KIND_ISO, KIND_ASG = 0, 1, 2, 4
+
+
+def nasg_kind_components(kind: int) -> int:
+    return int(_lib.nasg_kind_components(int(kind)))
+
+
+def nasg_kind_floats(kind: int, N: int, K: int) -> int:
+    return int(_lib.nasg_kind_floats(int(kind), N, K))
+
+
+def nasg_kind_pack(kind: int, means, dc, comp, out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    """means [N,3], dc [3,N], comp [K,N,M] (the M components of every lobe in the kind's order) -> record array."""
+    f32 = torch.float32
+    K, N, M = (int(x) for x in comp.shape)
+    _chk(means, "means", (N, 3), f32, "cuda"); _chk(dc, "dc", (3, N), f32, "cuda"); _chk(comp, "comp", (K, N, M), f32, "cuda")
+    if M != nasg_kind_components(kind):
+        raise ValueError(f"comp has {M} components per lobe, kind {kind} has {nasg_kind_components(kind)}")
+    nf = nasg_kind_floats(kind, N, K)
+    if out is None:
+        out = torch.empty(nf, dtype=f32, device=means.device)
+    _chk(out, "rec", (nf,), f32, "cuda")
+    rc = _lib.nasg_kind_pack(int(kind), N, K, _ptr(means), _ptr(dc), _ptr(comp), _ptr(out), _stream(stream))
+    if rc != 0:
+        raise NasgError(rc, "nasg_kind_pack")
+    return out
+
+
+def nasg_kind_unpack(kind: int, rec: torch.Tensor, N: int, K: int, stream=None) -> dict:
+    """Record array (parameters or gradients) of a kind -> dict means [N,3], dc [3,N], comp [K,N,M]."""
+    f32 = torch.float32
+    M = nasg_kind_components(kind)
+    _chk(rec, "rec", (nasg_kind_floats(kind, N, K),), f32, "cuda")
+    out = dict(means=torch.empty((N, 3), dtype=f32, device=rec.device), dc=torch.empty((3, N), dtype=f32, device=rec.device),
+               comp=torch.empty((K, N, M), dtype=f32, device=rec.device))
+    rc = _lib.nasg_kind_unpack(int(kind), N, K, _ptr(rec), _ptr(out["means"]), _ptr(out["dc"]), _ptr(out["comp"]), _stream(stream))
+    if rc != 0:
+        raise NasgError(rc, "nasg_kind_unpack")
+    return out
+
+
+def nasg_rec16_unpack(rec16: torch.Tensor, N: int, K: int, stream=None) -> dict:
+    """bf16 parameter record (nasg_rec16_pack) -> fp32 row arrays means, quat, shape, amp, dc (exact)."""
+    f32 = torch.float32
+    _chk(rec16, "rec16", (nasg_rec16_floats(N, K),), f32, "cuda")
+    dev = rec16.device
+    out = dict(means=torch.empty((N, 3), dtype=f32, device=dev), quat=torch.empty((K, N, 4), dtype=f32, device=dev),
+               shape=torch.empty((K, N, 4), dtype=f32, device=dev), amp=torch.empty((K, 3, N), dtype=f32, device=dev),
+               dc=torch.empty((3, N), dtype=f32, device=dev))
+    rc = _lib.nasg_rec16_unpack(N, K, _ptr(rec16), _ptr(out["means"]), _ptr(out["quat"]), _ptr(out["shape"]), _ptr(out["amp"]),
+                                _ptr(out["dc"]), _stream(stream))
+    if rc != 0:
+        raise NasgError(rc, "nasg_rec16_unpack")
     return out

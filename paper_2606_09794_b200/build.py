@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 SOURCES = [os.path.join(CSRC, f) for f in ("nasg_api.cu", "nasg_kernels.cu", "nasg_pipe_kernels.cu", "nasg_tile_kernels.cu", "nasg_rec_kernels.cu", "sh_kernels.cu",
-                                               "sh_pipe_kernels.cu", "nasg_host_pipeline.cu", "nasg_noalloc.cu")]
+                                               "sh_pipe_kernels.cu", "nasg_host_pipeline.cu", "nasg_noalloc.cu", "nasg_rec_convert.cu")]
 HEADERS = [os.path.join(CSRC, f) for f in ("nasg_internal.h", "nasg_math.cuh", "nasg_lp_math.cuh", "bulk_common.cuh", "pipe_common.cuh", "sh_math.cuh")] + [
     os.path.join(ROOT, "include", "nasg.h")]
 LIB = os.path.join(HERE, "libnasg_b200.so")

@@ -80,6 +80,24 @@ def test_error_codes_without_gpu(B):
     assert noalloc(inputs(N=256 * 21845 + 1, K=4, Cn=4), g) == -8               # one more row does not: NOALLOC_SIZE
     assert noalloc(inputs(N=256 * 87381 + 1, K=2, Cn=1), g) == -8
     assert "nasg_eval_bwd" in B.nasg_strerror(-8)
+    # nasg_kind_* (records of every kind from C): sizes and argument checks
+    from paper_2606_09794_b200 import workloads as W
+    assert [B.nasg_kind_components(k) for k in (0, 1, 2, 4, 3, 5, -1)] == [11, 9, 7, 9, 0, 0, 0]
+    for n, k in ((1, 2), (4_099, 4), (3_000_000, 8)):
+        assert B.nasg_kind_floats(0, n, k) == B.nasg_rec_floats(n, k) == W.rec_floats(n, k)
+        assert B.nasg_kind_floats(1, n, k) == B.nasg_paper_floats(n, k) == W.paper_rec_floats(n, k)
+        assert B.nasg_kind_floats(2, n, k) == B.nasg_iso_floats(n, k) == W.iso_rec_floats(n, k)
+        assert B.nasg_kind_floats(4, n, k) == B.nasg_asg_floats(n, k) == W.asg_rec_floats(n, k)
+    assert B.nasg_kind_floats(3, 100, 4) == 0 and B.nasg_kind_floats(0, 100, 3) == 0
+    lib.nasg_kind_pack.argtypes = [C.c_int, C.c_int64, C.c_int32] + [C.c_void_p] * 5
+    lib.nasg_kind_unpack.argtypes = [C.c_int, C.c_int64, C.c_int32] + [C.c_void_p] * 5
+    lib.nasg_rec16_unpack.argtypes = [C.c_int64, C.c_int32] + [C.c_void_p] * 7
+    assert lib.nasg_kind_pack(3, 4, 2, p, p, p, p, None) == -7                    # unknown kind
+    assert lib.nasg_kind_pack(0, 4, 3, p, p, p, p, None) == -3 and lib.nasg_kind_pack(0, -1, 2, p, p, p, p, None) == -2
+    assert lib.nasg_kind_pack(1, 4, 2, p, None, p, p, None) == -1 and lib.nasg_kind_pack(1, 4, 2, p, p, p, p + 4, None) == -4
+    assert lib.nasg_kind_pack(2, 0, 2, None, None, None, None, None) == 0         # N == 0 is a no-op
+    assert lib.nasg_kind_unpack(5, 4, 2, p, p, p, p, None) == -7 and lib.nasg_kind_unpack(4, 4, 2, None, p, p, p, None) == -1
+    assert lib.nasg_rec16_unpack(4, 5, p, p, p, p, p, p, None) == -3 and lib.nasg_rec16_unpack(4, 2, None, p, p, p, p, p, None) == -1
     for code in (0, -1, -2, -3, -4, -5, -7, -8):
         assert B.nasg_strerror(code) and "unknown" not in B.nasg_strerror(code)
     assert "unknown" in B.nasg_strerror(-99)
