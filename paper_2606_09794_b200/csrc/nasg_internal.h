@@ -87,7 +87,7 @@ cudaError_t launch_nasg_bwd(const BwdParams &p, int K, int mode, cudaStream_t st
 // fast path (nasg_pipe_kernels.cu): C <= 4, persistent threads, cp.async lobe ring
 cudaError_t launch_nasg_fwd_pipe(const FwdParams &p, int K, int mode, cudaStream_t st);
 cudaError_t launch_nasg_bwd_pipe(const BwdParams &p, int K, int mode, cudaStream_t st, int *grid_out);   // grid_out: blocks launched (= rows of cam_partial)
-// headline path (nasg_tile_kernels.cu): even K, C <= 4, aligned rows, no g_campos: lobe pairs on packed f32x2, TMA bulk-copy tiles
+// row arrays, tile kernels (nasg_tile_kernels.cu): even K, C <= 4, aligned rows, no g_campos: lobe pairs on packed f32x2, TMA bulk-copy tiles
 bool tile_path_ok(int64_t N, int K, int C, const void *means, const void *amp, const void *planar, const void *rows, const void *vis);
 cudaError_t launch_nasg_fwd_tile(const FwdParams &p, int K, int mode, cudaStream_t st);
 cudaError_t launch_nasg_bwd_tile(const BwdParams &p, int K, int mode, cudaStream_t st);

@@ -1,4 +1,5 @@
-// nasg_tile_kernels.cu — the headline path of the NASGabor kernels (sm_100a): even lobe counts (K = 2, 4, 8),
+// nasg_tile_kernels.cu — the tile kernels of the ROW-ARRAY entry points nasg_eval_fwd / nasg_eval_bwd (sm_100a; the
+// headline path is the record family of nasg_rec_kernels.cu, which this file preceded): even lobe counts (K = 2, 4, 8),
 // C <= 4 cameras, N a multiple of 4 (16 with a visibility mask) and 16-byte aligned arrays. Everything else
 // (odd K, C > 4, ragged N, misaligned views, g_campos, small N) runs the cp.async ring kernels of
 // nasg_pipe_kernels.cu or the generic kernels of nasg_kernels.cu.
